@@ -1,0 +1,119 @@
+/*
+ * streamkl.h -- C ABI of the B200-native StreamKL hot path (arxiv/paper_2606_20005).
+ *
+ * The operation.  For every (batch b, head h) and query row i, with logits
+ *     s_t[j] = c_t * <Q_t[b,h,i,:], K_t[b,h,j,:]>,   t in {1,2}          (sqrt(d) scale = c_t)
+ * over the visible keys V_i (all keys, or causal j <= i + (NK-NQ)), the library computes
+ *     lse_t[i] = log sum_{j in V_i} exp(s_t[j])                             (Eq.4)
+ *     kl[i]    = KL(P1 || P2) = sum_j P1[j] (log P1[j] - log P2[j])         (Eq.1)
+ * in ONE streaming pass over key tiles via  kl = acc/l1 + lse2 - lse1,  acc = sum_j e^{s1-m1}(s1-s2)
+ * (Eq.8; Algorithm 1; rescaling invariant Eq.9-10),
+ * and, in the backward pass, by tile-wise recomputation from the saved lse:
+ *     dS2 = g (P2 - P1)                      -> dQ2 = c2 dS2 K2,  dK2 = c2 dS2^T Q2   (Eq.2 :64; Alg.2 :224-234; :294)
+ *     dS1 = g P1 ((s1-s2) - (lse1-lse2) - kl) -> dQ1 = c1 dS1 K1,  dK1 = c1 dS1^T Q1   (Eq.3 :69; Eq.12 :304; Alg.3 :255-286; :309)
+ * with g = dkl_rows[i] the upstream gradient (dL in Alg.2/3).  No N_Q x N_K intermediate is ever written to HBM.
+ *
+ * Conventions (all entry points):
+ *  - Tensors are contiguous row-major [B][H][N][d] ("bsz" = B*H flattened); per-row vectors are
+ *    [B][H][NQ] float32.  Outputs are in natural-log units.  Same H for all four tensors (no GQA).
+ *  - `*_bf16` / `*_f32` name the element type of Q1,K1,Q2,K2 and of the gradient outputs (one rounding from
+ *    fp32 accumulators).  All accumulation is fp32.  bf16 with d1,d2 in {64,128} runs the tcgen05/TMA kernels;
+ *    every other case (fp32 inputs, other head dims <= 256) runs the SIMT fp32 kernels.
+ *  - Device entry points take DEVICE pointers owned by the caller; the library never allocates, frees or
+ *    retains them, and only enqueues work on `stream` (asynchronous; device faults surface at the caller's next
+ *    synchronisation).  `*_host` entry points take HOST pointers, allocate their own device scratch, copy in,
+ *    run, copy back and synchronise before returning.
+ *  - Return value: 0 (STREAMKL_OK) or a negative STREAMKL_ERR_* code.  A failed call enqueues nothing and
+ *    writes nothing.  The library never throws, prints or exits.  There is no CPU fallback: on a machine without
+ *    an sm_100 GPU every compute entry point returns STREAMKL_ERR_CUDA.
+ *  - Thread-safe for concurrent calls on distinct streams.
+ *  - Shapes: B,H >= 0 (B*H == 0 or NQ == 0 is a successful no-op), NK >= 1, 1 <= d1,d2 <= 256,
+ *    causal requires NQ <= NK (bottom-right aligned mask; rows would otherwise have empty support).
+ *    c1,c2 must be finite and > 0.  Pointers must be 16-byte aligned (TMA).
+ */
+#ifndef STREAMKL_H_
+#define STREAMKL_H_
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* A CUDA stream handle (cudaStream_t / CUstream) passed as an opaque pointer; NULL = the legacy default stream. */
+typedef void* streamkl_stream_t;
+
+enum {
+  STREAMKL_OK = 0,
+  STREAMKL_ERR_NULLPTR = -1,   /* a required pointer is NULL */
+  STREAMKL_ERR_SHAPE = -2,     /* negative size, NK < 1, d out of range, causal with NQ > NK, B*H*N overflow */
+  STREAMKL_ERR_ALIGN = -3,     /* a tensor pointer is not 16-byte aligned */
+  STREAMKL_ERR_SCALE = -4,     /* c1 or c2 is not finite and > 0 */
+  STREAMKL_ERR_WORKSPACE = -5, /* workspace NULL or smaller than streamkl_bwd_workspace_bytes() */
+  STREAMKL_ERR_CUDA = -6,      /* no sm_100 device, tensor-map encode / launch / copy / allocation failure */
+  STREAMKL_ERR_DTYPE = -7      /* unknown dtype code */
+};
+
+enum { STREAMKL_BF16 = 0, STREAMKL_F32 = 1 };
+
+/*
+ * Forward (Algorithm 1).  Device pointers.
+ *   Q1 [B][H][NQ][d1], K1 [B][H][NK][d1], Q2 [B][H][NQ][d2], K2 [B][H][NK][d2]  -- read only, `dtype` elements
+ *   kl_rows, lse1, lse2 [B][H][NQ] float32 -- overwritten (the 3*NQ scalars of PAPER.md:216-218)
+ * Extra HBM: none (O(NQ) outputs only).
+ */
+int streamkl_fwd(const void* Q1, const void* K1, const void* Q2, const void* K2,
+                 int B, int H, int NQ, int NK, int d1, int d2, float c1, float c2, int causal,
+                 float* kl_rows, float* lse1, float* lse2, streamkl_stream_t stream);          /* bf16 inputs */
+int streamkl_fwd_f32(const void* Q1, const void* K1, const void* Q2, const void* K2,
+                     int B, int H, int NQ, int NK, int d1, int d2, float c1, float c2, int causal,
+                     float* kl_rows, float* lse1, float* lse2, streamkl_stream_t stream);      /* fp32 inputs */
+
+/*
+ * Backward (Algorithms 2/3 and their K-tile-owner transposes).
+ *   kl_rows, lse1, lse2 : the forward's outputs;  dkl_rows [B][H][NQ] float32 upstream gradient (required).
+ *   dQ2 [B][H][NQ][d2], dK2 [B][H][NK][d2] : required, OVERWRITTEN (not accumulated), input dtype.
+ *   dQ1 [B][H][NQ][d1], dK1 [B][H][NK][d1] : both NULL => teacher frozen (Setting 1 only); both non-NULL =>
+ *                                            Setting 2 gradients too.  Exactly one NULL is STREAMKL_ERR_NULLPTR.
+ *   workspace : device scratch of at least streamkl_bwd_workspace_bytes(...) bytes (may be NULL when that is 0).
+ * dK is accumulated atomic-free by K-tile ownership; dQ by Q-tile ownership (deterministic, no atomics).
+ */
+int streamkl_bwd(const void* Q1, const void* K1, const void* Q2, const void* K2,
+                 int B, int H, int NQ, int NK, int d1, int d2, float c1, float c2, int causal,
+                 const float* kl_rows, const float* lse1, const float* lse2, const float* dkl_rows,
+                 void* dQ1, void* dK1, void* dQ2, void* dK2,
+                 void* workspace, size_t workspace_bytes, streamkl_stream_t stream);           /* bf16 */
+int streamkl_bwd_f32(const void* Q1, const void* K1, const void* Q2, const void* K2,
+                     int B, int H, int NQ, int NK, int d1, int d2, float c1, float c2, int causal,
+                     const float* kl_rows, const float* lse1, const float* lse2, const float* dkl_rows,
+                     void* dQ1, void* dK1, void* dQ2, void* dK2,
+                     void* workspace, size_t workspace_bytes, streamkl_stream_t stream);       /* fp32 */
+
+/* Bytes of device scratch streamkl_bwd needs for this shape (O((NQ+NK)*d) at most, never O(NQ*NK)). */
+size_t streamkl_bwd_workspace_bytes(int B, int H, int NQ, int NK, int d1, int d2, int want_teacher_grads);
+
+/*
+ * End-to-end variants with HOST buffers (same argument meaning; `dtype` = STREAMKL_BF16 | STREAMKL_F32).
+ * They cudaMalloc scratch for inputs/outputs, copy host->device, run the kernels above, copy device->host,
+ * free, and synchronise `stream` before returning.  Host buffers may be pageable or pinned.
+ * streamkl_fwd_bwd_host runs forward then backward on the same resident inputs (one "step" of the hot path);
+ * pass dQ1 = dK1 = NULL for Setting 1 only.
+ */
+int streamkl_fwd_host(int dtype, const void* Q1, const void* K1, const void* Q2, const void* K2,
+                      int B, int H, int NQ, int NK, int d1, int d2, float c1, float c2, int causal,
+                      float* kl_rows, float* lse1, float* lse2, streamkl_stream_t stream);
+int streamkl_fwd_bwd_host(int dtype, const void* Q1, const void* K1, const void* Q2, const void* K2,
+                          int B, int H, int NQ, int NK, int d1, int d2, float c1, float c2, int causal,
+                          const float* dkl_rows, float* kl_rows, float* lse1, float* lse2,
+                          void* dQ1, void* dK1, void* dQ2, void* dK2, streamkl_stream_t stream);
+
+/* Number of kernels the last successful streamkl_* call on this thread launched (for launch accounting). */
+int streamkl_last_launch_count(void);
+
+const char* streamkl_strerror(int code);
+const char* streamkl_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* STREAMKL_H_ */

@@ -1,0 +1,19 @@
+"""paper_2606_20005_b200 -- B200-native StreamKL (fused attention-KL forward/backward, arxiv/paper_2606_20005).
+
+The product is the C-ABI library `libstreamkl.so` (declared in include/streamkl.h, built from csrc/ for
+sm_100a).  This package is the thin Python binding: argument marshalling only, every step of the hot path
+runs in the CUDA kernels.  There is no CPU fallback -- importing the binding without the built library raises.
+"""
+from .binding import (  # noqa: F401
+    StreamKLError,
+    lib,
+    lib_path,
+    streamkl_bwd,
+    streamkl_bwd_workspace_bytes,
+    streamkl_fwd,
+    streamkl_fwd_bwd_host,
+    streamkl_fwd_host,
+    streamkl_last_launch_count,
+    streamkl_strerror,
+    streamkl_version,
+)

@@ -1,0 +1,254 @@
+"""ctypes binding of libstreamkl.so -- same names as include/streamkl.h, argument marshalling only.
+
+Device entry points take torch CUDA tensors (torch supplies device memory and the current stream, nothing
+else); `*_host` entry points take numpy arrays (bf16 carried as uint16 bit patterns, or float32).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+from .build import LIB_PATH
+
+__all__ = [
+    "StreamKLError", "lib", "lib_path", "streamkl_fwd", "streamkl_bwd", "streamkl_bwd_workspace_bytes",
+    "streamkl_fwd_host", "streamkl_fwd_bwd_host", "streamkl_last_launch_count", "streamkl_strerror",
+    "streamkl_version",
+]
+
+STREAMKL_BF16, STREAMKL_F32 = 0, 1
+
+
+class StreamKLError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__(f"{where}: {streamkl_strerror(code)} (code {code})")
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return LIB_PATH
+
+
+def lib() -> ctypes.CDLL:
+    """Load libstreamkl.so (built in-tree by `python -m paper_2606_20005_b200.build`).  Fails loudly if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2606_20005_b200.build` "
+            "(there is no CPU fallback for the StreamKL hot path)")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, ci, cf, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_float, ctypes.c_size_t
+    shape = [ci] * 6 + [cf, cf, ci]  # B,H,NQ,NK,d1,d2,c1,c2,causal
+    for name in ("streamkl_fwd", "streamkl_fwd_f32"):
+        f = getattr(L, name)
+        f.argtypes = [vp] * 4 + shape + [vp] * 3 + [vp]
+        f.restype = ci
+    for name in ("streamkl_bwd", "streamkl_bwd_f32"):
+        f = getattr(L, name)
+        f.argtypes = [vp] * 4 + shape + [vp] * 4 + [vp] * 4 + [vp, sz, vp]
+        f.restype = ci
+    L.streamkl_bwd_workspace_bytes.argtypes = [ci] * 7
+    L.streamkl_bwd_workspace_bytes.restype = sz
+    L.streamkl_fwd_host.argtypes = [ci] + [vp] * 4 + shape + [vp] * 3 + [vp]
+    L.streamkl_fwd_host.restype = ci
+    L.streamkl_fwd_bwd_host.argtypes = [ci] + [vp] * 4 + shape + [vp] + [vp] * 3 + [vp] * 4 + [vp]
+    L.streamkl_fwd_bwd_host.restype = ci
+    L.streamkl_last_launch_count.argtypes = []
+    L.streamkl_last_launch_count.restype = ci
+    L.streamkl_strerror.argtypes = [ci]
+    L.streamkl_strerror.restype = ctypes.c_char_p
+    L.streamkl_version.argtypes = []
+    L.streamkl_version.restype = ctypes.c_char_p
+    _lib = L
+    return L
+
+
+def streamkl_strerror(code: int) -> str:
+    return lib().streamkl_strerror(int(code)).decode()
+
+
+def streamkl_version() -> str:
+    return lib().streamkl_version().decode()
+
+
+def streamkl_last_launch_count() -> int:
+    return int(lib().streamkl_last_launch_count())
+
+
+def streamkl_bwd_workspace_bytes(B, H, NQ, NK, d1, d2, want_teacher_grads) -> int:
+    return int(lib().streamkl_bwd_workspace_bytes(B, H, NQ, NK, d1, d2, int(bool(want_teacher_grads))))
+
+
+# ------------------------------------------------------------------------------------------ device entry points
+def _check_dev(name, t, dtype=None):
+    import torch
+
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or not t.is_contiguous():
+        raise TypeError(f"{name}: expected a contiguous CUDA torch tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError(f"{name}: expected dtype {dtype}, got {t.dtype}")
+
+
+def _shape_of(Q1, K1, Q2, K2):
+    if Q1.dim() != 4 or K1.dim() != 4 or Q2.dim() != 4 or K2.dim() != 4:
+        raise ValueError("Q1,K1,Q2,K2 must be [B,H,N,d]")
+    B, H, NQ, d1 = Q1.shape
+    NK, d2 = K1.shape[2], Q2.shape[3]
+    if tuple(K1.shape) != (B, H, NK, d1) or tuple(Q2.shape) != (B, H, NQ, d2) or tuple(K2.shape) != (B, H, NK, d2):
+        raise ValueError("inconsistent Q1,K1,Q2,K2 shapes")
+    return B, H, NQ, NK, d1, d2
+
+
+def _stream_handle(stream):
+    import torch
+
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return ctypes.c_void_p(stream.cuda_stream)
+
+
+def _ptr(t):
+    return ctypes.c_void_p(t.data_ptr()) if t is not None else ctypes.c_void_p(0)
+
+
+def streamkl_fwd(Q1, K1, Q2, K2, c1, c2, causal, kl_rows=None, lse1=None, lse2=None, stream=None):
+    """Forward (Algorithm 1).  Returns (kl_rows, lse1, lse2), each [B,H,NQ] float32.  bf16 or fp32 inputs."""
+    import torch
+
+    for n, t in (("Q1", Q1), ("K1", K1), ("Q2", Q2), ("K2", K2)):
+        _check_dev(n, t, Q1.dtype)
+    B, H, NQ, NK, d1, d2 = _shape_of(Q1, K1, Q2, K2)
+    outs = []
+    for n, t in (("kl_rows", kl_rows), ("lse1", lse1), ("lse2", lse2)):
+        if t is None:
+            t = torch.empty((B, H, NQ), dtype=torch.float32, device=Q1.device)
+        _check_dev(n, t, torch.float32)
+        outs.append(t)
+    if Q1.dtype == torch.bfloat16:
+        fn = lib().streamkl_fwd
+    elif Q1.dtype == torch.float32:
+        fn = lib().streamkl_fwd_f32
+    else:
+        raise TypeError("inputs must be bfloat16 or float32")
+    with torch.cuda.device(Q1.device):
+        rc = fn(_ptr(Q1), _ptr(K1), _ptr(Q2), _ptr(K2), B, H, NQ, NK, d1, d2, float(c1), float(c2), int(bool(causal)),
+                _ptr(outs[0]), _ptr(outs[1]), _ptr(outs[2]), _stream_handle(stream))
+    if rc != 0:
+        raise StreamKLError(rc, "streamkl_fwd")
+    return tuple(outs)
+
+
+def streamkl_bwd(Q1, K1, Q2, K2, c1, c2, causal, kl_rows, lse1, lse2, dkl_rows, teacher=False,
+                 dQ1=None, dK1=None, dQ2=None, dK2=None, workspace=None, stream=None):
+    """Backward by recomputation (Alg.2/3 + K-owner transposes).  Returns (dQ1, dK1, dQ2, dK2); dQ1,dK1 None unless teacher."""
+    import torch
+
+    for n, t in (("Q1", Q1), ("K1", K1), ("Q2", Q2), ("K2", K2)):
+        _check_dev(n, t, Q1.dtype)
+    for n, t in (("kl_rows", kl_rows), ("lse1", lse1), ("lse2", lse2), ("dkl_rows", dkl_rows)):
+        _check_dev(n, t, torch.float32)
+    B, H, NQ, NK, d1, d2 = _shape_of(Q1, K1, Q2, K2)
+    if dQ2 is None:
+        dQ2 = torch.empty_like(Q2)
+    if dK2 is None:
+        dK2 = torch.empty_like(K2)
+    if teacher:
+        if dQ1 is None:
+            dQ1 = torch.empty_like(Q1)
+        if dK1 is None:
+            dK1 = torch.empty_like(K1)
+    else:
+        dQ1 = dK1 = None
+    for n, t in (("dQ1", dQ1), ("dK1", dK1), ("dQ2", dQ2), ("dK2", dK2)):
+        if t is not None:
+            _check_dev(n, t, Q1.dtype)
+    need = streamkl_bwd_workspace_bytes(B, H, NQ, NK, d1, d2, teacher)
+    if need > 0 and (workspace is None or workspace.numel() * workspace.element_size() < need):
+        workspace = torch.empty(need, dtype=torch.uint8, device=Q1.device)
+    ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    if Q1.dtype == torch.bfloat16:
+        fn = lib().streamkl_bwd
+    elif Q1.dtype == torch.float32:
+        fn = lib().streamkl_bwd_f32
+    else:
+        raise TypeError("inputs must be bfloat16 or float32")
+    with torch.cuda.device(Q1.device):
+        rc = fn(_ptr(Q1), _ptr(K1), _ptr(Q2), _ptr(K2), B, H, NQ, NK, d1, d2, float(c1), float(c2), int(bool(causal)),
+                _ptr(kl_rows), _ptr(lse1), _ptr(lse2), _ptr(dkl_rows), _ptr(dQ1), _ptr(dK1), _ptr(dQ2), _ptr(dK2),
+                _ptr(workspace), ctypes.c_size_t(ws_bytes), _stream_handle(stream))
+    if rc != 0:
+        raise StreamKLError(rc, "streamkl_bwd")
+    return dQ1, dK1, dQ2, dK2
+
+
+# ------------------------------------------------------------------------------------------ host entry points
+def _host_dtype(a: np.ndarray) -> int:
+    if a.dtype == np.uint16:
+        return STREAMKL_BF16
+    if a.dtype == np.float32:
+        return STREAMKL_F32
+    raise TypeError("host tensors must be uint16 (bf16 bit patterns) or float32")
+
+
+def _np_ptr(a):
+    return ctypes.c_void_p(a.ctypes.data) if a is not None else ctypes.c_void_p(0)
+
+
+def _host_inputs(Q1, K1, Q2, K2):
+    arrs = [np.ascontiguousarray(a) for a in (Q1, K1, Q2, K2)]
+    dt = _host_dtype(arrs[0])
+    for a in arrs:
+        if _host_dtype(a) != dt:
+            raise TypeError("Q1,K1,Q2,K2 must share a dtype")
+    B, H, NQ, d1 = arrs[0].shape
+    NK, d2 = arrs[1].shape[2], arrs[2].shape[3]
+    if arrs[1].shape != (B, H, NK, d1) or arrs[2].shape != (B, H, NQ, d2) or arrs[3].shape != (B, H, NK, d2):
+        raise ValueError("inconsistent Q1,K1,Q2,K2 shapes")
+    return arrs, dt, (B, H, NQ, NK, d1, d2)
+
+
+def streamkl_fwd_host(Q1, K1, Q2, K2, c1, c2, causal):
+    """End-to-end forward with HOST numpy buffers (copies inside the call).  Returns (kl_rows, lse1, lse2) numpy float32."""
+    arrs, dt, (B, H, NQ, NK, d1, d2) = _host_inputs(Q1, K1, Q2, K2)
+    kl, l1, l2 = (np.empty((B, H, NQ), np.float32) for _ in range(3))
+    rc = lib().streamkl_fwd_host(dt, *[_np_ptr(a) for a in arrs], B, H, NQ, NK, d1, d2, float(c1), float(c2),
+                                 int(bool(causal)), _np_ptr(kl), _np_ptr(l1), _np_ptr(l2), ctypes.c_void_p(0))
+    if rc != 0:
+        raise StreamKLError(rc, "streamkl_fwd_host")
+    return kl, l1, l2
+
+
+def streamkl_fwd_bwd_host(Q1, K1, Q2, K2, c1, c2, causal, dkl_rows, teacher=False, out=None):
+    """End-to-end forward + backward with HOST numpy buffers.  Returns dict(kl, lse1, lse2, dQ2, dK2[, dQ1, dK1]).
+
+    `out` may carry preallocated (e.g. pinned) result arrays under the same keys."""
+    arrs, dt, (B, H, NQ, NK, d1, d2) = _host_inputs(Q1, K1, Q2, K2)
+    g = np.ascontiguousarray(dkl_rows, dtype=np.float32)
+    if g.shape != (B, H, NQ):
+        raise ValueError("dkl_rows must be [B,H,NQ]")
+    st = arrs[0].dtype
+    out = {} if out is None else out
+    spec = {"kl": ((B, H, NQ), np.float32), "lse1": ((B, H, NQ), np.float32), "lse2": ((B, H, NQ), np.float32),
+            "dQ2": ((B, H, NQ, d2), st), "dK2": ((B, H, NK, d2), st)}
+    if teacher:
+        spec["dQ1"] = ((B, H, NQ, d1), st)
+        spec["dK1"] = ((B, H, NK, d1), st)
+    for k, (shp, dty) in spec.items():
+        if k not in out:
+            out[k] = np.empty(shp, dty)
+        elif out[k].shape != shp or out[k].dtype != dty or not out[k].flags.c_contiguous:
+            raise ValueError(f"out[{k!r}] has the wrong shape/dtype/layout")
+    rc = lib().streamkl_fwd_bwd_host(dt, *[_np_ptr(a) for a in arrs], B, H, NQ, NK, d1, d2, float(c1), float(c2),
+                                     int(bool(causal)), _np_ptr(g), _np_ptr(out["kl"]), _np_ptr(out["lse1"]),
+                                     _np_ptr(out["lse2"]), _np_ptr(out.get("dQ1")), _np_ptr(out.get("dK1")),
+                                     _np_ptr(out["dQ2"]), _np_ptr(out["dK2"]), ctypes.c_void_p(0))
+    if rc != 0:
+        raise StreamKLError(rc, "streamkl_fwd_bwd_host")
+    return out

@@ -1,0 +1,393 @@
+// streamkl.cu -- the C-ABI boundary (include/streamkl.h): argument validation, TMA tensor maps, kernel dispatch.
+// No torch types, no allocation on the device entry points, no CPU fallback.
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <cuda_bf16.h>
+
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+
+#include "../../include/streamkl.h"
+#include "streamkl_fwd_sm100.cuh"
+#include "streamkl_bwd_sm100.cuh"
+#include "streamkl_simt.cuh"
+
+namespace {
+
+thread_local int g_last_launches = 0;
+
+using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                   const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                   CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn get_encode_fn() {
+  static EncodeTiledFn fn = []() -> EncodeTiledFn {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess || q != cudaDriverEntryPointSuccess)
+      return nullptr;
+    return reinterpret_cast<EncodeTiledFn>(p);
+  }();
+  return fn;
+}
+
+// true iff the current device is sm_100 (B200): the only target this library is built for
+bool device_is_sm100() {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return false; }
+  int major = 0;
+  if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) { cudaGetLastError(); return false; }
+  return major == 10;
+}
+
+// [BH][N][d] bf16 row-major tensor, box = {64 elements (128 B), box_rows, 1}, 128-byte swizzle, zero OOB fill.
+bool make_tmap_bf16(CUtensorMap* m, const void* base, int BH, int N, int d, int box_rows) {
+  EncodeTiledFn enc = get_encode_fn();
+  if (!enc) return false;
+  cuuint64_t dims[3] = {cuuint64_t(d), cuuint64_t(N), cuuint64_t(BH)};
+  cuuint64_t strides[2] = {cuuint64_t(d) * 2, cuuint64_t(N) * cuuint64_t(d) * 2};
+  cuuint32_t box[3] = {64, cuuint32_t(box_rows), 1};
+  cuuint32_t estr[3] = {1, 1, 1};
+  return enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+struct Shape {
+  int B, H, NQ, NK, d1, d2, causal;
+  float c1, c2;
+  long long BH;
+};
+
+int validate_common(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s) {
+  if (s.B < 0 || s.H < 0 || s.NQ < 0 || s.NK < 1 || s.d1 < 1 || s.d2 < 1 || s.d1 > 256 || s.d2 > 256) return STREAMKL_ERR_SHAPE;
+  if (s.causal && s.NQ > s.NK) return STREAMKL_ERR_SHAPE;
+  if (s.BH > 65535 * 1024LL || s.BH * (long long)(s.NQ > s.NK ? s.NQ : s.NK) > (1LL << 40)) return STREAMKL_ERR_SHAPE;
+  if (!(std::isfinite(s.c1) && std::isfinite(s.c2) && s.c1 > 0.f && s.c2 > 0.f)) return STREAMKL_ERR_SCALE;
+  if (s.BH == 0 || s.NQ == 0) return STREAMKL_OK;
+  if (!Q1 || !K1 || !Q2 || !K2) return STREAMKL_ERR_NULLPTR;
+  if ((reinterpret_cast<uintptr_t>(Q1) | reinterpret_cast<uintptr_t>(K1) | reinterpret_cast<uintptr_t>(Q2) |
+       reinterpret_cast<uintptr_t>(K2)) & 15)
+    return STREAMKL_ERR_ALIGN;
+  return STREAMKL_OK;
+}
+
+bool tc_shape(int dtype, const Shape& s) {
+  return dtype == STREAMKL_BF16 && (s.d1 == 64 || s.d1 == 128) && (s.d2 == 64 || s.d2 == 128);
+}
+
+// ----------------------------------------------------------------------------------------- forward launchers
+template <int D1, int D2, bool CAUSAL>
+int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, float* kl, float* lse1, float* lse2,
+                  cudaStream_t stream) {
+  using C = skl::FwdCfg<D1, D2>;
+  CUtensorMap tQ1, tK1, tQ2, tK2;
+  if (!make_tmap_bf16(&tQ1, Q1, int(s.BH), s.NQ, D1, C::BM) || !make_tmap_bf16(&tK1, K1, int(s.BH), s.NK, D1, C::BK) ||
+      !make_tmap_bf16(&tQ2, Q2, int(s.BH), s.NQ, D2, C::BM) || !make_tmap_bf16(&tK2, K2, int(s.BH), s.NK, D2, C::BK))
+    return STREAMKL_ERR_CUDA;
+  auto kern = skl::streamkl_fwd_sm100_kernel<D1, D2, CAUSAL>;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
+    cudaGetLastError();
+    return STREAMKL_ERR_CUDA;
+  }
+  skl::FwdParams p;
+  p.NQ = s.NQ; p.NK = s.NK; p.BH = int(s.BH);
+  p.TQ = (s.NQ + C::BQ - 1) / C::BQ;
+  p.sc1 = s.c1 * 1.4426950408889634f;
+  p.sc2 = s.c2 * 1.4426950408889634f;
+  p.kl = kl; p.lse1 = lse1; p.lse2 = lse2;
+  const long long grid = (long long)p.TQ * s.BH;
+  if (grid > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
+  kern<<<dim3((unsigned)grid), C::THREADS, C::SMEM_BYTES, stream>>>(tQ1, tK1, tQ2, tK2, p);
+  if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
+  g_last_launches += 1;
+  return STREAMKL_OK;
+}
+
+int simt_block_rows(size_t floats_per_row, size_t fixed_floats, size_t* smem_bytes) {
+  for (int br : {128, 64, 32}) {
+    size_t b = (floats_per_row * br + fixed_floats) * sizeof(float);
+    if (b <= 200 * 1024) { *smem_bytes = b; return br; }
+  }
+  return 0;
+}
+
+template <typename T>
+int launch_fwd_simt(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, float* kl, float* lse1,
+                    float* lse2, cudaStream_t stream) {
+  size_t smem = 0;
+  const int br = simt_block_rows(size_t(s.d1 + s.d2 + 2), size_t(skl::SIMT_TILE) * (s.d1 + s.d2), &smem);
+  if (!br) return STREAMKL_ERR_SHAPE;
+  auto kern = skl::streamkl_fwd_simt_kernel<T>;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess) {
+    cudaGetLastError();
+    return STREAMKL_ERR_CUDA;
+  }
+  skl::SimtParams p{s.NQ, s.NK, s.d1, s.d2, s.causal, s.c1, s.c2};
+  dim3 grid((s.NQ + br - 1) / br, (unsigned)s.BH);
+  kern<<<grid, br, smem, stream>>>(static_cast<const T*>(Q1), static_cast<const T*>(K1), static_cast<const T*>(Q2),
+                                   static_cast<const T*>(K2), p, kl, lse1, lse2);
+  if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
+  g_last_launches += 1;
+  return STREAMKL_OK;
+}
+
+int fwd_dispatch(int dtype, const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1,
+                 int d2, float c1, float c2, int causal, float* kl, float* lse1, float* lse2, cudaStream_t stream) {
+  Shape s{B, H, NQ, NK, d1, d2, causal ? 1 : 0, c1, c2, (long long)B * (long long)H};
+  int rc = validate_common(Q1, K1, Q2, K2, s);
+  if (rc != STREAMKL_OK) return rc;
+  g_last_launches = 0;
+  if (s.BH == 0 || s.NQ == 0) return STREAMKL_OK;
+  if (!kl || !lse1 || !lse2) return STREAMKL_ERR_NULLPTR;
+  if (!device_is_sm100()) return STREAMKL_ERR_CUDA;
+  if (s.BH > 65535) return STREAMKL_ERR_SHAPE;
+  if (tc_shape(dtype, s)) {
+#define SKL_FWD_CASE(A, Bd)                                                                                                  \
+  if (d1 == A && d2 == Bd)                                                                                                   \
+    return s.causal ? launch_fwd_tc<A, Bd, true>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream)                                  \
+                    : launch_fwd_tc<A, Bd, false>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream);
+    SKL_FWD_CASE(128, 128)
+    SKL_FWD_CASE(128, 64)
+    SKL_FWD_CASE(64, 128)
+    SKL_FWD_CASE(64, 64)
+#undef SKL_FWD_CASE
+  }
+  if (dtype == STREAMKL_BF16) return launch_fwd_simt<__nv_bfloat16>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream);
+  if (dtype == STREAMKL_F32) return launch_fwd_simt<float>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream);
+  return STREAMKL_ERR_DTYPE;
+}
+
+// ----------------------------------------------------------------------------------------- backward launchers
+template <typename T, bool OWNER_K>
+int launch_bwd_simt(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, const float* kl,
+                    const float* lse1, const float* lse2, const float* dkl, void* dX1, void* dX2, cudaStream_t stream) {
+  size_t smem = 0;
+  const int br = simt_block_rows(size_t(2 * (s.d1 + s.d2 + 2)), size_t(skl::SIMT_TILE) * (s.d1 + s.d2 + 4), &smem);
+  if (!br) return STREAMKL_ERR_SHAPE;
+  auto kern = skl::streamkl_bwd_simt_kernel<T, OWNER_K>;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, int(smem)) != cudaSuccess) {
+    cudaGetLastError();
+    return STREAMKL_ERR_CUDA;
+  }
+  skl::SimtParams p{s.NQ, s.NK, s.d1, s.d2, s.causal, s.c1, s.c2};
+  const int NX = OWNER_K ? s.NK : s.NQ;
+  dim3 grid((NX + br - 1) / br, (unsigned)s.BH);
+  kern<<<grid, br, smem, stream>>>(static_cast<const T*>(Q1), static_cast<const T*>(K1), static_cast<const T*>(Q2),
+                                   static_cast<const T*>(K2), p, kl, lse1, lse2, dkl, static_cast<T*>(dX1), static_cast<T*>(dX2));
+  if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
+  g_last_launches += 1;
+  return STREAMKL_OK;
+}
+
+template <int D1, int D2, bool CAUSAL, bool TEACHER, bool OWNER_K>
+int launch_bwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, const float* kl, const float* lse1,
+                  const float* lse2, const float* dkl, void* dX1, void* dX2, cudaStream_t stream) {
+  using C = skl::BwdCfg<D1, D2, TEACHER>;
+  CUtensorMap tQ1, tK1, tQ2, tK2;
+  // the owner side is loaded in 128-row boxes, the streamed side in BY-row boxes
+  const int rq = OWNER_K ? C::BY : C::BX, rk = OWNER_K ? C::BX : C::BY;
+  if (!make_tmap_bf16(&tQ1, Q1, int(s.BH), s.NQ, D1, rq) || !make_tmap_bf16(&tK1, K1, int(s.BH), s.NK, D1, rk) ||
+      !make_tmap_bf16(&tQ2, Q2, int(s.BH), s.NQ, D2, rq) || !make_tmap_bf16(&tK2, K2, int(s.BH), s.NK, D2, rk))
+    return STREAMKL_ERR_CUDA;
+  auto kern = skl::streamkl_bwd_sm100_kernel<D1, D2, CAUSAL, TEACHER, OWNER_K>;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
+    cudaGetLastError();
+    return STREAMKL_ERR_CUDA;
+  }
+  skl::BwdParams p;
+  p.NQ = s.NQ; p.NK = s.NK; p.BH = int(s.BH);
+  p.TX = ((OWNER_K ? s.NK : s.NQ) + C::BX - 1) / C::BX;
+  p.c1 = s.c1; p.c2 = s.c2;
+  p.kl = kl; p.lse1 = lse1; p.lse2 = lse2; p.dkl = dkl;
+  p.dX1 = static_cast<__nv_bfloat16*>(dX1);
+  p.dX2 = static_cast<__nv_bfloat16*>(dX2);
+  const long long grid = (long long)p.TX * s.BH;
+  if (grid > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
+  kern<<<dim3((unsigned)grid), C::THREADS, C::SMEM_BYTES, stream>>>(tQ1, tK1, tQ2, tK2, p);
+  if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
+  g_last_launches += 1;
+  return STREAMKL_OK;
+}
+
+template <int D1, int D2>
+int bwd_tc_both(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, const float* kl, const float* lse1,
+                const float* lse2, const float* dkl, void* dQ1, void* dK1, void* dQ2, void* dK2, cudaStream_t st) {
+  const bool t = dQ1 != nullptr;
+  int rc;
+#define SKL_BWD(CA, TE)                                                                                                   \
+  rc = launch_bwd_tc<D1, D2, CA, TE, false>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dQ2, st);                        \
+  if (rc != STREAMKL_OK) return rc;                                                                                       \
+  return launch_bwd_tc<D1, D2, CA, TE, true>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dK1, dK2, st);
+  if (s.causal) { if (t) { SKL_BWD(true, true) } else { SKL_BWD(true, false) } }
+  else          { if (t) { SKL_BWD(false, true) } else { SKL_BWD(false, false) } }
+#undef SKL_BWD
+}
+
+int bwd_dispatch(int dtype, const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1,
+                 int d2, float c1, float c2, int causal, const float* kl, const float* lse1, const float* lse2, const float* dkl,
+                 void* dQ1, void* dK1, void* dQ2, void* dK2, void* workspace, size_t workspace_bytes, cudaStream_t stream) {
+  (void)workspace;
+  Shape s{B, H, NQ, NK, d1, d2, causal ? 1 : 0, c1, c2, (long long)B * (long long)H};
+  int rc = validate_common(Q1, K1, Q2, K2, s);
+  if (rc != STREAMKL_OK) return rc;
+  g_last_launches = 0;
+  if ((dQ1 == nullptr) != (dK1 == nullptr)) return STREAMKL_ERR_NULLPTR;
+  if (s.BH == 0) return STREAMKL_OK;
+  if (!dK2) return STREAMKL_ERR_NULLPTR;
+  if (s.NQ > 0 && (!kl || !lse1 || !lse2 || !dkl || !dQ2)) return STREAMKL_ERR_NULLPTR;
+  if ((reinterpret_cast<uintptr_t>(dQ1) | reinterpret_cast<uintptr_t>(dK1) | reinterpret_cast<uintptr_t>(dQ2) |
+       reinterpret_cast<uintptr_t>(dK2)) & 15)
+    return STREAMKL_ERR_ALIGN;
+  const size_t need = streamkl_bwd_workspace_bytes(B, H, NQ, NK, d1, d2, dQ1 != nullptr);
+  if (need > 0 && (!workspace || workspace_bytes < need)) return STREAMKL_ERR_WORKSPACE;
+  if (!device_is_sm100()) return STREAMKL_ERR_CUDA;
+  if (s.BH > 65535) return STREAMKL_ERR_SHAPE;
+  const size_t es = dtype == STREAMKL_BF16 ? 2 : 4;
+  if (s.NQ == 0) {  // no query rows: dK = 0, nothing else to write
+    if (cudaMemsetAsync(dK2, 0, size_t(s.BH) * NK * d2 * es, stream) != cudaSuccess) return STREAMKL_ERR_CUDA;
+    if (dK1 && cudaMemsetAsync(dK1, 0, size_t(s.BH) * NK * d1 * es, stream) != cudaSuccess) return STREAMKL_ERR_CUDA;
+    return STREAMKL_OK;
+  }
+  if (tc_shape(dtype, s)) {
+    if (d1 == 128 && d2 == 128) return bwd_tc_both<128, 128>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, stream);
+    if (d1 == 128 && d2 == 64) return bwd_tc_both<128, 64>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, stream);
+    if (d1 == 64 && d2 == 128) return bwd_tc_both<64, 128>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, stream);
+    if (d1 == 64 && d2 == 64) return bwd_tc_both<64, 64>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, stream);
+  }
+  if (dtype == STREAMKL_BF16) {
+    rc = launch_bwd_simt<__nv_bfloat16, false>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dQ2, stream);
+    if (rc != STREAMKL_OK) return rc;
+    return launch_bwd_simt<__nv_bfloat16, true>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dK1, dK2, stream);
+  }
+  if (dtype == STREAMKL_F32) {
+    rc = launch_bwd_simt<float, false>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dQ2, stream);
+    if (rc != STREAMKL_OK) return rc;
+    return launch_bwd_simt<float, true>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dK1, dK2, stream);
+  }
+  return STREAMKL_ERR_DTYPE;
+}
+
+// RAII device scratch for the *_host entry points
+struct DevBuf {
+  void* p = nullptr;
+  ~DevBuf() { if (p) cudaFree(p); }
+  bool alloc(size_t n) { return n == 0 || cudaMalloc(&p, n) == cudaSuccess; }
+};
+
+}  // namespace
+
+extern "C" {
+
+int streamkl_fwd(const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1, int d2, float c1,
+                 float c2, int causal, float* kl_rows, float* lse1, float* lse2, streamkl_stream_t stream) {
+  return fwd_dispatch(STREAMKL_BF16, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
+                      static_cast<cudaStream_t>(stream));
+}
+int streamkl_fwd_f32(const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1, int d2,
+                     float c1, float c2, int causal, float* kl_rows, float* lse1, float* lse2, streamkl_stream_t stream) {
+  return fwd_dispatch(STREAMKL_F32, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
+                      static_cast<cudaStream_t>(stream));
+}
+int streamkl_bwd(const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1, int d2, float c1,
+                 float c2, int causal, const float* kl_rows, const float* lse1, const float* lse2, const float* dkl_rows, void* dQ1,
+                 void* dK1, void* dQ2, void* dK2, void* workspace, size_t workspace_bytes, streamkl_stream_t stream) {
+  return bwd_dispatch(STREAMKL_BF16, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2, dkl_rows, dQ1, dK1,
+                      dQ2, dK2, workspace, workspace_bytes, static_cast<cudaStream_t>(stream));
+}
+int streamkl_bwd_f32(const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1, int d2,
+                     float c1, float c2, int causal, const float* kl_rows, const float* lse1, const float* lse2,
+                     const float* dkl_rows, void* dQ1, void* dK1, void* dQ2, void* dK2, void* workspace, size_t workspace_bytes,
+                     streamkl_stream_t stream) {
+  return bwd_dispatch(STREAMKL_F32, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2, dkl_rows, dQ1, dK1,
+                      dQ2, dK2, workspace, workspace_bytes, static_cast<cudaStream_t>(stream));
+}
+
+size_t streamkl_bwd_workspace_bytes(int, int, int, int, int, int, int) {
+  return 0;  // both gradients are produced by tile ownership: no fp32 accumulation workspace
+}
+
+int streamkl_fwd_host(int dtype, const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1,
+                      int d2, float c1, float c2, int causal, float* kl_rows, float* lse1, float* lse2, streamkl_stream_t stream) {
+  return streamkl_fwd_bwd_host(dtype, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, nullptr, kl_rows, lse1, lse2, nullptr,
+                               nullptr, nullptr, nullptr, stream);
+}
+
+int streamkl_fwd_bwd_host(int dtype, const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK,
+                          int d1, int d2, float c1, float c2, int causal, const float* dkl_rows, float* kl_rows, float* lse1,
+                          float* lse2, void* dQ1, void* dK1, void* dQ2, void* dK2, streamkl_stream_t stream_) {
+  if (dtype != STREAMKL_BF16 && dtype != STREAMKL_F32) return STREAMKL_ERR_DTYPE;
+  cudaStream_t stream = static_cast<cudaStream_t>(stream_);
+  Shape s{B, H, NQ, NK, d1, d2, causal ? 1 : 0, c1, c2, (long long)B * (long long)H};
+  // host pointers need no 16-byte alignment: validate with aligned stand-ins
+  int rc = validate_common(Q1 ? (const void*)16 : nullptr, K1 ? (const void*)16 : nullptr, Q2 ? (const void*)16 : nullptr,
+                           K2 ? (const void*)16 : nullptr, s);
+  if (rc != STREAMKL_OK) return rc;
+  const bool want_bwd = dQ2 != nullptr || dK2 != nullptr;
+  if (want_bwd && (!dQ2 || !dK2 || !dkl_rows)) return STREAMKL_ERR_NULLPTR;
+  if ((dQ1 == nullptr) != (dK1 == nullptr)) return STREAMKL_ERR_NULLPTR;
+  if (!want_bwd && dQ1) return STREAMKL_ERR_NULLPTR;
+  if (s.BH == 0 || s.NQ == 0) {
+    if (!want_bwd || s.BH == 0) return STREAMKL_OK;
+  } else if (!kl_rows || !lse1 || !lse2) {
+    return STREAMKL_ERR_NULLPTR;
+  }
+  if (!device_is_sm100()) return STREAMKL_ERR_CUDA;
+  const size_t es = dtype == STREAMKL_BF16 ? 2 : 4;
+  const size_t nq1 = size_t(s.BH) * NQ * d1 * es, nk1 = size_t(s.BH) * NK * d1 * es;
+  const size_t nq2 = size_t(s.BH) * NQ * d2 * es, nk2 = size_t(s.BH) * NK * d2 * es;
+  const size_t nrow = size_t(s.BH) * NQ * sizeof(float);
+  DevBuf bQ1, bK1, bQ2, bK2, bkl, bl1, bl2, bg, gQ1, gK1, gQ2, gK2;
+  if (!bQ1.alloc(nq1) || !bK1.alloc(nk1) || !bQ2.alloc(nq2) || !bK2.alloc(nk2) || !bkl.alloc(nrow) || !bl1.alloc(nrow) ||
+      !bl2.alloc(nrow)) { cudaGetLastError(); return STREAMKL_ERR_CUDA; }
+  if (want_bwd && (!bg.alloc(nrow) || !gQ2.alloc(nq2) || !gK2.alloc(nk2) || (dQ1 && (!gQ1.alloc(nq1) || !gK1.alloc(nk1))))) {
+    cudaGetLastError();
+    return STREAMKL_ERR_CUDA;
+  }
+  auto up = [&](void* d, const void* h, size_t n) { return n == 0 || cudaMemcpyAsync(d, h, n, cudaMemcpyHostToDevice, stream) == cudaSuccess; };
+  auto down = [&](void* h, const void* d, size_t n) { return n == 0 || cudaMemcpyAsync(h, d, n, cudaMemcpyDeviceToHost, stream) == cudaSuccess; };
+  if (!up(bQ1.p, Q1, nq1) || !up(bK1.p, K1, nk1) || !up(bQ2.p, Q2, nq2) || !up(bK2.p, K2, nk2)) return STREAMKL_ERR_CUDA;
+  if (want_bwd && !up(bg.p, dkl_rows, nrow)) return STREAMKL_ERR_CUDA;
+  int launches = 0;
+  if (s.NQ > 0) {
+    rc = fwd_dispatch(dtype, bQ1.p, bK1.p, bQ2.p, bK2.p, B, H, NQ, NK, d1, d2, c1, c2, causal, static_cast<float*>(bkl.p),
+                      static_cast<float*>(bl1.p), static_cast<float*>(bl2.p), stream);
+    if (rc != STREAMKL_OK) { cudaStreamSynchronize(stream); return rc; }
+    launches += g_last_launches;
+  }
+  if (want_bwd) {
+    rc = bwd_dispatch(dtype, bQ1.p, bK1.p, bQ2.p, bK2.p, B, H, NQ, NK, d1, d2, c1, c2, causal, static_cast<float*>(bkl.p),
+                      static_cast<float*>(bl1.p), static_cast<float*>(bl2.p), static_cast<float*>(bg.p), gQ1.p, gK1.p, gQ2.p, gK2.p,
+                      nullptr, 0, stream);
+    if (rc != STREAMKL_OK) { cudaStreamSynchronize(stream); return rc; }
+    launches += g_last_launches;
+  }
+  bool ok = down(kl_rows, bkl.p, nrow) && down(lse1, bl1.p, nrow) && down(lse2, bl2.p, nrow);
+  if (want_bwd) {
+    ok = ok && down(dQ2, gQ2.p, nq2) && down(dK2, gK2.p, nk2);
+    if (dQ1) ok = ok && down(dQ1, gQ1.p, nq1) && down(dK1, gK1.p, nk1);
+  }
+  if (cudaStreamSynchronize(stream) != cudaSuccess || !ok) { cudaGetLastError(); return STREAMKL_ERR_CUDA; }
+  g_last_launches = launches;
+  return STREAMKL_OK;
+}
+
+int streamkl_last_launch_count(void) { return g_last_launches; }
+
+const char* streamkl_strerror(int code) {
+  switch (code) {
+    case STREAMKL_OK: return "ok";
+    case STREAMKL_ERR_NULLPTR: return "required pointer is NULL";
+    case STREAMKL_ERR_SHAPE: return "unsupported shape (sizes, head dim, or causal with NQ > NK)";
+    case STREAMKL_ERR_ALIGN: return "tensor pointer not 16-byte aligned";
+    case STREAMKL_ERR_SCALE: return "scale c1/c2 must be finite and > 0";
+    case STREAMKL_ERR_WORKSPACE: return "workspace missing or too small";
+    case STREAMKL_ERR_CUDA: return "CUDA failure (no sm_100 device, tensor-map, launch, copy or allocation)";
+    case STREAMKL_ERR_DTYPE: return "unknown dtype code";
+    default: return "unknown error code";
+  }
+}
+
+const char* streamkl_version(void) { return "streamkl-b200 0.1 (sm_100a; tcgen05+TMA bf16, SIMT fp32)"; }
+
+}  // extern "C"

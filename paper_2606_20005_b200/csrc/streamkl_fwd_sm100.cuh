@@ -1,0 +1,281 @@
+// streamkl_fwd_sm100.cuh -- StreamKL forward (Algorithm 1) for sm_100a.
+//
+// One CTA owns 256 query rows of one (b,h) (two 128-row M-tiles) and streams 64-key tiles:
+//   warp 0      TMA producer : Q1,Q2 once; K1_j,K2_j through an NSTAGE ring          (F1, F2 of DESIGN.md)
+//   warp 1      MMA issuer   : S1 = Q1 K1_j^T, S2 = Q2 K2_j^T, tcgen05.mma -> TMEM    (F3)
+//   warp 2      TMEM allocator
+//   warps 4-7   softmax warpgroup of M-tile 0: thread = one query row                   (F4, F5, F6)
+//   warps 8-11  softmax warpgroup of M-tile 1
+// TMEM (512 columns): per M-tile two stages of {S1 (64 cols), S2 (64 cols)}.  A softmax thread pulls its whole
+// 64+64-logit row into registers, releases the TMEM stage at once (so the next tile's MMA overlaps the exp work)
+// and then performs the online update of (m1,l1,m2,l2,acc) -- Eq.9-10 -- entirely thread-locally in the log2
+// domain (exp2 instead of exp; R6).
+#pragma once
+#include <cuda_bf16.h>
+#include <math_constants.h>
+
+#include "sm100_ptx.cuh"
+
+namespace skl {
+
+template <int D1, int D2>
+struct FwdCfg {
+  static_assert(D1 % 64 == 0 && D2 % 64 == 0 && D1 <= 128 && D2 <= 128, "tcgen05 path: d in {64,128}");
+  static constexpr int BM = 128;             // rows per M-tile (TMEM lanes)
+  static constexpr int NMT = 2;              // M-tiles per CTA
+  static constexpr int BQ = BM * NMT;        // query rows per CTA
+  static constexpr int BK = 64;              // keys per step
+  static constexpr int KB1 = D1 / 64, KB2 = D2 / 64;  // 128-byte K-blocks per row
+  static constexpr int QBLK = BM * 128;      // bytes of one [128 rows x 64 bf16] swizzled block
+  static constexpr int KBLK = BK * 128;      // bytes of one [64 rows x 64 bf16] swizzled block
+  static constexpr int Q_BYTES = NMT * (KB1 + KB2) * QBLK;
+  static constexpr int STAGE_BYTES = (KB1 + KB2) * KBLK;
+  static constexpr int SMEM_LIMIT = 227 * 1024;
+  static constexpr int AUX_BYTES = 256;      // barriers + tmem pointer
+  static constexpr int NSTAGE_RAW = (SMEM_LIMIT - 1024 - AUX_BYTES - Q_BYTES) / STAGE_BYTES;
+  static constexpr int NSTAGE = NSTAGE_RAW > 6 ? 6 : NSTAGE_RAW;
+  static_assert(NSTAGE >= 2, "need at least a double-buffered K ring");
+  static constexpr int SMEM_BYTES = 1024 + Q_BYTES + NSTAGE * STAGE_BYTES + AUX_BYTES;
+  static constexpr int THREADS = 384;
+  static constexpr uint32_t TMEM_COLS = 512;
+};
+
+struct FwdParams {
+  int NQ, NK, TQ;       // TQ = number of 256-row super tiles per head
+  int BH;
+  float sc1, sc2;       // c_t * log2(e)
+  float* kl;
+  float* lse1;
+  float* lse2;
+};
+
+// Online update for one 64-key tile of one query row (thread-local).  Implements Alg.1 lines 8-12 with
+//   x_t = s_t*sc_t - m_t (log2 domain, shifted),  acc += sum p1*(x1-x2) + (m1-m2)*sum p1   [= sum p1 (s1'-s2')].
+struct RowState {
+  float m1, m2, l1, l2, acc;
+};
+
+template <bool MASKED>
+__device__ __forceinline__ void online_update64(RowState& st, const uint32_t (&r1)[64], const uint32_t (&r2)[64], float sc1,
+                                                float sc2, int kbase, int limit) {
+  float mx1a = -CUDART_INF_F, mx1b = -CUDART_INF_F, mx2a = -CUDART_INF_F, mx2b = -CUDART_INF_F;
+  if constexpr (!MASKED) {
+#pragma unroll
+    for (int e = 0; e < 64; e += 4) {
+      mx1a = max3(mx1a, __uint_as_float(r1[e]), __uint_as_float(r1[e + 1]));
+      mx1b = max3(mx1b, __uint_as_float(r1[e + 2]), __uint_as_float(r1[e + 3]));
+      mx2a = max3(mx2a, __uint_as_float(r2[e]), __uint_as_float(r2[e + 1]));
+      mx2b = max3(mx2b, __uint_as_float(r2[e + 2]), __uint_as_float(r2[e + 3]));
+    }
+  } else {
+#pragma unroll
+    for (int e = 0; e < 64; ++e) {
+      const bool ok = (kbase + e) <= limit;
+      mx1a = fmaxf(mx1a, ok ? __uint_as_float(r1[e]) : -CUDART_INF_F);
+      mx2a = fmaxf(mx2a, ok ? __uint_as_float(r2[e]) : -CUDART_INF_F);
+    }
+  }
+  const float m1n = fmaxf(st.m1, fmaxf(mx1a, mx1b) * sc1);  // sc > 0: max commutes with the scale
+  const float m2n = fmaxf(st.m2, fmaxf(mx2a, mx2b) * sc2);
+  // R7: a row whose every key so far is masked keeps m = -inf; use reference 0 so (-inf)-(-inf) never forms
+  const float ref1 = MASKED ? (m1n == -CUDART_INF_F ? 0.f : m1n) : m1n;
+  const float ref2 = MASKED ? (m2n == -CUDART_INF_F ? 0.f : m2n) : m2n;
+  const float a1 = ex2_approx(st.m1 - ref1);  // alpha_1 (Alg.1 line 9); m = -inf gives 0
+  const float a2 = ex2_approx(st.m2 - ref2);
+  float s1[4] = {0.f, 0.f, 0.f, 0.f}, s2[4] = {0.f, 0.f, 0.f, 0.f}, dd[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+  for (int e = 0; e < 64; ++e) {
+    const float x1 = fmaf(__uint_as_float(r1[e]), sc1, -ref1);
+    const float x2 = fmaf(__uint_as_float(r2[e]), sc2, -ref2);
+    float p1 = ex2_approx(x1);
+    float p2 = ex2_approx(x2);
+    if constexpr (MASKED) {  // R8: zero P~, take the difference from the raw (finite) logits
+      const bool ok = (kbase + e) <= limit;
+      p1 = ok ? p1 : 0.f;
+      p2 = ok ? p2 : 0.f;
+    }
+    s1[e & 3] += p1;
+    s2[e & 3] += p2;
+    dd[e & 3] = fmaf(p1, x1 - x2, dd[e & 3]);
+  }
+  const float sum1 = (s1[0] + s1[1]) + (s1[2] + s1[3]);
+  const float sum2 = (s2[0] + s2[1]) + (s2[2] + s2[3]);
+  const float dsum = (dd[0] + dd[1]) + (dd[2] + dd[3]);
+  st.l1 = fmaf(st.l1, a1, sum1);                               // line 11 (R9: alpha1 on l1, acc; alpha2 on l2)
+  st.l2 = fmaf(st.l2, a2, sum2);
+  st.acc = fmaf(st.acc, a1, fmaf(ref1 - ref2, sum1, dsum));    // line 12
+  st.m1 = m1n;
+  st.m2 = m2n;
+}
+
+template <int D1, int D2, bool CAUSAL>
+__global__ void __launch_bounds__(384, 1)
+streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid_constant__ CUtensorMap tmK1,
+                          const __grid_constant__ CUtensorMap tmQ2, const __grid_constant__ CUtensorMap tmK2, const FwdParams p) {
+  using C = FwdCfg<D1, D2>;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t* sQ1 = smem;
+  uint8_t* sQ2 = sQ1 + C::NMT * C::KB1 * C::QBLK;
+  uint8_t* sK = smem + C::Q_BYTES;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sK + C::NSTAGE * C::STAGE_BYTES);
+  uint64_t* q_full = bars;                    // 1
+  uint64_t* k_full = bars + 1;                // NSTAGE
+  uint64_t* k_empty = k_full + C::NSTAGE;     // NSTAGE
+  uint64_t* s_full = k_empty + C::NSTAGE;     // [mt][st] 4
+  uint64_t* s_empty = s_full + 4;             // [mt][st] 4
+  uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(s_empty + 4);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  // heavy (late, causal) query tiles first within each head; consecutive CTAs share a head (K stays in L2)
+  const int bh = blockIdx.x / p.TQ;
+  const int qt = p.TQ - 1 - (blockIdx.x % p.TQ);
+  const int q0 = qt * C::BQ;
+  const int off = p.NK - p.NQ;
+  const int TK = (p.NK + C::BK - 1) / C::BK;
+
+  int nsteps_mt[2];
+#pragma unroll
+  for (int mt = 0; mt < 2; ++mt) {
+    const int r0 = q0 + mt * C::BM;
+    int n = TK;
+    if (CAUSAL) {
+      const int lastkey = min(p.NK - 1, r0 + C::BM - 1 + off);
+      n = lastkey / C::BK + 1;
+    }
+    nsteps_mt[mt] = (r0 < p.NQ) ? n : 0;
+  }
+  const int nsteps = max(nsteps_mt[0], nsteps_mt[1]);
+
+  if (warp == 0 && lane == 0) {
+    tma_prefetch_desc(&tmQ1); tma_prefetch_desc(&tmK1); tma_prefetch_desc(&tmQ2); tma_prefetch_desc(&tmK2);
+  }
+  if (warp == 1 && lane == 0) {
+    mbar_init(q_full, 1);
+    for (int s = 0; s < C::NSTAGE; ++s) { mbar_init(&k_full[s], 1); mbar_init(&k_empty[s], 1); }
+    for (int i = 0; i < 4; ++i) { mbar_init(&s_full[i], 1); mbar_init(&s_empty[i], 4); }
+    fence_mbar_init();
+  }
+  if (warp == 2) tmem_alloc<C::TMEM_COLS>(tmem_ptr);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_ptr;
+
+  if (warp == 0) {
+    // ===================== TMA producer =====================
+    if (lane == 0) {
+      const uint64_t pol_q = l2_policy_evict_first(), pol_k = l2_policy_evict_last();
+      mbar_arrive_expect_tx(q_full, C::Q_BYTES);
+#pragma unroll
+      for (int mt = 0; mt < C::NMT; ++mt) {
+#pragma unroll
+        for (int kb = 0; kb < C::KB1; ++kb)
+          tma_load_3d_hint(sQ1 + (mt * C::KB1 + kb) * C::QBLK, &tmQ1, q_full, kb * 64, q0 + mt * C::BM, bh, pol_q);
+#pragma unroll
+        for (int kb = 0; kb < C::KB2; ++kb)
+          tma_load_3d_hint(sQ2 + (mt * C::KB2 + kb) * C::QBLK, &tmQ2, q_full, kb * 64, q0 + mt * C::BM, bh, pol_q);
+      }
+      for (int j = 0; j < nsteps; ++j) {
+        const int s = j % C::NSTAGE;
+        const uint32_t ph = (j / C::NSTAGE) & 1;
+        mbar_wait(&k_empty[s], ph ^ 1);
+        mbar_arrive_expect_tx(&k_full[s], C::STAGE_BYTES);
+        uint8_t* st = sK + s * C::STAGE_BYTES;
+#pragma unroll
+        for (int kb = 0; kb < C::KB1; ++kb) tma_load_3d_hint(st + kb * C::KBLK, &tmK1, &k_full[s], kb * 64, j * C::BK, bh, pol_k);
+#pragma unroll
+        for (int kb = 0; kb < C::KB2; ++kb)
+          tma_load_3d_hint(st + (C::KB1 + kb) * C::KBLK, &tmK2, &k_full[s], kb * 64, j * C::BK, bh, pol_k);
+      }
+    }
+  } else if (warp == 1) {
+    // ===================== MMA issuer =====================
+    if (lane == 0) {
+      constexpr uint32_t idesc = umma_idesc_bf16(C::BM, C::BK, 0, 0);
+      mbar_wait(q_full, 0);
+      tc_fence_after();
+      for (int j = 0; j < nsteps; ++j) {
+        const int s = j % C::NSTAGE;
+        const uint32_t ph = (j / C::NSTAGE) & 1;
+        mbar_wait(&k_full[s], ph);
+        tc_fence_after();
+        const uint32_t kaddr = smem_u32(sK + s * C::STAGE_BYTES);
+        const int st = j & 1;
+        const uint32_t sph = (j >> 1) & 1;
+#pragma unroll
+        for (int mt = 0; mt < C::NMT; ++mt) {
+          if (j < nsteps_mt[mt]) {
+            mbar_wait(&s_empty[mt * 2 + st], sph ^ 1);
+            tc_fence_after();
+            const uint32_t dS1 = tmem_base + (mt * 2 + st) * 128;
+            const uint32_t dS2 = dS1 + 64;
+            const uint32_t q1addr = smem_u32(sQ1 + mt * C::KB1 * C::QBLK);
+            const uint32_t q2addr = smem_u32(sQ2 + mt * C::KB2 * C::QBLK);
+#pragma unroll
+            for (int kb = 0; kb < C::KB1; ++kb)
+#pragma unroll
+              for (int k = 0; k < 4; ++k)
+                umma_bf16_ss(dS1, umma_smem_desc_sw128(q1addr + kb * C::QBLK + k * 32, 16, 1024),
+                             umma_smem_desc_sw128(kaddr + kb * C::KBLK + k * 32, 16, 1024), idesc, (kb | k) != 0);
+#pragma unroll
+            for (int kb = 0; kb < C::KB2; ++kb)
+#pragma unroll
+              for (int k = 0; k < 4; ++k)
+                umma_bf16_ss(dS2, umma_smem_desc_sw128(q2addr + kb * C::QBLK + k * 32, 16, 1024),
+                             umma_smem_desc_sw128(kaddr + (C::KB1 + kb) * C::KBLK + k * 32, 16, 1024), idesc, (kb | k) != 0);
+            umma_commit(&s_full[mt * 2 + st]);
+          }
+        }
+        umma_commit(&k_empty[s]);  // K stage reusable once every MMA that read it has retired
+      }
+    }
+  } else if (warp >= 4) {
+    // ===================== softmax warpgroups =====================
+    const int mt = (warp - 4) >> 2;
+    const int quarter = warp & 3;  // TMEM lane quarter this warp may access
+    const int row = q0 + mt * C::BM + quarter * 32 + lane;
+    const int limit = CAUSAL ? min(p.NK - 1, row + off) : p.NK - 1;  // last visible key of this row
+    const int first_row_limit = (q0 + mt * C::BM) + off;             // causal frontier of the tile's first row
+    RowState st{-CUDART_INF_F, -CUDART_INF_F, 0.f, 0.f, 0.f};
+    const int n = nsteps_mt[mt];
+    for (int j = 0; j < n; ++j) {
+      const int sg = j & 1;
+      const uint32_t sph = (j >> 1) & 1;
+      mbar_wait(&s_full[mt * 2 + sg], sph);
+      tc_fence_after();
+      const uint32_t taddr = tmem_base + (uint32_t(quarter * 32) << 16) + (mt * 2 + sg) * 128;
+      uint32_t r1[64], r2[64];
+      tmem_ld32(taddr, *reinterpret_cast<uint32_t(*)[32]>(&r1[0]));
+      tmem_ld32(taddr + 32, *reinterpret_cast<uint32_t(*)[32]>(&r1[32]));
+      tmem_ld32(taddr + 64, *reinterpret_cast<uint32_t(*)[32]>(&r2[0]));
+      tmem_ld32(taddr + 96, *reinterpret_cast<uint32_t(*)[32]>(&r2[32]));
+      tmem_wait_ld();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&s_empty[mt * 2 + sg]);  // logits are in registers: MMA may refill this stage
+      const int kbase = j * C::BK;
+      const bool masked = (CAUSAL && (kbase + C::BK - 1 > first_row_limit)) || (kbase + C::BK > p.NK);
+      if (masked) online_update64<true>(st, r1, r2, p.sc1, p.sc2, kbase, limit);
+      else        online_update64<false>(st, r1, r2, p.sc1, p.sc2, kbase, limit);
+    }
+    if (row < p.NQ) {
+      // Alg.1 lines 13-15 in natural-log units (R6): LSE = ln2*(m + log2 l); KL = ln2*acc/l1 + LSE2 - LSE1
+      const float LN2 = 0.6931471805599453f;
+      const float e1 = LN2 * (st.m1 + log2f(st.l1));
+      const float e2 = LN2 * (st.m2 + log2f(st.l2));
+      const size_t o = size_t(bh) * p.NQ + row;
+      p.lse1[o] = e1;
+      p.lse2[o] = e2;
+      p.kl[o] = fmaf(LN2, st.acc / st.l1, e2 - e1);
+    }
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 2) {
+    tc_fence_after();
+    tmem_dealloc<C::TMEM_COLS>(tmem_base);
+  }
+}
+
+}  // namespace skl

@@ -1,0 +1,104 @@
+"""CPU-side checks of the C-ABI boundary: the library builds, loads without a GPU, exports every symbol the header
+declares, validates arguments before touching the device, and refuses to compute without an sm_100 GPU
+(no CPU fallback).  No compute calls are made here."""
+from __future__ import annotations
+
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "streamkl.h")
+
+
+@pytest.fixture(scope="module")
+def L():
+    from paper_2606_20005_b200.build import build_library
+
+    build_library()
+    from paper_2606_20005_b200.binding import lib
+
+    return lib()
+
+
+def declared_functions():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(streamkl_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_header_declares_the_north_star_entry_points():
+    names = declared_functions()
+    for must in ("streamkl_fwd", "streamkl_bwd", "streamkl_fwd_f32", "streamkl_bwd_f32", "streamkl_bwd_workspace_bytes",
+                 "streamkl_fwd_host", "streamkl_fwd_bwd_host", "streamkl_strerror", "streamkl_version"):
+        assert must in names
+
+
+def test_every_declared_symbol_is_exported(L):
+    for name in declared_functions():
+        assert hasattr(L, name), f"{name} declared in include/streamkl.h but not exported"
+
+
+def test_binding_exposes_the_same_names():
+    import paper_2606_20005_b200 as skl
+
+    for name in declared_functions():
+        if name.endswith("_f32"):
+            continue  # the binding dispatches on the tensor dtype
+        assert hasattr(skl, name)
+
+
+def test_version_and_strerror(L):
+    assert b"sm_100a" in L.streamkl_version()
+    assert L.streamkl_strerror(0) == b"ok"
+    msgs = {L.streamkl_strerror(c) for c in range(-7, 1)}
+    assert len(msgs) == 8
+
+
+def _call_fwd(L, ptrs=(16, 16, 16, 16), B=1, H=1, NQ=8, NK=8, d1=64, d2=64, c1=0.125, c2=0.125, causal=0, outs=(16, 16, 16)):
+    return L.streamkl_fwd(*[ctypes.c_void_p(p) for p in ptrs], B, H, NQ, NK, d1, d2, c1, c2, causal,
+                          *[ctypes.c_void_p(p) for p in outs], ctypes.c_void_p(0))
+
+
+def test_argument_validation_happens_before_any_device_work(L):
+    ERR_NULL, ERR_SHAPE, ERR_ALIGN, ERR_SCALE, ERR_CUDA = -1, -2, -3, -4, -6
+    assert _call_fwd(L, NK=0) == ERR_SHAPE
+    assert _call_fwd(L, d1=0) == ERR_SHAPE
+    assert _call_fwd(L, d2=300) == ERR_SHAPE
+    assert _call_fwd(L, NQ=9, NK=8, causal=1) == ERR_SHAPE      # R5: causal needs NQ <= NK
+    assert _call_fwd(L, c1=0.0) == ERR_SCALE
+    assert _call_fwd(L, c2=float("nan")) == ERR_SCALE
+    assert _call_fwd(L, ptrs=(0, 16, 16, 16)) == ERR_NULL
+    assert _call_fwd(L, ptrs=(16, 24, 16, 16)) == ERR_ALIGN
+    assert _call_fwd(L, outs=(0, 16, 16)) == ERR_NULL
+    assert _call_fwd(L, B=0) == 0                                 # empty batch: successful no-op
+    assert _call_fwd(L, NQ=0) == 0
+
+
+def test_no_gpu_means_error_not_fallback(L):
+    import torch
+
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    assert _call_fwd(L) == -6  # STREAMKL_ERR_CUDA: the product path never computes on the CPU
+    import paper_2606_20005_b200 as skl
+
+    a = np.zeros((1, 1, 4, 64), np.float32)
+    with pytest.raises(skl.StreamKLError):
+        skl.streamkl_fwd_host(a, a, a, a, 0.125, 0.125, False)
+
+
+def test_bwd_teacher_pointers_must_come_in_pairs(L):
+    vp = ctypes.c_void_p
+    rc = L.streamkl_bwd(vp(16), vp(16), vp(16), vp(16), 1, 1, 8, 8, 64, 64, 0.125, 0.125, 0, vp(16), vp(16), vp(16), vp(16),
+                        vp(16), vp(0), vp(16), vp(16), vp(0), 0, vp(0))
+    assert rc == -1
+
+
+def test_workspace_is_never_quadratic(L):
+    small = L.streamkl_bwd_workspace_bytes(1, 32, 4096, 4096, 128, 128, 1)
+    big = L.streamkl_bwd_workspace_bytes(1, 32, 65536, 65536, 128, 128, 1)
+    assert big <= 16 * max(small, 1) + 4 * 32 * 65536 * 256 * 4  # O((NQ+NK) d), not O(NQ NK)
