@@ -3,6 +3,7 @@
 // Only what the kernels need; all names are ours.
 #pragma once
 #include <cstdint>
+#include <cstdio>
 #include <cuda.h>
 
 namespace skl {
