@@ -1,0 +1,452 @@
+#!/usr/bin/env python
+"""bench.py -- StreamKL hot path on B200: one JSON line per run (driver contract).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4|cfg3|cfg2|cfg5] [--impl reference]
+
+A "step" is ONE pass of the whole hot path over one batch of the workload: streamkl_fwd (F1-F6 of DESIGN.md) followed
+by streamkl_bwd (B1-B6; teacher gradients too where the config asks for them).  The default workload is BASELINE.json's
+64K configuration (configs[3]: B=1, H=32, NQ=NK=65536, d=128/128, bf16, causal), the larger of the two sizes the metric
+is quoted on; the 16K one (configs[2]) is timed beside it and reported under "also".
+  value   = algorithmic TFLOP/s of the step (fwd 2*pairs*(d1+d2) + bwd 2*pairs*((d1+d2)+2*d2+2*d1), pairs = NQ*NK/2 causal),
+            all ranks' work / max-over-ranks device time, inputs resident in HBM.
+  e2e     = the same metric through streamkl_fwd_bwd_host: pinned HOST buffers, host<->device copies inside the timed region.
+  roofline= the dominant kernel's achieved tensor TFLOP/s (its algorithmic FLOPs / its average CUDA-event duration inside
+            the timed region) against the measured dense bf16 peak of MEASURED_PEAKS.json.
+  cpu_baseline = the float64 oracle, as it stands, timed on this box's host cores on a bounded row sample of the workload.
+With N > 1 (torchrun) every rank runs its own batch of the same shape (heads are independent: no collective on the data
+path) -> "scaling": "weak".  `--impl reference` times the oracle alone (rank 0), same metric and config.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import workloads as W  # noqa: E402
+
+METRIC = "attn-KL fwd+bwd step throughput (H=32, N=64K, bf16, causal; fwd/bwd ms and % of B200 bf16 peak in detail)"
+UNIT = "TFLOP/s"
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+SPEC_BF16_TFLOPS = 2250.0
+WORKLOADS = {"cfg2": 2, "cfg3": 3, "cfg4": 4, "cfg5": 5}
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            d = json.load(fh)
+        d["_source"] = "measured"
+        return d
+    d = dict(FALLBACK_PEAKS)
+    d["_source"] = "fallback"
+    return d
+
+
+def cfg_json(cfg: W.Config, world: int):
+    return {
+        "workload": f"cfg{cfg.idx} {cfg.name}: B={cfg.B} H={cfg.H} NQ={cfg.NQ} NK={cfg.NK} d1={cfg.d1} d2={cfg.d2} "
+                    f"{cfg.dtype} {'causal' if cfg.causal else 'no-mask'}; step = streamkl_fwd + streamkl_bwd"
+                    f"({'dQ1,dK1,dQ2,dK2' if cfg.teacher_grads else 'dQ2,dK2'})",
+        "batch_per_gpu": cfg.BH, "global_batch": cfg.BH * world, "seq_len": cfg.NQ,
+        "parallelism": f"independent (b,h) replicas x{world}" if world > 1 else "single GPU",
+        "l2": "inputs larger than L2 (no flush)" if input_bytes(cfg) > 200e6 else "L2 flushed between steps",
+    }
+
+
+def input_bytes(cfg: W.Config) -> int:
+    es = 2 if cfg.dtype == "bf16" else 4
+    return cfg.BH * ((cfg.NQ + cfg.NK) * (cfg.d1 + cfg.d2) * es + cfg.NQ * 4)
+
+
+def output_bytes(cfg: W.Config) -> int:
+    es = 2 if cfg.dtype == "bf16" else 4
+    b = cfg.BH * (3 * cfg.NQ * 4 + (cfg.NQ + cfg.NK) * cfg.d2 * es)
+    if cfg.teacher_grads:
+        b += cfg.BH * (cfg.NQ + cfg.NK) * cfg.d1 * es
+    return b
+
+
+def gen_inputs(cfg: W.Config, rank: int):
+    """Seeded host inputs of this rank's batch: batch index b is offset by rank*B so ranks hold different data."""
+    from concurrent.futures import ThreadPoolExecutor
+
+    heads = [(rank * cfg.B + b, h) for b in range(cfg.B) for h in range(cfg.H)]
+    with ThreadPoolExecutor(max_workers=min(16, os.cpu_count() or 1)) as ex:
+        per = list(ex.map(lambda bh: W.head_inputs(cfg, *bh), heads))
+    out = {}
+    for k in ("Q1", "K1", "Q2", "K2", "g"):
+        a = np.stack([p[k] for p in per])
+        out[k] = a.reshape((cfg.B, cfg.H) + a.shape[1:])
+    return out
+
+
+# ------------------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    """Samples SM clock / power / throttle reasons of one GPU through NVML while a timed region runs."""
+
+    BITS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+            0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x100: "display_clock_setting",
+            0x10: "sync_boost"}
+
+    def __init__(self, index: int):
+        self.samples, self.power, self.reasons = [], [], set()
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._thr = None
+        try:
+            import pynvml
+
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = int(vis.split(",")[index]) if vis and vis.split(",")[index].isdigit() else index
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:  # noqa: BLE001 - NVML missing: report nulls, never fail the bench
+            self.nv = None
+
+    def _run(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(float(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+                r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                for bit, name in self.BITS.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:  # noqa: BLE001
+                pass
+            time.sleep(0.02)
+
+    def __enter__(self):
+        if self.nv is not None:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr is not None:
+            self._thr.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": [], "samples": 0}
+        return {"sm_mhz": statistics.median(self.samples), "sm_min_mhz": min(self.samples), "sm_max_mhz": self.max_mhz,
+                "power_w_max": max(self.power) if self.power else None, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------------------ oracle legs
+def oracle_sample(cfg: W.Config, budget_s: float, rows_per_block: int = 256, max_blocks: int = 64):
+    """Time the float64 oracle (oracle/streamkl_oracle.py, untouched) on evenly spread row blocks of head (0,0).
+
+    Returns (tflops, seconds, flops, description).  Work counted = the visible pairs of the sampled rows, with the same
+    per-pair FLOP convention as the GPU number."""
+    from oracle.streamkl_oracle import attention_kl_rows
+
+    inp = W.head_inputs(cfg, 0, 0)
+    Q1, K1, Q2, K2 = (W.widen_f64(inp[k]) for k in ("Q1", "K1", "Q2", "K2"))
+    g = inp["g"].astype(np.float64)
+    nblk_total = max(1, cfg.NQ // rows_per_block)
+    # visit blocks in a low-discrepancy order so that any prefix is spread over the causal triangle
+    order = sorted(range(nblk_total), key=lambda i: int(format(i, "032b")[::-1], 2))
+    mac = (cfg.d1 + cfg.d2) + (cfg.d1 + cfg.d2) + 2 * cfg.d2 + (2 * cfg.d1 if cfg.teacher_grads else 0)  # fwd + bwd
+    off = cfg.NK - cfg.NQ
+    flops, rows_done, t0 = 0.0, 0, time.perf_counter()
+    nb = 0
+    for bi in order[:max_blocks]:
+        rows = np.arange(bi * rows_per_block, min(cfg.NQ, (bi + 1) * rows_per_block))
+        attention_kl_rows(Q1, K1, Q2, K2, cfg.c1, cfg.c2, cfg.causal, rows, g, cfg.teacher_grads)
+        vis = (np.minimum(rows + off + 1, cfg.NK)).sum() if cfg.causal else len(rows) * cfg.NK
+        flops += 2.0 * float(vis) * mac
+        rows_done += len(rows)
+        nb += 1
+        if time.perf_counter() - t0 >= budget_s:
+            break
+    dt = time.perf_counter() - t0
+    desc = (f"{nb} blocks of {rows_per_block} query rows (bit-reversed spread over NQ) of head (b=0,h=0) of cfg{cfg.idx}, "
+            f"fwd+bwd by the float64 definition incl. this block's dK contribution; {rows_done} rows, {dt:.1f} s")
+    return flops / dt / 1e12, dt, flops, desc
+
+
+def host_threads() -> int:
+    try:
+        from threadpoolctl import threadpool_info
+
+        n = [i.get("num_threads", 1) for i in threadpool_info() if i.get("user_api") == "blas"]
+        if n:
+            return int(max(n))
+    except Exception:  # noqa: BLE001
+        pass
+    return os.cpu_count() or 1
+
+
+def run_reference(args, cfg: W.Config, rank: int, world: int):
+    """--impl reference: the oracle alone, K steps, each a bounded sample (one 256-row block per step)."""
+    if rank != 0:
+        return
+    per_step = max(1.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    vals, secs = [], []
+    desc = ""
+    for i in range(args.warmup + args.steps):
+        tf, dt, _, desc = oracle_sample(cfg, budget_s=per_step, max_blocks=8)
+        if i >= args.warmup:
+            vals.append(tf)
+            secs.append(dt)
+    v = float(np.mean(vals))
+    line = {
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(secs)), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg_json(cfg, 1),
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": host_threads(), "kind": "oracle", "sample": "each step: " + desc},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------ GPU legs
+def to_dev(a: np.ndarray):
+    import torch
+
+    if a.dtype == np.uint16:
+        return torch.from_numpy(a.view(np.int16)).view(torch.bfloat16).cuda(non_blocking=False)
+    return torch.from_numpy(a).cuda()
+
+
+def pinned_like(a: np.ndarray):
+    """A pinned host numpy array holding a copy of `a` (torch owns the pinned allocation)."""
+    import torch
+
+    t = torch.empty(a.shape, dtype=torch.int16 if a.dtype == np.uint16 else torch.float32, pin_memory=True)
+    v = t.numpy().view(a.dtype)
+    v[...] = a
+    return t, v
+
+
+def pinned_empty(shape, dtype):
+    import torch
+
+    t = torch.empty(shape, dtype=torch.int16 if dtype == np.uint16 else torch.float32, pin_memory=True)
+    return t, t.numpy().view(dtype)
+
+
+def time_passes(skl, cfg, dev, steps, warmup, barrier):
+    """K timed steps (fwd + bwd) on device-resident inputs.  Returns dict(step_ms, fwd_ms, bwd_ms, kernels, launches)."""
+    import torch
+
+    Q1, K1, Q2, K2, g = dev
+    teacher = cfg.teacher_grads
+    kl, l1, l2 = skl.streamkl_fwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, cfg.causal)
+    grads = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, cfg.causal, kl, l1, l2, g, teacher=teacher)
+    need = skl.streamkl_bwd_workspace_bytes(cfg.B, cfg.H, cfg.NQ, cfg.NK, cfg.d1, cfg.d2, teacher)
+    ws = torch.empty(max(need, 1), dtype=torch.uint8, device="cuda")
+
+    def step():
+        skl.streamkl_fwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, cfg.causal, kl, l1, l2)
+        n = skl.streamkl_last_launch_count()
+        skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, cfg.causal, kl, l1, l2, g, teacher=teacher, dQ1=grads[0], dK1=grads[1],
+                         dQ2=grads[2], dK2=grads[3], workspace=ws)
+        return n + skl.streamkl_last_launch_count()
+
+    for _ in range(warmup):
+        step()
+    torch.cuda.synchronize()
+    barrier()
+    torch.cuda.synchronize()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+    skl.streamkl_profile_enable(True)
+    launches = 0
+    ev[0].record()
+    for _ in range(steps):
+        launches += step()
+    ev[1].record()
+    torch.cuda.synchronize()
+    barrier()
+    torch.cuda.synchronize()
+    skl.streamkl_profile_enable(False)
+    total_ms = ev[0].elapsed_time(ev[1])
+    recs = skl.streamkl_profile_collect()
+    kernels = {}
+    for name, ms in recs:
+        kernels.setdefault(name, []).append(ms)
+    fwd_ms = sum(sum(v) for k, v in kernels.items() if "fwd" in k) / steps
+    bwd_ms = sum(sum(v) for k, v in kernels.items() if "bwd" in k) / steps
+    return {"step_ms": total_ms / steps, "fwd_ms": fwd_ms, "bwd_ms": bwd_ms, "launches": launches,
+            "kernels": {k: {"launches_per_step": len(v) / steps, "avg_ms": sum(v) / len(v), "min_ms": min(v)} for k, v in kernels.items()},
+            "outputs": (kl, l1, l2, grads), "workspace_bytes": need}
+
+
+def kernel_flops(cfg: W.Config, name: str) -> float:
+    """Algorithmic tensor FLOPs ONE launch of kernel `name` performs ('Algorithmic work per kernel')."""
+    pairs = cfg.visible_pairs_convention()
+    if "fwd" in name:
+        return 2.0 * pairs * (cfg.d1 + cfg.d2)
+    t = cfg.teacher_grads
+    # each backward kernel recomputes both logit tiles and runs one gradient GEMM per distribution it differentiates
+    return 2.0 * pairs * ((cfg.d1 + cfg.d2) + cfg.d2 + (cfg.d1 if t else 0))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="streamkl", choices=["streamkl", "reference"])
+    ap.add_argument("--workload", default="cfg4", choices=sorted(WORKLOADS))
+    ap.add_argument("--no-also", action="store_true", help="skip the secondary 16K measurement")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiling runs)")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "streamkl" else args.warmup
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    cfg = W.CONFIGS[WORKLOADS[args.workload]]
+
+    if args.impl == "reference":
+        run_reference(args, cfg, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_2606_20005_b200 as skl  # fails loudly if libstreamkl.so is missing: no CPU fallback
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a B200: the StreamKL hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+
+    def max_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    pk = peaks()
+    host = gen_inputs(cfg, rank)
+    dev = tuple(to_dev(host[k]) for k in ("Q1", "K1", "Q2", "K2", "g"))
+    torch.cuda.synchronize()
+    base_mem = torch.cuda.memory_allocated()
+    torch.cuda.reset_peak_memory_stats()
+
+    with ClockSampler(local) as clk:
+        res = time_passes(skl, cfg, dev, args.steps, args.warmup, barrier)
+    step_ms = max_over_ranks(res["step_ms"])
+    flop_f, flop_b = cfg.fwd_flop(), cfg.bwd_flop()
+    value = world * (flop_f + flop_b) / (step_ms * 1e-3) / 1e12
+    extra_hbm = torch.cuda.max_memory_allocated() - base_mem
+
+    # ---- roofline of the dominant kernel (largest share of the step), from the events recorded inside the timed region
+    dom = max(res["kernels"].items(), key=lambda kv: kv[1]["avg_ms"] * kv[1]["launches_per_step"])
+    dom_name, dom_stat = dom
+    peak_tf = float(pk["bf16_tflops_sustained"] if step_ms * args.steps > 1000.0 else pk["bf16_tflops"])
+    ach = kernel_flops(cfg, dom_name) / (dom_stat["avg_ms"] * 1e-3) / 1e12
+    roofline = {"bound": "tensor", "kernel": dom_name, "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
+                "traffic": None, "peak_source": f"{pk['_source']} bf16 "
+                + ("sustained" if step_ms * args.steps > 1000.0 else "burst") + " (MEASURED_PEAKS.json)",
+                "share_of_step": dom_stat["avg_ms"] * dom_stat["launches_per_step"] / res["step_ms"],
+                "avg_ms": dom_stat["avg_ms"]}
+
+    detail = {
+        "fwd_ms": res["fwd_ms"], "bwd_ms": res["bwd_ms"],
+        "fwd_tflops": flop_f / (res["fwd_ms"] * 1e-3) / 1e12, "bwd_tflops": flop_b / (res["bwd_ms"] * 1e-3) / 1e12,
+        "fwd_frac_of_measured_bf16_burst": flop_f / (res["fwd_ms"] * 1e-3) / 1e12 / float(pk["bf16_tflops"]),
+        "fwd_frac_of_spec_2250": flop_f / (res["fwd_ms"] * 1e-3) / 1e12 / SPEC_BF16_TFLOPS,
+        "fwd_exp_per_s": 2.0 * cfg.visible_pairs_convention() / (res["fwd_ms"] * 1e-3),
+        "kernels": res["kernels"],
+        "extra_hbm_bytes": {"total_peak_over_inputs": int(extra_hbm), "outputs": output_bytes(cfg),
+                            "workspace": int(res["workspace_bytes"])},
+    }
+
+    # ---- secondary: the 16K configuration the metric also names
+    also = {}
+    if not args.no_also and args.workload == "cfg4":
+        c3 = W.CONFIGS[3]
+        h3 = gen_inputs(c3, rank)
+        d3 = tuple(to_dev(h3[k]) for k in ("Q1", "K1", "Q2", "K2", "g"))
+        r3 = time_passes(skl, c3, d3, max(args.steps, 10), args.warmup, barrier)
+        also["cfg3 indexer 16K (H=32, d=128/64, causal, dQ2,dK2 only)"] = {
+            "fwd_ms": r3["fwd_ms"], "bwd_ms": r3["bwd_ms"], "fwd_tflops": c3.fwd_flop() / (r3["fwd_ms"] * 1e-3) / 1e12,
+            "bwd_tflops": c3.bwd_flop() / (r3["bwd_ms"] * 1e-3) / 1e12,
+            "fwd_frac_of_measured_bf16_burst": c3.fwd_flop() / (r3["fwd_ms"] * 1e-3) / 1e12 / float(pk["bf16_tflops"])}
+        del d3, h3, r3
+
+    # ---- e2e: host buffers through streamkl_fwd_bwd_host (copies inside the timed region)
+    e2e = None
+    if not args.no_e2e:
+        del res["outputs"]
+        keep = {}
+        pins = {}
+        for k in ("Q1", "K1", "Q2", "K2", "g"):
+            keep[k], pins[k] = pinned_like(host[k])
+        st = np.uint16 if cfg.dtype == "bf16" else np.float32
+        out = {}
+        spec = {"kl": ((cfg.B, cfg.H, cfg.NQ), np.float32), "lse1": ((cfg.B, cfg.H, cfg.NQ), np.float32),
+                "lse2": ((cfg.B, cfg.H, cfg.NQ), np.float32), "dQ2": ((cfg.B, cfg.H, cfg.NQ, cfg.d2), st),
+                "dK2": ((cfg.B, cfg.H, cfg.NK, cfg.d2), st)}
+        if cfg.teacher_grads:
+            spec["dQ1"] = ((cfg.B, cfg.H, cfg.NQ, cfg.d1), st)
+            spec["dK1"] = ((cfg.B, cfg.H, cfg.NK, cfg.d1), st)
+        for k, (shp, dt) in spec.items():
+            keep["o" + k], out[k] = pinned_empty(shp, dt)
+        del dev
+        torch.cuda.empty_cache()
+        n_e2e = max(1, min(args.steps, 5))
+        for _ in range(2):
+            skl.streamkl_fwd_bwd_host(pins["Q1"], pins["K1"], pins["Q2"], pins["K2"], cfg.c1, cfg.c2, cfg.causal, pins["g"],
+                                      teacher=cfg.teacher_grads, out=out)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(n_e2e):
+            skl.streamkl_fwd_bwd_host(pins["Q1"], pins["K1"], pins["Q2"], pins["K2"], cfg.c1, cfg.c2, cfg.causal, pins["g"],
+                                      teacher=cfg.teacher_grads, out=out)
+        e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3 / n_e2e)
+        barrier()
+        e2e = {"value": world * (flop_f + flop_b) / (e2e_ms * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": e2e_ms, "steps": n_e2e,
+               "h2d_bytes_per_step": input_bytes(cfg), "d2h_bytes_per_step": output_bytes(cfg),
+               "api": "streamkl_fwd_bwd_host (pinned host buffers; cudaMalloc, H2D, fwd, bwd, D2H, cudaFree inside the call)",
+               "check_mean_kl": float(out["kl"].mean())}
+
+    # ---- cpu baseline: the oracle as it stands, bounded sample, rank 0 at N=1 only
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        tf, dt, _, desc = oracle_sample(cfg, budget_s=15.0)
+        cpu = {"value": tf, "unit": UNIT, "cores": host_threads(), "kind": "oracle", "sample": desc, "seconds": dt}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+            "data": "synthetic (seeded N(0,1) per BASELINE.json configs; workloads.py)", "config": cfg_json(cfg, world),
+            "clocks": clk.summary(), "e2e": e2e, "gpu_launches": res["launches"], "roofline": roofline, "cpu_baseline": cpu,
+            "detail": detail, "also": also, "peaks": {k: pk.get(k) for k in ("bf16_tflops", "bf16_tflops_sustained", "hbm_gbs", "_source")},
+            "library": skl.streamkl_version(),
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -110,6 +110,18 @@ int streamkl_fwd_bwd_host(int dtype, const void* Q1, const void* K1, const void*
 /* Number of kernels the last successful streamkl_* call on this thread launched (for launch accounting). */
 int streamkl_last_launch_count(void);
 
+/*
+ * Per-kernel timing, a measurement aid (bench.py's roofline block uses it).  streamkl_profile_enable(1) makes every
+ * later kernel launch from the calling thread record a CUDA event on the launch stream immediately before and after
+ * the kernel; streamkl_profile_collect() synchronises those events, writes up to max_records (kernel id, milliseconds)
+ * pairs in launch order, forgets them and returns how many it wrote (or a negative STREAMKL_ERR_* code).
+ * streamkl_kernel_name() maps a kernel id to the kernel's name (static string).  Disabled by default; when disabled
+ * the launch path does not touch events at all.
+ */
+int streamkl_profile_enable(int on);
+int streamkl_profile_collect(int max_records, int* kernel_ids, float* ms);
+const char* streamkl_kernel_name(int kernel_id);
+
 const char* streamkl_strerror(int code);
 const char* streamkl_version(void);
 

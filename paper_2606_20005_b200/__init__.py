@@ -13,7 +13,10 @@ from .binding import (  # noqa: F401
     streamkl_fwd,
     streamkl_fwd_bwd_host,
     streamkl_fwd_host,
+    streamkl_kernel_name,
     streamkl_last_launch_count,
+    streamkl_profile_collect,
+    streamkl_profile_enable,
     streamkl_strerror,
     streamkl_version,
 )

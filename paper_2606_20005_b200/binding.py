@@ -15,6 +15,7 @@ from .build import LIB_PATH
 __all__ = [
     "StreamKLError", "lib", "lib_path", "streamkl_fwd", "streamkl_bwd", "streamkl_bwd_workspace_bytes",
     "streamkl_fwd_host", "streamkl_fwd_bwd_host", "streamkl_last_launch_count", "streamkl_strerror",
+    "streamkl_profile_enable", "streamkl_profile_collect", "streamkl_kernel_name",
     "streamkl_version",
 ]
 
@@ -62,6 +63,12 @@ def lib() -> ctypes.CDLL:
     L.streamkl_fwd_bwd_host.restype = ci
     L.streamkl_last_launch_count.argtypes = []
     L.streamkl_last_launch_count.restype = ci
+    L.streamkl_profile_enable.argtypes = [ci]
+    L.streamkl_profile_enable.restype = ci
+    L.streamkl_profile_collect.argtypes = [ci, vp, vp]
+    L.streamkl_profile_collect.restype = ci
+    L.streamkl_kernel_name.argtypes = [ci]
+    L.streamkl_kernel_name.restype = ctypes.c_char_p
     L.streamkl_strerror.argtypes = [ci]
     L.streamkl_strerror.restype = ctypes.c_char_p
     L.streamkl_version.argtypes = []
@@ -80,6 +87,24 @@ def streamkl_version() -> str:
 
 def streamkl_last_launch_count() -> int:
     return int(lib().streamkl_last_launch_count())
+
+
+def streamkl_profile_enable(on: bool) -> None:
+    lib().streamkl_profile_enable(int(bool(on)))
+
+
+def streamkl_profile_collect(max_records: int = 4096):
+    """-> list of (kernel_name, ms) for every kernel launched on this thread since profiling was enabled / last collected."""
+    ids = (ctypes.c_int * max_records)()
+    ms = (ctypes.c_float * max_records)()
+    n = lib().streamkl_profile_collect(max_records, ctypes.cast(ids, ctypes.c_void_p), ctypes.cast(ms, ctypes.c_void_p))
+    if n < 0:
+        raise StreamKLError(n, "streamkl_profile_collect")
+    return [(lib().streamkl_kernel_name(ids[i]).decode(), float(ms[i])) for i in range(n)]
+
+
+def streamkl_kernel_name(kernel_id: int) -> str:
+    return lib().streamkl_kernel_name(int(kernel_id)).decode()
 
 
 def streamkl_bwd_workspace_bytes(B, H, NQ, NK, d1, d2, want_teacher_grads) -> int:

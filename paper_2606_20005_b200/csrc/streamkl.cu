@@ -7,6 +7,7 @@
 #include <cmath>
 #include <cstdint>
 #include <cstring>
+#include <vector>
 
 #include "../../include/streamkl.h"
 #include "streamkl_fwd_sm100.cuh"
@@ -16,6 +17,28 @@
 namespace {
 
 thread_local int g_last_launches = 0;
+
+// ---- optional per-kernel timing (streamkl_profile_*): CUDA events recorded on the launch stream around every kernel
+enum KernelId { KID_FWD_TC = 0, KID_BWD_DQ_TC, KID_BWD_DK_TC, KID_FWD_SIMT, KID_BWD_DQ_SIMT, KID_BWD_DK_SIMT, KID_COUNT };
+const char* const kKernelNames[KID_COUNT] = {"streamkl_fwd_sm100_kernel", "streamkl_bwd_sm100_kernel<OWNER_Q>",
+                                             "streamkl_bwd_sm100_kernel<OWNER_K>", "streamkl_fwd_simt_kernel",
+                                             "streamkl_bwd_simt_kernel<OWNER_Q>", "streamkl_bwd_simt_kernel<OWNER_K>"};
+struct ProfRecord { int id; cudaEvent_t a, b; };
+thread_local bool g_prof_on = false;
+thread_local std::vector<ProfRecord>* g_prof = nullptr;
+
+struct ProfScope {  // brackets ONE kernel launch; a no-op unless profiling is enabled on this thread
+  cudaStream_t st; cudaEvent_t b = nullptr;
+  ProfScope(int id, cudaStream_t s) : st(s) {
+    if (!g_prof_on) return;
+    if (!g_prof) g_prof = new std::vector<ProfRecord>();
+    cudaEvent_t a = nullptr;
+    if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { cudaGetLastError(); b = nullptr; return; }
+    cudaEventRecord(a, st);
+    g_prof->push_back({id, a, b});
+  }
+  ~ProfScope() { if (b) cudaEventRecord(b, st); }
+};
 
 using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                    const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -98,7 +121,10 @@ int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2
   p.kl = kl; p.lse1 = lse1; p.lse2 = lse2;
   const long long grid = (long long)p.TQ * s.BH;
   if (grid > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
-  kern<<<dim3((unsigned)grid), C::THREADS, C::SMEM_BYTES, stream>>>(tQ1, tK1, tQ2, tK2, p);
+  {
+    ProfScope ps(KID_FWD_TC, stream);
+    kern<<<dim3((unsigned)grid), C::THREADS, C::SMEM_BYTES, stream>>>(tQ1, tK1, tQ2, tK2, p);
+  }
   if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
   g_last_launches += 1;
   return STREAMKL_OK;
@@ -125,8 +151,11 @@ int launch_fwd_simt(const void* Q1, const void* K1, const void* Q2, const void* 
   }
   skl::SimtParams p{s.NQ, s.NK, s.d1, s.d2, s.causal, s.c1, s.c2};
   dim3 grid((s.NQ + br - 1) / br, (unsigned)s.BH);
-  kern<<<grid, br, smem, stream>>>(static_cast<const T*>(Q1), static_cast<const T*>(K1), static_cast<const T*>(Q2),
-                                   static_cast<const T*>(K2), p, kl, lse1, lse2);
+  {
+    ProfScope ps(KID_FWD_SIMT, stream);
+    kern<<<grid, br, smem, stream>>>(static_cast<const T*>(Q1), static_cast<const T*>(K1), static_cast<const T*>(Q2),
+                                     static_cast<const T*>(K2), p, kl, lse1, lse2);
+  }
   if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
   g_last_launches += 1;
   return STREAMKL_OK;
@@ -173,8 +202,11 @@ int launch_bwd_simt(const void* Q1, const void* K1, const void* Q2, const void* 
   skl::SimtParams p{s.NQ, s.NK, s.d1, s.d2, s.causal, s.c1, s.c2};
   const int NX = OWNER_K ? s.NK : s.NQ;
   dim3 grid((NX + br - 1) / br, (unsigned)s.BH);
-  kern<<<grid, br, smem, stream>>>(static_cast<const T*>(Q1), static_cast<const T*>(K1), static_cast<const T*>(Q2),
-                                   static_cast<const T*>(K2), p, kl, lse1, lse2, dkl, static_cast<T*>(dX1), static_cast<T*>(dX2));
+  {
+    ProfScope ps(OWNER_K ? KID_BWD_DK_SIMT : KID_BWD_DQ_SIMT, stream);
+    kern<<<grid, br, smem, stream>>>(static_cast<const T*>(Q1), static_cast<const T*>(K1), static_cast<const T*>(Q2),
+                                     static_cast<const T*>(K2), p, kl, lse1, lse2, dkl, static_cast<T*>(dX1), static_cast<T*>(dX2));
+  }
   if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
   g_last_launches += 1;
   return STREAMKL_OK;
@@ -204,7 +236,10 @@ int launch_bwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2
   p.dX2 = static_cast<__nv_bfloat16*>(dX2);
   const long long grid = (long long)p.TX * s.BH;
   if (grid > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
-  kern<<<dim3((unsigned)grid), C::THREADS, C::SMEM_BYTES, stream>>>(tQ1, tK1, tQ2, tK2, p);
+  {
+    ProfScope ps(OWNER_K ? KID_BWD_DK_TC : KID_BWD_DQ_TC, stream);
+    kern<<<dim3((unsigned)grid), C::THREADS, C::SMEM_BYTES, stream>>>(tQ1, tK1, tQ2, tK2, p);
+  }
   if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
   g_last_launches += 1;
   return STREAMKL_OK;
@@ -373,6 +408,30 @@ int streamkl_fwd_bwd_host(int dtype, const void* Q1, const void* K1, const void*
 }
 
 int streamkl_last_launch_count(void) { return g_last_launches; }
+
+int streamkl_profile_enable(int on) {
+  g_prof_on = on != 0;
+  return STREAMKL_OK;
+}
+
+int streamkl_profile_collect(int max_records, int* kernel_ids, float* ms) {
+  if (max_records < 0 || (max_records > 0 && (!kernel_ids || !ms))) return STREAMKL_ERR_NULLPTR;
+  if (!g_prof) return 0;
+  int n = 0, rc = 0;
+  for (ProfRecord& r : *g_prof) {
+    float t = 0.f;
+    if (cudaEventSynchronize(r.b) != cudaSuccess || cudaEventElapsedTime(&t, r.a, r.b) != cudaSuccess) { cudaGetLastError(); rc = STREAMKL_ERR_CUDA; }
+    else if (n < max_records) { kernel_ids[n] = r.id; ms[n] = t; ++n; }
+    cudaEventDestroy(r.a);
+    cudaEventDestroy(r.b);
+  }
+  g_prof->clear();
+  return rc < 0 ? rc : n;
+}
+
+const char* streamkl_kernel_name(int kernel_id) {
+  return (kernel_id >= 0 && kernel_id < KID_COUNT) ? kKernelNames[kernel_id] : "unknown kernel id";
+}
 
 const char* streamkl_strerror(int code) {
   switch (code) {

@@ -59,6 +59,11 @@ class Config:
         off = self.NK - self.NQ  # row i sees keys 0..i+off  (i+off+1 <= NK for every row)
         return self.BH * (self.NQ * (off + 1) + self.NQ * (self.NQ - 1) // 2)
 
+    def visible_pairs_convention(self) -> float:
+        """(query,key) pairs under BASELINE.json's FLOP convention: NQ*NK per head, halved for causal."""
+        p = float(self.BH) * self.NQ * self.NK
+        return p / 2 if self.causal else p
+
     def fwd_flop(self) -> float:
         """BASELINE.json convention: 2*NQ*NK*(d1+d2) per head, halved for causal."""
         f = 2.0 * self.BH * self.NQ * self.NK * (self.d1 + self.d2)
