@@ -4,12 +4,15 @@
 //   warp 0      TMA producer : Q1,Q2 once; K1_j,K2_j through an NSTAGE ring          (F1, F2 of DESIGN.md)
 //   warp 1      MMA issuer   : S1 = Q1 K1_j^T, S2 = Q2 K2_j^T, tcgen05.mma -> TMEM    (F3)
 //   warp 2      TMEM allocator
-//   warps 4-7   softmax warpgroup of M-tile 0: thread = one query row                   (F4, F5, F6)
-//   warps 8-11  softmax warpgroup of M-tile 1
-// TMEM (512 columns): per M-tile two stages of {S1 (64 cols), S2 (64 cols)}.  A softmax thread pulls its whole
-// 64+64-logit row into registers, releases the TMEM stage at once (so the next tile's MMA overlaps the exp work)
-// and then performs the online update of (m1,l1,m2,l2,acc) -- Eq.9-10 -- entirely thread-locally in the log2
-// domain (exp2 instead of exp; R6).
+//   warps 4-19  sixteen softmax warps = 2 M-tiles x 2 column halves x 4 TMEM lane quarters          (F4, F5, F6)
+// TMEM (512 columns): per M-tile two stages of {S1 (64 cols), S2 (64 cols)}.  A softmax thread owns ONE query row and
+// ONE 32-column half of every key tile: it pulls its 32+32 logits into registers, releases the TMEM stage at once (so
+// the next tile's MMA overlaps the exp work) and performs the online update of its own partial (m1,l1,m2,l2,acc) --
+// Eq.9-10 -- entirely thread-locally in the log2 domain (exp2 instead of exp; R6).  The two
+// column halves of a row are independent partial statistics over disjoint key sets; they are merged once, after the
+// last tile, with the associative merge of Eq.11 (carrying (m2,l2) too: R11).  Four softmax warps per
+// SM sub-partition (instead of two) keep the MUFU pipe fed while other warps sit in their no-exp phases (TMEM load,
+// running-max reduction): DESIGN.md "forward kernel".
 #pragma once
 #include <cuda_bf16.h>
 #include <math_constants.h>
@@ -36,7 +39,9 @@ struct FwdCfg {
   static constexpr int NSTAGE = NSTAGE_RAW > 6 ? 6 : NSTAGE_RAW;
   static_assert(NSTAGE >= 2, "need at least a double-buffered K ring");
   static constexpr int SMEM_BYTES = 1024 + Q_BYTES + NSTAGE * STAGE_BYTES + AUX_BYTES;
-  static constexpr int THREADS = 384;
+  static constexpr int NHALF = 2;            // column halves of a key tile (one softmax thread per row and half)
+  static constexpr int BC = BK / NHALF;      // columns per softmax thread and step
+  static constexpr int THREADS = 128 + NMT * NHALF * 128;
   static constexpr uint32_t TMEM_COLS = 512;
 };
 
@@ -49,19 +54,19 @@ struct FwdParams {
   float* lse2;
 };
 
-// Online update for one 64-key tile of one query row (thread-local).  Implements Alg.1 lines 8-12 with
+// Online update for NC keys of one query row (thread-local).  Implements Alg.1 lines 8-12 with
 //   x_t = s_t*sc_t - m_t (log2 domain, shifted),  acc += sum p1*(x1-x2) + (m1-m2)*sum p1   [= sum p1 (s1'-s2')].
 struct RowState {
   float m1, m2, l1, l2, acc;
 };
 
-template <bool MASKED>
-__device__ __forceinline__ void online_update64(RowState& st, const uint32_t (&r1)[64], const uint32_t (&r2)[64], float sc1,
-                                                float sc2, int kbase, int limit) {
+template <bool MASKED, int NC>
+__device__ __forceinline__ void online_update(RowState& st, const uint32_t (&r1)[NC], const uint32_t (&r2)[NC], float sc1,
+                                              float sc2, int kbase, int limit) {
   float mx1a = -CUDART_INF_F, mx1b = -CUDART_INF_F, mx2a = -CUDART_INF_F, mx2b = -CUDART_INF_F;
   if constexpr (!MASKED) {
 #pragma unroll
-    for (int e = 0; e < 64; e += 4) {
+    for (int e = 0; e < NC; e += 4) {
       mx1a = max3(mx1a, __uint_as_float(r1[e]), __uint_as_float(r1[e + 1]));
       mx1b = max3(mx1b, __uint_as_float(r1[e + 2]), __uint_as_float(r1[e + 3]));
       mx2a = max3(mx2a, __uint_as_float(r2[e]), __uint_as_float(r2[e + 1]));
@@ -69,7 +74,7 @@ __device__ __forceinline__ void online_update64(RowState& st, const uint32_t (&r
     }
   } else {
 #pragma unroll
-    for (int e = 0; e < 64; ++e) {
+    for (int e = 0; e < NC; ++e) {
       const bool ok = (kbase + e) <= limit;
       mx1a = fmaxf(mx1a, ok ? __uint_as_float(r1[e]) : -CUDART_INF_F);
       mx2a = fmaxf(mx2a, ok ? __uint_as_float(r2[e]) : -CUDART_INF_F);
@@ -82,25 +87,45 @@ __device__ __forceinline__ void online_update64(RowState& st, const uint32_t (&r
   const float ref2 = MASKED ? (m2n == -CUDART_INF_F ? 0.f : m2n) : m2n;
   const float a1 = ex2_approx(st.m1 - ref1);  // alpha_1 (Alg.1 line 9); m = -inf gives 0
   const float a2 = ex2_approx(st.m2 - ref2);
-  float s1[4] = {0.f, 0.f, 0.f, 0.f}, s2[4] = {0.f, 0.f, 0.f, 0.f}, dd[4] = {0.f, 0.f, 0.f, 0.f};
+  float sum1, sum2, dsum;
+  if constexpr (!MASKED) {
+    // packed fp32x2 lanes over column pairs (e, e+1): half the issue slots of the scalar form (the loop is
+    // issue/MUFU bound); two independent accumulator pairs per quantity
+    const float2 vsc1 = make_float2(sc1, sc1), vsc2 = make_float2(sc2, sc2);
+    const float2 vr1 = make_float2(-ref1, -ref1), vr2 = make_float2(-ref2, -ref2);
+    float2 s1v[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)}, s2v[2] = {s1v[0], s1v[0]}, ddv[2] = {s1v[0], s1v[0]};
 #pragma unroll
-  for (int e = 0; e < 64; ++e) {
-    const float x1 = fmaf(__uint_as_float(r1[e]), sc1, -ref1);
-    const float x2 = fmaf(__uint_as_float(r2[e]), sc2, -ref2);
-    float p1 = ex2_approx(x1);
-    float p2 = ex2_approx(x2);
-    if constexpr (MASKED) {  // R8: zero P~, take the difference from the raw (finite) logits
-      const bool ok = (kbase + e) <= limit;
-      p1 = ok ? p1 : 0.f;
-      p2 = ok ? p2 : 0.f;
+    for (int e = 0; e < NC; e += 2) {
+      const float2 x1 = fma2(make_float2(__uint_as_float(r1[e]), __uint_as_float(r1[e + 1])), vsc1, vr1);
+      const float2 x2 = fma2(make_float2(__uint_as_float(r2[e]), __uint_as_float(r2[e + 1])), vsc2, vr2);
+      const float2 p1 = make_float2(ex2_approx(x1.x), ex2_approx(x1.y));
+      const float2 p2 = make_float2(ex2_approx(x2.x), ex2_approx(x2.y));
+      const int a = (e >> 1) & 1;
+      s1v[a] = add2(s1v[a], p1);
+      s2v[a] = add2(s2v[a], p2);
+      ddv[a] = fma2(p1, sub2(x1, x2), ddv[a]);
     }
-    s1[e & 3] += p1;
-    s2[e & 3] += p2;
-    dd[e & 3] = fmaf(p1, x1 - x2, dd[e & 3]);
+    sum1 = (s1v[0].x + s1v[0].y) + (s1v[1].x + s1v[1].y);
+    sum2 = (s2v[0].x + s2v[0].y) + (s2v[1].x + s2v[1].y);
+    dsum = (ddv[0].x + ddv[0].y) + (ddv[1].x + ddv[1].y);
+  } else {
+    float s1[4] = {0.f, 0.f, 0.f, 0.f}, s2[4] = {0.f, 0.f, 0.f, 0.f}, dd[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+    for (int e = 0; e < NC; ++e) {
+      const float x1 = fmaf(__uint_as_float(r1[e]), sc1, -ref1);
+      const float x2 = fmaf(__uint_as_float(r2[e]), sc2, -ref2);
+      // R8: zero P~ at masked entries, take the difference from the raw (finite) logits
+      const bool ok = (kbase + e) <= limit;
+      const float p1 = ok ? ex2_approx(x1) : 0.f;
+      const float p2 = ok ? ex2_approx(x2) : 0.f;
+      s1[e & 3] += p1;
+      s2[e & 3] += p2;
+      dd[e & 3] = fmaf(p1, x1 - x2, dd[e & 3]);
+    }
+    sum1 = (s1[0] + s1[1]) + (s1[2] + s1[3]);
+    sum2 = (s2[0] + s2[1]) + (s2[2] + s2[3]);
+    dsum = (dd[0] + dd[1]) + (dd[2] + dd[3]);
   }
-  const float sum1 = (s1[0] + s1[1]) + (s1[2] + s1[3]);
-  const float sum2 = (s2[0] + s2[1]) + (s2[2] + s2[3]);
-  const float dsum = (dd[0] + dd[1]) + (dd[2] + dd[3]);
   st.l1 = fmaf(st.l1, a1, sum1);                               // line 11 (R9: alpha1 on l1, acc; alpha2 on l2)
   st.l2 = fmaf(st.l2, a2, sum2);
   st.acc = fmaf(st.acc, a1, fmaf(ref1 - ref2, sum1, dsum));    // line 12
@@ -109,7 +134,7 @@ __device__ __forceinline__ void online_update64(RowState& st, const uint32_t (&r
 }
 
 template <int D1, int D2, bool CAUSAL>
-__global__ void __launch_bounds__(384, 1)
+__global__ void __launch_bounds__(FwdCfg<D1, D2>::THREADS, 1)
 streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid_constant__ CUtensorMap tmK1,
                           const __grid_constant__ CUtensorMap tmQ2, const __grid_constant__ CUtensorMap tmK2, const FwdParams p) {
   using C = FwdCfg<D1, D2>;
@@ -153,7 +178,7 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
   if (warp == 1 && lane == 0) {
     mbar_init(q_full, 1);
     for (int s = 0; s < C::NSTAGE; ++s) { mbar_init(&k_full[s], 1); mbar_init(&k_empty[s], 1); }
-    for (int i = 0; i < 4; ++i) { mbar_init(&s_full[i], 1); mbar_init(&s_empty[i], 4); }
+    for (int i = 0; i < 4; ++i) { mbar_init(&s_full[i], 1); mbar_init(&s_empty[i], 4 * C::NHALF); }
     fence_mbar_init();
   }
   if (warp == 2) tmem_alloc<C::TMEM_COLS>(tmem_ptr);
@@ -162,7 +187,9 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
   tc_fence_after();
   const uint32_t tmem_base = *tmem_ptr;
 
-  if (warp == 0) {
+  if (warp < 4) {
+   reg_dealloc<24>();   // (pool: (96-24)*128 = 9216 >= (112-96)*512) producer / MMA / allocator warpgroup gives its registers to the two softmax warpgroups
+   if (warp == 0) {
     // ===================== TMA producer =====================
     if (lane == 0) {
       const uint64_t pol_q = l2_policy_evict_first(), pol_k = l2_policy_evict_last();
@@ -191,50 +218,60 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
-    if (lane == 0) {
-      constexpr uint32_t idesc = umma_idesc_bf16(C::BM, C::BK, 0, 0);
-      mbar_wait(q_full, 0);
+    // The whole warp runs the loop (warp-uniform control flow and descriptors stay in uniform registers); only the
+    // tcgen05.mma / tcgen05.commit instructions themselves are issued by one elected lane.
+    constexpr uint32_t idesc = umma_idesc_bf16(C::BM, C::BK, 0, 0);
+    const uint64_t dq1 = umma_smem_desc_sw128(smem_u32(sQ1), 16, 1024);
+    const uint64_t dq2 = umma_smem_desc_sw128(smem_u32(sQ2), 16, 1024);
+    const uint64_t dk = umma_smem_desc_sw128(smem_u32(sK), 16, 1024);
+    mbar_wait(q_full, 0);
+    tc_fence_after();
+    for (int j = 0; j < nsteps; ++j) {
+      const int s = j % C::NSTAGE;
+      const uint32_t ph = (j / C::NSTAGE) & 1;
+      mbar_wait(&k_full[s], ph);
       tc_fence_after();
-      for (int j = 0; j < nsteps; ++j) {
-        const int s = j % C::NSTAGE;
-        const uint32_t ph = (j / C::NSTAGE) & 1;
-        mbar_wait(&k_full[s], ph);
-        tc_fence_after();
-        const uint32_t kaddr = smem_u32(sK + s * C::STAGE_BYTES);
-        const int st = j & 1;
-        const uint32_t sph = (j >> 1) & 1;
+      const uint64_t dks = dk + uint64_t((s * C::STAGE_BYTES) >> 4);
+      const int st = j & 1;
+      const uint32_t sph = (j >> 1) & 1;
 #pragma unroll
-        for (int mt = 0; mt < C::NMT; ++mt) {
-          if (j < nsteps_mt[mt]) {
-            mbar_wait(&s_empty[mt * 2 + st], sph ^ 1);
-            tc_fence_after();
-            const uint32_t dS1 = tmem_base + (mt * 2 + st) * 128;
-            const uint32_t dS2 = dS1 + 64;
-            const uint32_t q1addr = smem_u32(sQ1 + mt * C::KB1 * C::QBLK);
-            const uint32_t q2addr = smem_u32(sQ2 + mt * C::KB2 * C::QBLK);
+      for (int mt = 0; mt < C::NMT; ++mt) {
+        if (j < nsteps_mt[mt]) {
+          mbar_wait(&s_empty[mt * 2 + st], sph ^ 1);
+          tc_fence_after();
+          const uint32_t dS1 = tmem_base + (mt * 2 + st) * 128;
+          const uint32_t dS2 = dS1 + 64;
+          if (elect_one()) {
 #pragma unroll
             for (int kb = 0; kb < C::KB1; ++kb)
 #pragma unroll
               for (int k = 0; k < 4; ++k)
-                umma_bf16_ss(dS1, umma_smem_desc_sw128(q1addr + kb * C::QBLK + k * 32, 16, 1024),
-                             umma_smem_desc_sw128(kaddr + kb * C::KBLK + k * 32, 16, 1024), idesc, (kb | k) != 0);
+                umma_bf16_ss(dS1, dq1 + uint64_t(((mt * C::KB1 + kb) * C::QBLK + k * 32) >> 4),
+                             dks + uint64_t((kb * C::KBLK + k * 32) >> 4), idesc, (kb | k) != 0);
 #pragma unroll
             for (int kb = 0; kb < C::KB2; ++kb)
 #pragma unroll
               for (int k = 0; k < 4; ++k)
-                umma_bf16_ss(dS2, umma_smem_desc_sw128(q2addr + kb * C::QBLK + k * 32, 16, 1024),
-                             umma_smem_desc_sw128(kaddr + (C::KB1 + kb) * C::KBLK + k * 32, 16, 1024), idesc, (kb | k) != 0);
+                umma_bf16_ss(dS2, dq2 + uint64_t(((mt * C::KB2 + kb) * C::QBLK + k * 32) >> 4),
+                             dks + uint64_t(((C::KB1 + kb) * C::KBLK + k * 32) >> 4), idesc, (kb | k) != 0);
             umma_commit(&s_full[mt * 2 + st]);
           }
+          __syncwarp();
         }
-        umma_commit(&k_empty[s]);  // K stage reusable once every MMA that read it has retired
       }
+      if (elect_one()) umma_commit(&k_empty[s]);  // K stage reusable once every MMA that read it has retired
+      __syncwarp();
     }
-  } else if (warp >= 4) {
-    // ===================== softmax warpgroups =====================
-    const int mt = (warp - 4) >> 2;
-    const int quarter = warp & 3;  // TMEM lane quarter this warp may access
-    const int row = q0 + mt * C::BM + quarter * 32 + lane;
+   }
+  } else {
+    // ===================== softmax warps =====================
+    reg_alloc<112>();    // needs 16*512 = 8192 registers from the pool the other warpgroup released
+    const int sw = warp - 4;
+    const int quarter = warp & 3;          // TMEM lane quarter this warp may access
+    const int mt = (sw >> 2) & 1;
+    const int half = sw >> 3;              // which 32-column half of every key tile
+    const int rloc = quarter * 32 + lane;
+    const int row = q0 + mt * C::BM + rloc;
     const int limit = CAUSAL ? min(p.NK - 1, row + off) : p.NK - 1;  // last visible key of this row
     const int first_row_limit = (q0 + mt * C::BM) + off;             // causal frontier of the tile's first row
     RowState st{-CUDART_INF_F, -CUDART_INF_F, 0.f, 0.f, 0.f};
@@ -244,30 +281,43 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
       const uint32_t sph = (j >> 1) & 1;
       mbar_wait(&s_full[mt * 2 + sg], sph);
       tc_fence_after();
-      const uint32_t taddr = tmem_base + (uint32_t(quarter * 32) << 16) + (mt * 2 + sg) * 128;
-      uint32_t r1[64], r2[64];
-      tmem_ld32(taddr, *reinterpret_cast<uint32_t(*)[32]>(&r1[0]));
-      tmem_ld32(taddr + 32, *reinterpret_cast<uint32_t(*)[32]>(&r1[32]));
-      tmem_ld32(taddr + 64, *reinterpret_cast<uint32_t(*)[32]>(&r2[0]));
-      tmem_ld32(taddr + 96, *reinterpret_cast<uint32_t(*)[32]>(&r2[32]));
+      const uint32_t taddr = tmem_base + (uint32_t(quarter * 32) << 16) + (mt * 2 + sg) * 128 + half * C::BC;
+      uint32_t r1[C::BC], r2[C::BC];
+      tmem_ld32(taddr, r1);
+      tmem_ld32(taddr + C::BK, r2);
       tmem_wait_ld();
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(&s_empty[mt * 2 + sg]);  // logits are in registers: MMA may refill this stage
-      const int kbase = j * C::BK;
-      const bool masked = (CAUSAL && (kbase + C::BK - 1 > first_row_limit)) || (kbase + C::BK > p.NK);
-      if (masked) online_update64<true>(st, r1, r2, p.sc1, p.sc2, kbase, limit);
-      else        online_update64<false>(st, r1, r2, p.sc1, p.sc2, kbase, limit);
+      const int kbase = j * C::BK + half * C::BC;
+      const bool masked = (CAUSAL && (kbase + C::BC - 1 > first_row_limit)) || (kbase + C::BC > p.NK);
+      if (masked) online_update<true, C::BC>(st, r1, r2, p.sc1, p.sc2, kbase, limit);
+      else        online_update<false, C::BC>(st, r1, r2, p.sc1, p.sc2, kbase, limit);
     }
-    if (row < p.NQ) {
-      // Alg.1 lines 13-15 in natural-log units (R6): LSE = ln2*(m + log2 l); KL = ln2*acc/l1 + LSE2 - LSE1
-      const float LN2 = 0.6931471805599453f;
-      const float e1 = LN2 * (st.m1 + log2f(st.l1));
-      const float e2 = LN2 * (st.m2 + log2f(st.l2));
-      const size_t o = size_t(bh) * p.NQ + row;
-      p.lse1[o] = e1;
-      p.lse2[o] = e2;
-      p.kl[o] = fmaf(LN2, st.acc / st.l1, e2 - e1);
+    if (n > 0) {
+      // merge the two column halves of each row (Eq.11 with (m2,l2) carried too, R11).  The exchange buffer aliases this
+      // M-tile's own Q1 block: every MMA that reads it has completed (the last s_full of this M-tile has been observed).
+      float* xch = reinterpret_cast<float*>(sQ1 + mt * C::KB1 * C::QBLK);
+      if (half == 1) {
+        xch[0 * C::BM + rloc] = st.m1; xch[1 * C::BM + rloc] = st.l1; xch[2 * C::BM + rloc] = st.m2;
+        xch[3 * C::BM + rloc] = st.l2; xch[4 * C::BM + rloc] = st.acc;
+      }
+      asm volatile("bar.sync %0, 256;" ::"r"(1 + mt) : "memory");
+      if (half == 0 && row < p.NQ) {
+        const float m1b = xch[0 * C::BM + rloc], l1b = xch[1 * C::BM + rloc], m2b = xch[2 * C::BM + rloc];
+        const float l2b = xch[3 * C::BM + rloc], accb = xch[4 * C::BM + rloc];
+        const float m1 = fmaxf(st.m1, m1b), m2 = fmaxf(st.m2, m2b);   // half 0 holds key 0: its maxima are finite
+        const float wa1 = exp2f(st.m1 - m1), wb1 = exp2f(m1b - m1), wa2 = exp2f(st.m2 - m2), wb2 = exp2f(m2b - m2);
+        const float l1 = st.l1 * wa1 + l1b * wb1, l2 = st.l2 * wa2 + l2b * wb2, acc = st.acc * wa1 + accb * wb1;
+        // Alg.1 lines 13-15 in natural-log units (R6): LSE = ln2*(m + log2 l); KL = ln2*acc/l1 + LSE2 - LSE1
+        const float LN2 = 0.6931471805599453f;
+        const float e1 = LN2 * (m1 + log2f(l1));
+        const float e2 = LN2 * (m2 + log2f(l2));
+        const size_t o = size_t(bh) * p.NQ + row;
+        p.lse1[o] = e1;
+        p.lse2[o] = e2;
+        p.kl[o] = fmaf(LN2, acc / l1, e2 - e1);
+      }
     }
   }
   tc_fence_before();
