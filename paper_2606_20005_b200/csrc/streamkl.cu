@@ -19,10 +19,11 @@ namespace {
 thread_local int g_last_launches = 0;
 
 // ---- optional per-kernel timing (streamkl_profile_*): CUDA events recorded on the launch stream around every kernel
-enum KernelId { KID_FWD_TC = 0, KID_BWD_DQ_TC, KID_BWD_DK_TC, KID_FWD_SIMT, KID_BWD_DQ_SIMT, KID_BWD_DK_SIMT, KID_COUNT };
+enum KernelId { KID_FWD_TC = 0, KID_BWD_DQ_TC, KID_BWD_DK_TC, KID_FWD_SIMT, KID_BWD_DQ_SIMT, KID_BWD_DK_SIMT, KID_BWD_STATS, KID_COUNT };
 const char* const kKernelNames[KID_COUNT] = {"streamkl_fwd_sm100_kernel", "streamkl_bwd_sm100_kernel<OWNER_Q>",
                                              "streamkl_bwd_sm100_kernel<OWNER_K>", "streamkl_fwd_simt_kernel",
-                                             "streamkl_bwd_simt_kernel<OWNER_Q>", "streamkl_bwd_simt_kernel<OWNER_K>"};
+                                             "streamkl_bwd_simt_kernel<OWNER_Q>", "streamkl_bwd_simt_kernel<OWNER_K>",
+                                             "streamkl_bwd_stats_kernel"};
 struct ProfRecord { int id; cudaEvent_t a, b; };
 thread_local bool g_prof_on = false;
 thread_local std::vector<ProfRecord>* g_prof = nullptr;
@@ -213,8 +214,8 @@ int launch_bwd_simt(const void* Q1, const void* K1, const void* Q2, const void* 
 }
 
 template <int D1, int D2, bool CAUSAL, bool TEACHER, bool OWNER_K>
-int launch_bwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, const float* kl, const float* lse1,
-                  const float* lse2, const float* dkl, void* dX1, void* dX2, cudaStream_t stream) {
+int launch_bwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, const float4* stats, void* dX1,
+                  void* dX2, cudaStream_t stream) {
   using C = skl::BwdCfg<D1, D2, TEACHER>;
   CUtensorMap tQ1, tK1, tQ2, tK2;
   // the owner side is loaded in 128-row boxes, the streamed side in BY-row boxes
@@ -231,7 +232,7 @@ int launch_bwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2
   p.NQ = s.NQ; p.NK = s.NK; p.BH = int(s.BH);
   p.TX = ((OWNER_K ? s.NK : s.NQ) + C::BX - 1) / C::BX;
   p.c1 = s.c1; p.c2 = s.c2;
-  p.kl = kl; p.lse1 = lse1; p.lse2 = lse2; p.dkl = dkl;
+  p.stats = stats;
   p.dX1 = static_cast<__nv_bfloat16*>(dX1);
   p.dX2 = static_cast<__nv_bfloat16*>(dX2);
   const long long grid = (long long)p.TX * s.BH;
@@ -247,13 +248,26 @@ int launch_bwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2
 
 template <int D1, int D2>
 int bwd_tc_both(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, const float* kl, const float* lse1,
-                const float* lse2, const float* dkl, void* dQ1, void* dK1, void* dQ2, void* dK2, cudaStream_t st) {
+                const float* lse2, const float* dkl, void* dQ1, void* dK1, void* dQ2, void* dK2, void* workspace, cudaStream_t st) {
   const bool t = dQ1 != nullptr;
   int rc;
+  // B1: per-query scalars, packed for the dS warps, into the caller's workspace
+  float4* stats = static_cast<float4*>(workspace);
+  {
+    const long long pph = skl::bwd_stats_padded_rows(s.NQ) / 2, total = pph * s.BH;
+    const long long blocks = (total + 255) / 256;
+    if (blocks > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
+    {
+      ProfScope ps(KID_BWD_STATS, st);
+      skl::streamkl_bwd_stats_kernel<<<dim3((unsigned)blocks), 256, 0, st>>>(kl, lse1, lse2, dkl, stats, s.NQ, pph, total);
+    }
+    if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
+    g_last_launches += 1;
+  }
 #define SKL_BWD(CA, TE)                                                                                                   \
-  rc = launch_bwd_tc<D1, D2, CA, TE, false>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dQ2, st);                        \
+  rc = launch_bwd_tc<D1, D2, CA, TE, false>(Q1, K1, Q2, K2, s, stats, dQ1, dQ2, st);                                      \
   if (rc != STREAMKL_OK) return rc;                                                                                       \
-  return launch_bwd_tc<D1, D2, CA, TE, true>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dK1, dK2, st);
+  return launch_bwd_tc<D1, D2, CA, TE, true>(Q1, K1, Q2, K2, s, stats, dK1, dK2, st);
   if (s.causal) { if (t) { SKL_BWD(true, true) } else { SKL_BWD(true, false) } }
   else          { if (t) { SKL_BWD(false, true) } else { SKL_BWD(false, false) } }
 #undef SKL_BWD
@@ -262,7 +276,6 @@ int bwd_tc_both(const void* Q1, const void* K1, const void* Q2, const void* K2, 
 int bwd_dispatch(int dtype, const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1,
                  int d2, float c1, float c2, int causal, const float* kl, const float* lse1, const float* lse2, const float* dkl,
                  void* dQ1, void* dK1, void* dQ2, void* dK2, void* workspace, size_t workspace_bytes, cudaStream_t stream) {
-  (void)workspace;
   Shape s{B, H, NQ, NK, d1, d2, causal ? 1 : 0, c1, c2, (long long)B * (long long)H};
   int rc = validate_common(Q1, K1, Q2, K2, s);
   if (rc != STREAMKL_OK) return rc;
@@ -276,6 +289,7 @@ int bwd_dispatch(int dtype, const void* Q1, const void* K1, const void* Q2, cons
     return STREAMKL_ERR_ALIGN;
   const size_t need = streamkl_bwd_workspace_bytes(B, H, NQ, NK, d1, d2, dQ1 != nullptr);
   if (need > 0 && (!workspace || workspace_bytes < need)) return STREAMKL_ERR_WORKSPACE;
+  if (reinterpret_cast<uintptr_t>(workspace) & 15) return STREAMKL_ERR_ALIGN;
   if (!device_is_sm100()) return STREAMKL_ERR_CUDA;
   if (s.BH > 65535) return STREAMKL_ERR_SHAPE;
   const size_t es = dtype == STREAMKL_BF16 ? 2 : 4;
@@ -285,10 +299,10 @@ int bwd_dispatch(int dtype, const void* Q1, const void* K1, const void* Q2, cons
     return STREAMKL_OK;
   }
   if (tc_shape(dtype, s)) {
-    if (d1 == 128 && d2 == 128) return bwd_tc_both<128, 128>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, stream);
-    if (d1 == 128 && d2 == 64) return bwd_tc_both<128, 64>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, stream);
-    if (d1 == 64 && d2 == 128) return bwd_tc_both<64, 128>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, stream);
-    if (d1 == 64 && d2 == 64) return bwd_tc_both<64, 64>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, stream);
+    if (d1 == 128 && d2 == 128) return bwd_tc_both<128, 128>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, workspace, stream);
+    if (d1 == 128 && d2 == 64) return bwd_tc_both<128, 64>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, workspace, stream);
+    if (d1 == 64 && d2 == 128) return bwd_tc_both<64, 128>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, workspace, stream);
+    if (d1 == 64 && d2 == 64) return bwd_tc_both<64, 64>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, workspace, stream);
   }
   if (dtype == STREAMKL_BF16) {
     rc = launch_bwd_simt<__nv_bfloat16, false>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dQ2, stream);
@@ -338,8 +352,12 @@ int streamkl_bwd_f32(const void* Q1, const void* K1, const void* Q2, const void*
                       dQ2, dK2, workspace, workspace_bytes, static_cast<cudaStream_t>(stream));
 }
 
-size_t streamkl_bwd_workspace_bytes(int, int, int, int, int, int, int) {
-  return 0;  // both gradients are produced by tile ownership: no fp32 accumulation workspace
+size_t streamkl_bwd_workspace_bytes(int B, int H, int NQ, int, int d1, int d2, int) {
+  // both gradients are produced by tile ownership: no fp32 accumulation workspace.  The tcgen05 kernels read the
+  // per-query scalars (lse1, lse2, dkl, kl) from a packed copy: 16 B per query, rows padded to 64 per head -- O(NQ).
+  if (B <= 0 || H <= 0 || NQ <= 0) return 0;
+  if (!((d1 == 64 || d1 == 128) && (d2 == 64 || d2 == 128))) return 0;
+  return size_t(B) * size_t(H) * size_t(skl::bwd_stats_padded_rows(NQ)) * 16;
 }
 
 int streamkl_fwd_host(int dtype, const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1,
@@ -372,10 +390,11 @@ int streamkl_fwd_bwd_host(int dtype, const void* Q1, const void* K1, const void*
   const size_t nq1 = size_t(s.BH) * NQ * d1 * es, nk1 = size_t(s.BH) * NK * d1 * es;
   const size_t nq2 = size_t(s.BH) * NQ * d2 * es, nk2 = size_t(s.BH) * NK * d2 * es;
   const size_t nrow = size_t(s.BH) * NQ * sizeof(float);
-  DevBuf bQ1, bK1, bQ2, bK2, bkl, bl1, bl2, bg, gQ1, gK1, gQ2, gK2;
+  DevBuf bQ1, bK1, bQ2, bK2, bkl, bl1, bl2, bg, gQ1, gK1, gQ2, gK2, bws;
+  const size_t ws_bytes = want_bwd ? streamkl_bwd_workspace_bytes(B, H, NQ, NK, d1, d2, dQ1 != nullptr) : 0;
   if (!bQ1.alloc(nq1) || !bK1.alloc(nk1) || !bQ2.alloc(nq2) || !bK2.alloc(nk2) || !bkl.alloc(nrow) || !bl1.alloc(nrow) ||
       !bl2.alloc(nrow)) { cudaGetLastError(); return STREAMKL_ERR_CUDA; }
-  if (want_bwd && (!bg.alloc(nrow) || !gQ2.alloc(nq2) || !gK2.alloc(nk2) || (dQ1 && (!gQ1.alloc(nq1) || !gK1.alloc(nk1))))) {
+  if (want_bwd && (!bws.alloc(ws_bytes) || !bg.alloc(nrow) || !gQ2.alloc(nq2) || !gK2.alloc(nk2) || (dQ1 && (!gQ1.alloc(nq1) || !gK1.alloc(nk1))))) {
     cudaGetLastError();
     return STREAMKL_ERR_CUDA;
   }
@@ -393,7 +412,7 @@ int streamkl_fwd_bwd_host(int dtype, const void* Q1, const void* K1, const void*
   if (want_bwd) {
     rc = bwd_dispatch(dtype, bQ1.p, bK1.p, bQ2.p, bK2.p, B, H, NQ, NK, d1, d2, c1, c2, causal, static_cast<float*>(bkl.p),
                       static_cast<float*>(bl1.p), static_cast<float*>(bl2.p), static_cast<float*>(bg.p), gQ1.p, gK1.p, gQ2.p, gK2.p,
-                      nullptr, 0, stream);
+                      bws.p, ws_bytes, stream);
     if (rc != STREAMKL_OK) { cudaStreamSynchronize(stream); return rc; }
     launches += g_last_launches;
   }

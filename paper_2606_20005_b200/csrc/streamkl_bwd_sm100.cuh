@@ -5,14 +5,23 @@
 //   OWNER_K = false : CTA owns a 128-row Q tile, streams 64-key tiles      -> dQ1, dQ2   (Alg.2 :224-234, Alg.3 :255-286)
 //   OWNER_K = true  : CTA owns a 128-row K tile, streams 64-query tiles    -> dK1, dK2   (transposed tiling, :294, :309)
 // With X the owner side and Y the streamed side, per step:
-//   S1' = X1 Y1^T, S2' = X2 Y2^T        tcgen05.mma -> TMEM (lane = owner row)                                   (B2)
+//   S1' = X1 Y1^T, S2' = X2 Y2^T        tcgen05.mma (SS) -> TMEM, lane = owner row                                (B2)
 //   P_t = exp2(S_t' sc_t - lse_t log2e)  recomputed from the saved LSE (:216)                                     (B3)
 //   dS2 = g (P2 - P1)   [fp32 subtract, one bf16 rounding]      dS1 = g P1 ((s1 - s2) - (lse1 - lse2) - kl)  Eq.12 (B4)
-//   dX2 += dS2 Y2,  dX1 += dS1 Y1       tcgen05.mma, A = dS from swizzled smem, B = the Y tile read MN-major,
-//                                        accumulators stay in TMEM for the whole CTA                               (B5)
+//   dX2 += dS2 Y2,  dX1 += dS1 Y1       tcgen05.mma with A = dS read FROM TMEM (the softmax warps write bf16 dS over
+//                                        the logits they have just consumed, tcgen05.st), B = the Y tile in shared
+//                                        memory read MN-major; accumulators stay in TMEM for the whole CTA         (B5)
 // Epilogue: dX * c_t -> bf16 -> HBM, one rounding (B6).
-// Warp roles: warp 0 TMA producer (+ per-query scalars when OWNER_K), warp 1 MMA issuer, warp 2 TMEM allocator,
-// warps 4-7 / 8-11 two softmax warpgroups that take alternate steps (each has its own S' stage and dS buffer).
+//
+// Everything is kept in the log2 domain: x_t = s_t' sc_t - lse_t log2e (sc_t = c_t log2e) so P_t = exp2(x_t) and
+// (s1 - s2) - (lse1 - lse2) - kl = ln2 (x1 - x2 - kl log2e); the ln2 (and, for the Q owner, the per-row g) is folded
+// into the epilogue scale.  Per-query scalars come from a small pre-pass (streamkl_bwd_stats_kernel) that writes, for
+// every PAIR of queries, {-lse1 log2e (x2), -lse2 log2e (x2)}, {g (x2), kl log2e (x2)} -- the packed-fp32x2 operand
+// layout -- padded to a multiple of 64 queries per head with values that make padded queries contribute exactly 0.
+//
+// Warp roles (640 threads): warp 0 TMA producer (X once, Y ring + the streamed queries' scalars when OWNER_K),
+// warp 1 MMA issuer, warp 2 TMEM allocator, warps 4-19 sixteen dS warps = 2 S' stages x 2 column halves x 4 TMEM
+// lane quarters.  TMEM (512 columns): two S' stages of {S1' 64, S2' 64} (dS aliases them) + D1 + D2 accumulator columns.
 #pragma once
 #include <cuda_bf16.h>
 #include <math_constants.h>
@@ -29,31 +38,52 @@ struct BwdCfg {
   static constexpr int KB1 = D1 / 64, KB2 = D2 / 64;
   static constexpr int XBLK = BX * 128, YBLK = BY * 128;
   static constexpr int X_BYTES = (KB1 + KB2) * XBLK;
-  static constexpr int DS_TILE = BX * BY * 2;                        // one [128 x 64] bf16 dS tile
-  static constexpr int DS_PER_WG = (TEACHER ? 2 : 1) * DS_TILE;
-  static constexpr int DS_BYTES = 2 * DS_PER_WG;
   static constexpr int Y_STAGE = (KB1 + KB2) * YBLK;
-  static constexpr int STAT_STAGE = BY * 16;                         // float4 per streamed query (OWNER_K)
+  static constexpr int STAT_STAGE = BY * 16;                         // two float4 per PAIR of streamed queries (OWNER_K)
   static constexpr int AUX_BYTES = 512;
-  static constexpr int NSTAGE_RAW = (227 * 1024 - 1024 - AUX_BYTES - X_BYTES - DS_BYTES) / (Y_STAGE + STAT_STAGE);
+  static constexpr int NSTAGE_RAW = (227 * 1024 - 1024 - AUX_BYTES - X_BYTES) / (Y_STAGE + STAT_STAGE);
   static constexpr int NSTAGE = NSTAGE_RAW > 6 ? 6 : NSTAGE_RAW;
   static_assert(NSTAGE >= 2, "need at least a double-buffered Y ring");
-  static constexpr int SMEM_BYTES = 1024 + X_BYTES + DS_BYTES + NSTAGE * (Y_STAGE + STAT_STAGE) + AUX_BYTES;
-  static constexpr int THREADS = 384;
+  static constexpr int SMEM_BYTES = 1024 + X_BYTES + NSTAGE * (Y_STAGE + STAT_STAGE) + AUX_BYTES;
+  static constexpr int THREADS = 128 + 512;
   static constexpr uint32_t TMEM_COLS = 512;
   static constexpr uint32_t COL_DX1 = 256, COL_DX2 = 256 + (TEACHER ? D1 : 0);   // after the two S' stages (2 x 128)
 };
 
+// queries per head in the padded per-query scalar array
+__host__ __device__ constexpr long long bwd_stats_padded_rows(long long NQ) { return (NQ + 63) / 64 * 64; }
+
 struct BwdParams {
   int NQ, NK, TX, BH;
   float c1, c2;
-  const float* kl;
-  const float* lse1;
-  const float* lse2;
-  const float* dkl;
+  const float4* stats;  // [BH][NQP/2][2] float4, NQP = bwd_stats_padded_rows(NQ)
   __nv_bfloat16* dX1;   // dQ1 or dK1 (nullptr when !TEACHER)
   __nv_bfloat16* dX2;   // dQ2 or dK2
 };
+
+// B1: per-query scalars in the layout the dS warps consume (see the header comment)
+__global__ void streamkl_bwd_stats_kernel(const float* __restrict__ kl, const float* __restrict__ lse1, const float* __restrict__ lse2,
+                                          const float* __restrict__ dkl, float4* __restrict__ stats, int NQ, long long pairs_per_head,
+                                          long long total_pairs) {
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= total_pairs) return;
+  const long long bh = idx / pairs_per_head;
+  const int q = int(idx % pairs_per_head);
+  const float L2E = 1.4426950408889634f;
+  float v[2][4];
+#pragma unroll
+  for (int u = 0; u < 2; ++u) {
+    const int i = 2 * q + u;
+    if (i < NQ) {
+      const size_t o = size_t(bh) * NQ + i;
+      v[u][0] = -lse1[o] * L2E; v[u][1] = -lse2[o] * L2E; v[u][2] = dkl[o]; v[u][3] = kl[o] * L2E;
+    } else {  // padded query: P = exp2(x - 1e30) = 0 and g = 0
+      v[u][0] = -1e30f; v[u][1] = -1e30f; v[u][2] = 0.f; v[u][3] = 0.f;
+    }
+  }
+  stats[idx * 2 + 0] = make_float4(v[0][0], v[1][0], v[0][1], v[1][1]);
+  stats[idx * 2 + 1] = make_float4(v[0][2], v[1][2], v[0][3], v[1][3]);
+}
 
 __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   uint32_t r;
@@ -61,30 +91,68 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   return r;
 }
 
-// dX accumulator (this warp's 32 lanes x NCOLS fp32 columns) -> * scale -> bf16 -> global row
-template <int NCOLS>
-__device__ __forceinline__ void store_dx_row(uint32_t taddr, float scale, __nv_bfloat16* out_row, bool valid) {
+// dX accumulator (this warp's 32 lanes x NC fp32 columns) -> * scale -> bf16 -> global row
+template <int NC>
+__device__ __forceinline__ void store_dx_cols(uint32_t taddr, float scale, __nv_bfloat16* out, bool valid) {
+  static_assert(NC == 16 || NC == 32, "column slice per dS warp group");
+  uint32_t v[NC];
+  if constexpr (NC == 32) tmem_ld32(taddr, v); else tmem_ld16(taddr, v);
+  tmem_wait_ld();
+  if (valid) {
 #pragma unroll
-  for (int c0 = 0; c0 < NCOLS; c0 += 32) {
-    uint32_t v[32];
-    tmem_ld32(taddr + c0, v);
-    tmem_wait_ld();
-    if (valid) {
-#pragma unroll
-      for (int q = 0; q < 4; ++q) {
-        uint4 o;
-        o.x = pack_bf16x2(__uint_as_float(v[q * 8 + 0]) * scale, __uint_as_float(v[q * 8 + 1]) * scale);
-        o.y = pack_bf16x2(__uint_as_float(v[q * 8 + 2]) * scale, __uint_as_float(v[q * 8 + 3]) * scale);
-        o.z = pack_bf16x2(__uint_as_float(v[q * 8 + 4]) * scale, __uint_as_float(v[q * 8 + 5]) * scale);
-        o.w = pack_bf16x2(__uint_as_float(v[q * 8 + 6]) * scale, __uint_as_float(v[q * 8 + 7]) * scale);
-        *reinterpret_cast<uint4*>(out_row + c0 + q * 8) = o;
-      }
+    for (int q = 0; q < NC / 8; ++q) {
+      uint4 o;
+      o.x = pack_bf16x2(__uint_as_float(v[q * 8 + 0]) * scale, __uint_as_float(v[q * 8 + 1]) * scale);
+      o.y = pack_bf16x2(__uint_as_float(v[q * 8 + 2]) * scale, __uint_as_float(v[q * 8 + 3]) * scale);
+      o.z = pack_bf16x2(__uint_as_float(v[q * 8 + 4]) * scale, __uint_as_float(v[q * 8 + 5]) * scale);
+      o.w = pack_bf16x2(__uint_as_float(v[q * 8 + 6]) * scale, __uint_as_float(v[q * 8 + 7]) * scale);
+      *reinterpret_cast<uint4*>(out + q * 8) = o;
     }
   }
 }
 
+// B3 + B4 for one owner row and 32 streamed columns: logits r1,r2 (fp32 bits) -> packed bf16 dS1 (o1), dS2 (o2).
+//   OWNER_Q: the row's scalars (nL1,nL2,klog) are thread constants and g is applied in the epilogue.
+//   OWNER_K: per-column scalars come from shared memory (`stat`, this half's 16 column pairs), g is applied here.
+// MASKED: causal diagonal tiles and streamed-key tails; P (possibly inf for a zero-filled logit) is discarded by SELECT.
+template <bool TEACHER, bool OWNER_K, bool CAUSAL, bool MASKED>
+__device__ __forceinline__ void ds_row32(const uint32_t (&r1)[32], const uint32_t (&r2)[32], uint32_t (&o1)[16], uint32_t (&o2)[16],
+                                         float sc1, float sc2, float nL1, float nL2, float klog, const float4* stat, int xrow,
+                                         int y0, int off, int NK) {
+  const float2 vsc1 = make_float2(sc1, sc1), vsc2 = make_float2(sc2, sc2);
+  float2 vn1 = make_float2(nL1, nL1), vn2 = make_float2(nL2, nL2), vk = make_float2(klog, klog), vg = make_float2(1.f, 1.f);
+#pragma unroll
+  for (int e = 0; e < 32; e += 2) {
+    if constexpr (OWNER_K) {
+      const float4 a = stat[e], b = stat[e + 1];   // pair e/2: two float4
+      vn1 = make_float2(a.x, a.y); vn2 = make_float2(a.z, a.w); vg = make_float2(b.x, b.y); vk = make_float2(b.z, b.w);
+    }
+    const float2 x1 = fma2(make_float2(__uint_as_float(r1[e]), __uint_as_float(r1[e + 1])), vsc1, vn1);
+    const float2 x2 = fma2(make_float2(__uint_as_float(r2[e]), __uint_as_float(r2[e + 1])), vsc2, vn2);
+    const float2 p1 = make_float2(ex2_approx(x1.x), ex2_approx(x1.y));   // P1 = exp(s1 - lse1)   (Alg.2 line 7)
+    const float2 p2 = make_float2(ex2_approx(x2.x), ex2_approx(x2.y));
+    float2 a2 = sub2(p2, p1);                                            // dS2 / g (Alg.2 line 8): fp32 subtract, rounded once below
+    if constexpr (OWNER_K) a2 = mul2(a2, vg);
+    float2 a1 = make_float2(0.f, 0.f);
+    if constexpr (TEACHER) {                                             // dS1 / (g ln2) = P1 (x1 - x2 - kl log2e)   (Alg.3 lines 9-10, Eq.12)
+      const float2 d = sub2(sub2(x1, x2), vk);
+      a1 = mul2(OWNER_K ? mul2(p1, vg) : p1, d);
+    }
+    if constexpr (MASKED) {
+      const int y = y0 + e;
+      bool ok0, ok1;
+      if constexpr (OWNER_K) { ok0 = !CAUSAL || xrow <= y + off; ok1 = !CAUSAL || xrow <= y + 1 + off; }
+      else { ok0 = (y < NK) && (!CAUSAL || y <= xrow + off); ok1 = (y + 1 < NK) && (!CAUSAL || y + 1 <= xrow + off); }
+      a2.x = ok0 ? a2.x : 0.f; a2.y = ok1 ? a2.y : 0.f;
+      a1.x = ok0 ? a1.x : 0.f; a1.y = ok1 ? a1.y : 0.f;
+    }
+    o2[e >> 1] = pack_bf16x2(a2.x, a2.y);
+    if constexpr (TEACHER) o1[e >> 1] = pack_bf16x2(a1.x, a1.y);
+  }
+}
+
 template <int D1, int D2, bool CAUSAL, bool TEACHER, bool OWNER_K>
-__global__ void __launch_bounds__(384, 1)
+__global__ void __launch_bounds__(BwdCfg<D1, D2, TEACHER>::THREADS, 1)
 streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid_constant__ CUtensorMap tmK1,
                           const __grid_constant__ CUtensorMap tmQ2, const __grid_constant__ CUtensorMap tmK2, const BwdParams p) {
   using C = BwdCfg<D1, D2, TEACHER>;
@@ -92,18 +160,15 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   uint8_t* sX1 = smem;
   uint8_t* sX2 = sX1 + C::KB1 * C::XBLK;
-  uint8_t* sDS = smem + C::X_BYTES;                       // [wg][{dS2, dS1}] 16 KB tiles
-  uint8_t* sY = sDS + C::DS_BYTES;                        // NSTAGE x {Y1 blocks, Y2 blocks}
-  float4* sStat = reinterpret_cast<float4*>(sY + C::NSTAGE * C::Y_STAGE);   // NSTAGE x BY float4
+  uint8_t* sY = smem + C::X_BYTES;                        // NSTAGE x {Y1 blocks, Y2 blocks}
+  float4* sStat = reinterpret_cast<float4*>(sY + C::NSTAGE * C::Y_STAGE);   // NSTAGE x 64 float4
   uint64_t* bars = reinterpret_cast<uint64_t*>(reinterpret_cast<uint8_t*>(sStat) + C::NSTAGE * C::STAT_STAGE);
   uint64_t* x_full = bars;                       // 1
   uint64_t* y_full = bars + 1;                   // NSTAGE
   uint64_t* y_empty = y_full + C::NSTAGE;        // NSTAGE
-  uint64_t* s_full = y_empty + C::NSTAGE;        // 2 (per softmax WG)
-  uint64_t* s_empty = s_full + 2;                // 2
-  uint64_t* ds_full = s_empty + 2;               // 2
-  uint64_t* ds_empty = ds_full + 2;              // 2
-  uint64_t* dx_full = ds_empty + 2;              // 1
+  uint64_t* s_full = y_empty + C::NSTAGE;        // 2 (per S' stage)
+  uint64_t* ds_full = s_full + 2;                // 2
+  uint64_t* dx_full = ds_full + 2;               // 1
   uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(dx_full + 1);
 
   const CUtensorMap* tmX1 = OWNER_K ? &tmK1 : &tmQ1;
@@ -119,6 +184,7 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
   const int off = p.NK - p.NQ;
   const int NX = OWNER_K ? p.NK : p.NQ;
   const int NY = OWNER_K ? p.NQ : p.NK;
+  const long long NQP = bwd_stats_padded_rows(p.NQ);
   int j_begin = 0, j_end = (NY + C::BY - 1) / C::BY;
   if (CAUSAL) {
     if (OWNER_K) j_begin = max(0, x0 - off) / C::BY;                       // first query that sees key x0
@@ -132,10 +198,7 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
   if (warp == 1 && lane == 0) {
     mbar_init(x_full, 1);
     for (int s = 0; s < C::NSTAGE; ++s) { mbar_init(&y_full[s], 1); mbar_init(&y_empty[s], 1); }
-    for (int w = 0; w < 2; ++w) {
-      mbar_init(&s_full[w], 1); mbar_init(&s_empty[w], 4);
-      mbar_init(&ds_full[w], 4); mbar_init(&ds_empty[w], 1);
-    }
+    for (int w = 0; w < 2; ++w) { mbar_init(&s_full[w], 1); mbar_init(&ds_full[w], 8); }
     mbar_init(dx_full, 1);
     fence_mbar_init();
   }
@@ -144,203 +207,163 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_ptr;
-  const float L2E = 1.4426950408889634f;
 
-  if (warp == 0) {
-    // ===================== producer =====================
-    uint64_t pol_x = 0, pol_y = 0;
-    if (lane == 0) {
-      pol_x = l2_policy_evict_first(); pol_y = l2_policy_evict_last();
-      mbar_arrive_expect_tx(x_full, C::X_BYTES);
-#pragma unroll
-      for (int kb = 0; kb < C::KB1; ++kb) tma_load_3d_hint(sX1 + kb * C::XBLK, tmX1, x_full, kb * 64, x0, bh, pol_x);
-#pragma unroll
-      for (int kb = 0; kb < C::KB2; ++kb) tma_load_3d_hint(sX2 + kb * C::XBLK, tmX2, x_full, kb * 64, x0, bh, pol_x);
-    }
-    for (int it = 0; it < nsteps; ++it) {
-      const int j = j_begin + it;
-      const int s = it % C::NSTAGE;
-      const uint32_t ph = (it / C::NSTAGE) & 1;
-      if (lane == 0) mbar_wait(&y_empty[s], ph ^ 1);
-      __syncwarp();
-      if (OWNER_K) {  // per-query scalars of the streamed query tile -> shared (B1)
-#pragma unroll
-        for (int t = 0; t < C::BY / 32; ++t) {
-          const int qi = j * C::BY + t * 32 + lane;
-          float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-          if (qi < p.NQ) {
-            const size_t o = size_t(bh) * p.NQ + qi;
-            const float a = p.lse1[o], b = p.lse2[o];
-            v = make_float4(a * L2E, b * L2E, p.dkl[o], (a - b) + p.kl[o]);
-          }
-          sStat[s * C::BY + t * 32 + lane] = v;
-        }
-        __syncwarp();
-      }
+  if (warp < 4) {
+    reg_dealloc<32>();   // producer / MMA / allocator warpgroup gives its registers to the sixteen dS warps: 128*(96-32) = 512*(112-96)
+    if (warp == 0) {
+      // ===================== producer =====================
       if (lane == 0) {
-        mbar_arrive_expect_tx(&y_full[s], C::Y_STAGE);
-        uint8_t* st = sY + s * C::Y_STAGE;
+        const uint64_t pol_x = l2_policy_evict_first(), pol_y = l2_policy_evict_last();
+        mbar_arrive_expect_tx(x_full, C::X_BYTES);
 #pragma unroll
-        for (int kb = 0; kb < C::KB1; ++kb) tma_load_3d_hint(st + kb * C::YBLK, tmY1, &y_full[s], kb * 64, j * C::BY, bh, pol_y);
+        for (int kb = 0; kb < C::KB1; ++kb) tma_load_3d_hint(sX1 + kb * C::XBLK, tmX1, x_full, kb * 64, x0, bh, pol_x);
 #pragma unroll
-        for (int kb = 0; kb < C::KB2; ++kb)
-          tma_load_3d_hint(st + (C::KB1 + kb) * C::YBLK, tmY2, &y_full[s], kb * 64, j * C::BY, bh, pol_y);
+        for (int kb = 0; kb < C::KB2; ++kb) tma_load_3d_hint(sX2 + kb * C::XBLK, tmX2, x_full, kb * 64, x0, bh, pol_x);
+        for (int it = 0; it < nsteps; ++it) {
+          const int j = j_begin + it;
+          const int s = it % C::NSTAGE;
+          const uint32_t ph = (it / C::NSTAGE) & 1;
+          mbar_wait(&y_empty[s], ph ^ 1);
+          mbar_arrive_expect_tx(&y_full[s], C::Y_STAGE + (OWNER_K ? C::STAT_STAGE : 0));
+          uint8_t* st = sY + s * C::Y_STAGE;
+#pragma unroll
+          for (int kb = 0; kb < C::KB1; ++kb) tma_load_3d_hint(st + kb * C::YBLK, tmY1, &y_full[s], kb * 64, j * C::BY, bh, pol_y);
+#pragma unroll
+          for (int kb = 0; kb < C::KB2; ++kb)
+            tma_load_3d_hint(st + (C::KB1 + kb) * C::YBLK, tmY2, &y_full[s], kb * 64, j * C::BY, bh, pol_y);
+          if (OWNER_K)   // the streamed queries' scalars (B1): 64 queries = 32 pairs x 32 B, contiguous and 1 KB aligned
+            bulk_load_1d(sStat + s * C::BY, p.stats + (size_t(bh) * NQP + size_t(j) * C::BY), C::STAT_STAGE, &y_full[s]);
+        }
       }
-    }
-  } else if (warp == 1) {
-    // ===================== MMA issuer =====================
-    if (lane == 0 && nsteps > 0) {
-      constexpr uint32_t idesc_s = umma_idesc_bf16(C::BX, C::BY, 0, 0);      // S' = X Y^T   : A,B K-major
-      constexpr uint32_t idesc_g1 = umma_idesc_bf16(C::BX, D1, 0, 1);        // dX1 += dS1 Y1: B MN-major
+    } else if (warp == 1) {
+      // ===================== MMA issuer =====================
+      // The whole warp runs the loop (warp-uniform control flow); only the tcgen05 instructions are issued by one lane.
+      constexpr uint32_t idesc_s = umma_idesc_bf16(C::BX, C::BY, 0, 0);      // S' = X Y^T   : A,B K-major from smem
+      constexpr uint32_t idesc_g1 = umma_idesc_bf16(C::BX, D1, 0, 1);        // dX1 += dS1 Y1: A from TMEM, B MN-major
       constexpr uint32_t idesc_g2 = umma_idesc_bf16(C::BX, D2, 0, 1);
-      const uint32_t x1addr = smem_u32(sX1), x2addr = smem_u32(sX2);
-      mbar_wait(x_full, 0);
-      tc_fence_after();
+      const uint64_t dx1 = umma_smem_desc_sw128(smem_u32(sX1), 16, 1024);
+      const uint64_t dx2 = umma_smem_desc_sw128(smem_u32(sX2), 16, 1024);
+      const uint64_t dyk = umma_smem_desc_sw128(smem_u32(sY), 16, 1024);          // Y as the K-major B operand of S'
+      const uint64_t dym = umma_smem_desc_sw128(smem_u32(sY), C::YBLK, 1024);     // Y as the MN-major B operand of dX:
+      //   64-column chunks YBLK apart (LBO), 8-row groups 1024 B apart (SBO); a K=16 slice = 16 streamed rows = 2048 B
+      if (nsteps > 0) {
+        mbar_wait(x_full, 0);
+        tc_fence_after();
+      }
       auto issue_S = [&](int it) {
         const int s = it % C::NSTAGE;
         const uint32_t ph = (it / C::NSTAGE) & 1;
-        const int w = it & 1;
-        const uint32_t wph = (it >> 1) & 1;
+        const int st = it & 1;
         mbar_wait(&y_full[s], ph);
-        mbar_wait(&s_empty[w], wph ^ 1);
         tc_fence_after();
-        const uint32_t yaddr = smem_u32(sY + s * C::Y_STAGE);
-        const uint32_t dS1 = tmem_base + w * 128, dS2 = dS1 + 64;
+        // No "stage empty" barrier: the previous user of this S' stage is step it-2, whose dS was awaited (ds_full)
+        // before its dX MMAs were issued, and tcgen05.mma executes in issue order.
+        const uint64_t dys = dyk + uint64_t((s * C::Y_STAGE) >> 4);
+        const uint32_t tS1 = tmem_base + st * 128, tS2 = tS1 + 64;
+        if (elect_one()) {
 #pragma unroll
-        for (int kb = 0; kb < C::KB1; ++kb)
+          for (int kb = 0; kb < C::KB1; ++kb)
 #pragma unroll
-          for (int k = 0; k < 4; ++k)
-            umma_bf16_ss(dS1, umma_smem_desc_sw128(x1addr + kb * C::XBLK + k * 32, 16, 1024),
-                         umma_smem_desc_sw128(yaddr + kb * C::YBLK + k * 32, 16, 1024), idesc_s, (kb | k) != 0);
+            for (int k = 0; k < 4; ++k)
+              umma_bf16_ss(tS1, dx1 + uint64_t((kb * C::XBLK + k * 32) >> 4), dys + uint64_t((kb * C::YBLK + k * 32) >> 4), idesc_s,
+                           (kb | k) != 0);
 #pragma unroll
-        for (int kb = 0; kb < C::KB2; ++kb)
+          for (int kb = 0; kb < C::KB2; ++kb)
 #pragma unroll
-          for (int k = 0; k < 4; ++k)
-            umma_bf16_ss(dS2, umma_smem_desc_sw128(x2addr + kb * C::XBLK + k * 32, 16, 1024),
-                         umma_smem_desc_sw128(yaddr + (C::KB1 + kb) * C::YBLK + k * 32, 16, 1024), idesc_s, (kb | k) != 0);
-        umma_commit(&s_full[w]);
-      };
-      auto issue_dX = [&](int it) {
-        const int s = it % C::NSTAGE;
-        const int w = it & 1;
-        const uint32_t wph = (it >> 1) & 1;
-        mbar_wait(&ds_full[w], wph);
-        tc_fence_after();
-        const uint32_t yaddr = smem_u32(sY + s * C::Y_STAGE);
-        const uint32_t dsaddr = smem_u32(sDS + w * C::DS_PER_WG);
-        const uint32_t acc = it > 0;
-        // dX2 += dS2 (128 x 64, K-major) * Y2 (64 x D2 read MN-major: 64-column chunks YBLK apart, 8-row groups 1024 B apart)
-#pragma unroll
-        for (int k = 0; k < 4; ++k)
-          umma_bf16_ss(tmem_base + C::COL_DX2, umma_smem_desc_sw128(dsaddr + k * 32, 16, 1024),
-                       umma_smem_desc_sw128(yaddr + C::KB1 * C::YBLK + k * 2048, C::YBLK, 1024), idesc_g2, acc | (k != 0));
-        if (TEACHER) {
-#pragma unroll
-          for (int k = 0; k < 4; ++k)
-            umma_bf16_ss(tmem_base + C::COL_DX1, umma_smem_desc_sw128(dsaddr + C::DS_TILE + k * 32, 16, 1024),
-                         umma_smem_desc_sw128(yaddr + k * 2048, C::YBLK, 1024), idesc_g1, acc | (k != 0));
+            for (int k = 0; k < 4; ++k)
+              umma_bf16_ss(tS2, dx2 + uint64_t((kb * C::XBLK + k * 32) >> 4),
+                           dys + uint64_t(((C::KB1 + kb) * C::YBLK + k * 32) >> 4), idesc_s, (kb | k) != 0);
+          umma_commit(&s_full[st]);
         }
-        umma_commit(&ds_empty[w]);
-        umma_commit(&y_empty[s]);
+        __syncwarp();
       };
-      issue_S(0);
+      if (nsteps > 0) issue_S(0);
       for (int it = 0; it < nsteps; ++it) {
-        if (it + 1 < nsteps) issue_S(it + 1);   // keep the tensor pipe busy while the softmax warps work on step `it`
-        issue_dX(it);
+        if (it + 1 < nsteps) issue_S(it + 1);   // the tensor pipe works on the next logits while the dS warps work on step `it`
+        const int s = it % C::NSTAGE;
+        const int st = it & 1;
+        mbar_wait(&ds_full[st], (it >> 1) & 1);
+        tc_fence_after();
+        const uint64_t dys = dym + uint64_t((s * C::Y_STAGE) >> 4);
+        const uint32_t tA = tmem_base + st * 128;
+        const uint32_t acc = it > 0;
+        if (elect_one()) {
+          // K-slice k (16 streamed rows) of dS lives in 8 TMEM columns: column half (k>>1) at +32, slice (k&1) at +8
+#pragma unroll
+          for (int k = 0; k < 4; ++k)
+            umma_bf16_ts(tmem_base + C::COL_DX2, tA + 64 + (k >> 1) * 32 + (k & 1) * 8,
+                         dys + uint64_t((C::KB1 * C::YBLK + k * 2048) >> 4), idesc_g2, acc | (k != 0));
+          if (TEACHER) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k)
+              umma_bf16_ts(tmem_base + C::COL_DX1, tA + (k >> 1) * 32 + (k & 1) * 8, dys + uint64_t((k * 2048) >> 4), idesc_g1,
+                           acc | (k != 0));
+          }
+          umma_commit(&y_empty[s]);
+          if (it + 1 == nsteps) umma_commit(dx_full);
+        }
+        __syncwarp();
       }
-      umma_commit(dx_full);
     }
-  } else if (warp >= 4) {
-    // ===================== softmax / dS warpgroups =====================
-    const int w = (warp - 4) >> 2;
-    const int quarter = warp & 3;
+  } else {
+    // ===================== dS warps =====================
+    reg_alloc<112>();
+    const int sw = warp - 4;
+    const int quarter = warp & 3;             // TMEM lane quarter this warp may access
+    const int grp = sw >> 2;                  // 0..3
+    const int st = grp & 1;                   // S' stage this warp group serves (steps of that parity)
+    const int half = grp >> 1;                // 32-column half of every streamed tile
     const int rloc = quarter * 32 + lane;     // owner row within the tile = TMEM lane
     const int xrow = x0 + rloc;
+    const float L2E = 1.4426950408889634f, LN2 = 0.6931471805599453f;
     const float sc1 = p.c1 * L2E, sc2 = p.c2 * L2E;
-    float my_L1 = 0.f, my_L2 = 0.f, my_g = 0.f, my_term = 0.f;
+    float nL1 = -1e30f, nL2 = -1e30f, klog = 0.f, my_g = 0.f;
     if (!OWNER_K && xrow < p.NQ) {
-      const size_t o = size_t(bh) * p.NQ + xrow;
-      const float a = p.lse1[o], b = p.lse2[o];
-      my_L1 = a * L2E; my_L2 = b * L2E; my_g = p.dkl[o]; my_term = (a - b) + p.kl[o];
+      const float* sp = reinterpret_cast<const float*>(p.stats + (size_t(bh) * NQP + size_t(xrow & ~1)));  // pair (xrow>>1): 2 float4
+      const int u = xrow & 1;
+      nL1 = sp[u]; nL2 = sp[2 + u]; my_g = sp[4 + u]; klog = sp[6 + u];
     }
-    uint8_t* ds2_row = sDS + w * C::DS_PER_WG + rloc * 128;
-    uint8_t* ds1_row = ds2_row + C::DS_TILE;
-    const int sw = rloc & 7;
-    for (int it = w; it < nsteps; it += 2) {
+    const uint32_t lane_addr = tmem_base + (uint32_t(quarter * 32) << 16);
+    for (int it = st; it < nsteps; it += 2) {
       const int j = j_begin + it;
       const int s = it % C::NSTAGE;
-      const uint32_t wph = (it >> 1) & 1;
-      mbar_wait(&s_full[w], wph);
+      mbar_wait(&s_full[st], (it >> 1) & 1);
       tc_fence_after();
-      const uint32_t taddr = tmem_base + (uint32_t(quarter * 32) << 16) + w * 128;
-      uint32_t r1[64], r2[64];
-      tmem_ld32(taddr, *reinterpret_cast<uint32_t(*)[32]>(&r1[0]));
-      tmem_ld32(taddr + 32, *reinterpret_cast<uint32_t(*)[32]>(&r1[32]));
-      tmem_ld32(taddr + 64, *reinterpret_cast<uint32_t(*)[32]>(&r2[0]));
-      tmem_ld32(taddr + 96, *reinterpret_cast<uint32_t(*)[32]>(&r2[32]));
+      const uint32_t taddr = lane_addr + st * 128 + half * 32;
+      uint32_t r1[32], r2[32], o1[16], o2[16];
+      tmem_ld32(taddr, r1);
+      tmem_ld32(taddr + 64, r2);
       tmem_wait_ld();
+      const int y0 = j * C::BY + half * 32;
+      // tile-uniform: does any (query,key) pair of this half tile fall outside the mask?
+      // (a streamed KEY tail is masked too: TMA zero-fills those rows, but P = exp2(0 - lse) may overflow)
+      const bool masked = OWNER_K ? (CAUSAL && (y0 + off < x0 + C::BX - 1))
+                                  : ((CAUSAL && (y0 + 31 > x0 + off)) || (y0 + 32 > p.NK));
+      const float4* stat = sStat + s * C::BY + half * 32;
+      if (masked) ds_row32<TEACHER, OWNER_K, CAUSAL, true>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
+      else        ds_row32<TEACHER, OWNER_K, CAUSAL, false>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
+      // dS over the logits this thread has just consumed: K-elements [32 half, 32 half + 32) -> 16 packed columns
+      tmem_st16(taddr + 64, o2);
+      if (TEACHER) tmem_st16(taddr, o1);
+      tmem_wait_st();
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(&s_empty[w]);
-      const int ybase = j * C::BY;
-      // tile-uniform: does any (query,key) pair of this tile fall outside the causal mask?
-      // (a streamed KEY tail is masked too: TMA zero-fills those rows, but P = exp2(0 - lse) may overflow and inf * 0 = NaN)
-      const bool masked = (CAUSAL && (OWNER_K ? (ybase + off < x0 + C::BX - 1) : (ybase + C::BY - 1 > x0 + off))) ||
-                          (!OWNER_K && ybase + C::BY > p.NK);
-      mbar_wait(&ds_empty[w], wph ^ 1);   // the dX MMAs of this warpgroup's previous step have consumed the dS buffer
-      const float4* stat = sStat + s * C::BY;
-#pragma unroll
-      for (int c = 0; c < 8; ++c) {
-        uint32_t o2[4], o1[4];
-#pragma unroll
-        for (int h = 0; h < 4; ++h) {
-          float d2v[2], d1v[2];
-#pragma unroll
-          for (int u = 0; u < 2; ++u) {
-            const int e = c * 8 + h * 2 + u;
-            float L1 = my_L1, L2 = my_L2, g = my_g, term = my_term;
-            if (OWNER_K) { const float4 t = stat[e]; L1 = t.x; L2 = t.y; g = t.z; term = t.w; }
-            const float s1 = __uint_as_float(r1[e]), s2 = __uint_as_float(r2[e]);
-            const float p1 = ex2_approx(fmaf(s1, sc1, -L1));      // P1 = exp(s1 - lse1)   (Alg.2 line 7)
-            const float p2 = ex2_approx(fmaf(s2, sc2, -L2));
-            float a2 = g * (p2 - p1);                              // dS2 (Alg.2 line 8): fp32 subtract, rounded once below
-            float a1 = 0.f;
-            if (TEACHER) a1 = (g * p1) * (fmaf(s1, p.c1, -term) - s2 * p.c2);   // dS1 (Alg.3 lines 9-10, Eq.12)
-            if (masked) {
-              const bool ok = OWNER_K ? (xrow <= ybase + e + off) : ((ybase + e < p.NK) && (!CAUSAL || ybase + e <= xrow + off));
-              a2 = ok ? a2 : 0.f;
-              a1 = ok ? a1 : 0.f;
-            }
-            d2v[u] = a2; d1v[u] = a1;
-          }
-          o2[h] = pack_bf16x2(d2v[0], d2v[1]);
-          if (TEACHER) o1[h] = pack_bf16x2(d1v[0], d1v[1]);
-        }
-        const int chunk = (c ^ sw) << 4;   // 128-byte swizzle: 16-byte chunk index XOR (row mod 8)
-        *reinterpret_cast<uint4*>(ds2_row + chunk) = make_uint4(o2[0], o2[1], o2[2], o2[3]);
-        if (TEACHER) *reinterpret_cast<uint4*>(ds1_row + chunk) = make_uint4(o1[0], o1[1], o1[2], o1[3]);
-      }
-      fence_proxy_async_smem();   // generic-proxy stores -> visible to the tensor core's async-proxy reads
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&ds_full[w]);
+      if (lane == 0) mbar_arrive(&ds_full[st]);
     }
-    // ---- epilogue: dX (TMEM fp32) * c_t -> bf16 -> HBM
+    // ---- epilogue: dX (TMEM fp32) * c_t -> bf16 -> HBM; each warp group takes a quarter of the columns
     const bool valid = xrow < NX;
-    const uint32_t lane_addr = tmem_base + (uint32_t(quarter * 32) << 16);
     const size_t orow = size_t(bh) * NX + (valid ? xrow : 0);
+    const float g_row = OWNER_K ? 1.f : my_g;   // Q owner: g is a per-row factor of dS, applied here
     if (nsteps > 0) {
       mbar_wait(dx_full, 0);
       tc_fence_after();
-      if (TEACHER) {
-        if (w == 0) store_dx_row<D1>(lane_addr + C::COL_DX1, p.c1, p.dX1 + orow * D1, valid);
-        else        store_dx_row<D2>(lane_addr + C::COL_DX2, p.c2, p.dX2 + orow * D2, valid);
-      } else {
-        store_dx_row<D2 / 2>(lane_addr + C::COL_DX2 + w * (D2 / 2), p.c2, p.dX2 + orow * D2 + w * (D2 / 2), valid);
-      }
+      store_dx_cols<D2 / 4>(lane_addr + C::COL_DX2 + grp * (D2 / 4), p.c2 * g_row, p.dX2 + orow * D2 + grp * (D2 / 4), valid);
+      if (TEACHER)
+        store_dx_cols<D1 / 4>(lane_addr + C::COL_DX1 + grp * (D1 / 4), p.c1 * LN2 * g_row, p.dX1 + orow * D1 + grp * (D1 / 4), valid);
     } else if (valid) {
       const uint4 z = make_uint4(0, 0, 0, 0);
-      if (w == 0) { for (int c = 0; c < D2; c += 8) *reinterpret_cast<uint4*>(p.dX2 + orow * D2 + c) = z; }
-      else if (TEACHER) { for (int c = 0; c < D1; c += 8) *reinterpret_cast<uint4*>(p.dX1 + orow * D1 + c) = z; }
+      for (int c = 0; c < D2 / 4; c += 8) *reinterpret_cast<uint4*>(p.dX2 + orow * D2 + grp * (D2 / 4) + c) = z;
+      if (TEACHER) for (int c = 0; c < D1 / 4; c += 8) *reinterpret_cast<uint4*>(p.dX1 + orow * D1 + grp * (D1 / 4) + c) = z;
     }
   }
   tc_fence_before();
