@@ -20,8 +20,8 @@
 // layout -- padded to a multiple of 64 queries per head with values that make padded queries contribute exactly 0.
 //
 // Warp roles (640 threads): warp 0 TMA producer (X once, Y ring + the streamed queries' scalars when OWNER_K),
-// warp 1 MMA issuer, warp 2 TMEM allocator, warps 4-19 sixteen dS warps = 2 S' stages x 2 column halves x 4 TMEM
-// lane quarters.  TMEM (512 columns): two S' stages of {S1' 64, S2' 64} (dS aliases them) + D1 + D2 accumulator columns.
+// warp 1 MMA issuer, warp 2 TMEM allocator, warps 4-19 sixteen dS warps = 4 column quarters x 4 TMEM lane quarters,
+// all on the same step.  TMEM (512 columns): two S' stages of {S1' 64, S2' 64} (dS aliases them) + D1 + D2 accumulator columns.
 #pragma once
 #include <cuda_bf16.h>
 #include <math_constants.h>
@@ -111,20 +111,27 @@ __device__ __forceinline__ void store_dx_cols(uint32_t taddr, float scale, __nv_
   }
 }
 
-// B3 + B4 for one owner row and 32 streamed columns: logits r1,r2 (fp32 bits) -> packed bf16 dS1 (o1), dS2 (o2).
+__device__ __forceinline__ float4 lds_f4(uint32_t saddr) {
+  float4 v;
+  asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(saddr));
+  return v;
+}
+
+// B3 + B4 for one owner row and 16 streamed columns: logits r1,r2 (fp32 bits) -> packed bf16 dS1 (o1), dS2 (o2).
 //   OWNER_Q: the row's scalars (nL1,nL2,klog) are thread constants and g is applied in the epilogue.
-//   OWNER_K: per-column scalars come from shared memory (`stat`, this half's 16 column pairs), g is applied here.
+//   OWNER_K: per-column scalars come from shared memory (`stat`: shared-space address of this quarter's 8 column
+//            pairs, two float4 each), g is applied here.
 // MASKED: causal diagonal tiles and streamed-key tails; P (possibly inf for a zero-filled logit) is discarded by SELECT.
 template <bool TEACHER, bool OWNER_K, bool CAUSAL, bool MASKED>
-__device__ __forceinline__ void ds_row32(const uint32_t (&r1)[32], const uint32_t (&r2)[32], uint32_t (&o1)[16], uint32_t (&o2)[16],
-                                         float sc1, float sc2, float nL1, float nL2, float klog, const float4* stat, int xrow,
+__device__ __forceinline__ void ds_row16(const uint32_t (&r1)[16], const uint32_t (&r2)[16], uint32_t (&o1)[8], uint32_t (&o2)[8],
+                                         float sc1, float sc2, float nL1, float nL2, float klog, uint32_t stat, int xrow,
                                          int y0, int off, int NK) {
   const float2 vsc1 = make_float2(sc1, sc1), vsc2 = make_float2(sc2, sc2);
   float2 vn1 = make_float2(nL1, nL1), vn2 = make_float2(nL2, nL2), vk = make_float2(klog, klog), vg = make_float2(1.f, 1.f);
 #pragma unroll
-  for (int e = 0; e < 32; e += 2) {
+  for (int e = 0; e < 16; e += 2) {
     if constexpr (OWNER_K) {
-      const float4 a = stat[e], b = stat[e + 1];   // pair e/2: two float4
+      const float4 a = lds_f4(stat + e * 16), b = lds_f4(stat + e * 16 + 16);   // pair e/2: two float4
       vn1 = make_float2(a.x, a.y); vn2 = make_float2(a.z, a.w); vg = make_float2(b.x, b.y); vk = make_float2(b.z, b.w);
     }
     const float2 x1 = fma2(make_float2(__uint_as_float(r1[e]), __uint_as_float(r1[e + 1])), vsc1, vn1);
@@ -198,7 +205,7 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
   if (warp == 1 && lane == 0) {
     mbar_init(x_full, 1);
     for (int s = 0; s < C::NSTAGE; ++s) { mbar_init(&y_full[s], 1); mbar_init(&y_empty[s], 1); }
-    for (int w = 0; w < 2; ++w) { mbar_init(&s_full[w], 1); mbar_init(&ds_full[w], 8); }
+    for (int w = 0; w < 2; ++w) { mbar_init(&s_full[w], 1); mbar_init(&ds_full[w], 16); }
     mbar_init(dx_full, 1);
     fence_mbar_init();
   }
@@ -288,15 +295,15 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
         const uint32_t tA = tmem_base + st * 128;
         const uint32_t acc = it > 0;
         if (elect_one()) {
-          // K-slice k (16 streamed rows) of dS lives in 8 TMEM columns: column half (k>>1) at +32, slice (k&1) at +8
+          // K-slice k (16 streamed rows) of dS lives in the first 8 of warp group k's 16 columns
 #pragma unroll
           for (int k = 0; k < 4; ++k)
-            umma_bf16_ts(tmem_base + C::COL_DX2, tA + 64 + (k >> 1) * 32 + (k & 1) * 8,
+            umma_bf16_ts(tmem_base + C::COL_DX2, tA + 64 + k * 16,
                          dys + uint64_t((C::KB1 * C::YBLK + k * 2048) >> 4), idesc_g2, acc | (k != 0));
           if (TEACHER) {
 #pragma unroll
             for (int k = 0; k < 4; ++k)
-              umma_bf16_ts(tmem_base + C::COL_DX1, tA + (k >> 1) * 32 + (k & 1) * 8, dys + uint64_t((k * 2048) >> 4), idesc_g1,
+              umma_bf16_ts(tmem_base + C::COL_DX1, tA + k * 16, dys + uint64_t((k * 2048) >> 4), idesc_g1,
                            acc | (k != 0));
           }
           umma_commit(&y_empty[s]);
@@ -310,9 +317,7 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
     reg_alloc<112>();
     const int sw = warp - 4;
     const int quarter = warp & 3;             // TMEM lane quarter this warp may access
-    const int grp = sw >> 2;                  // 0..3
-    const int st = grp & 1;                   // S' stage this warp group serves (steps of that parity)
-    const int half = grp >> 1;                // 32-column half of every streamed tile
+    const int grp = sw >> 2;                  // 0..3: the 16-column quarter of every streamed tile this warp group takes
     const int rloc = quarter * 32 + lane;     // owner row within the tile = TMEM lane
     const int xrow = x0 + rloc;
     const float L2E = 1.4426950408889634f, LN2 = 0.6931471805599453f;
@@ -324,27 +329,31 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
       nL1 = sp[u]; nL2 = sp[2 + u]; my_g = sp[4 + u]; klog = sp[6 + u];
     }
     const uint32_t lane_addr = tmem_base + (uint32_t(quarter * 32) << 16);
-    for (int it = st; it < nsteps; it += 2) {
+    const uint32_t stat_base = smem_u32(sStat) + grp * 16 * 16;
+    // All sixteen warps work on the same step (one owner row x 16 streamed columns per thread): while they do, the
+    // tensor pipe runs dX of the previous step and S' of the next one into the other stage.
+    for (int it = 0; it < nsteps; ++it) {
       const int j = j_begin + it;
       const int s = it % C::NSTAGE;
+      const int st = it & 1;
       mbar_wait(&s_full[st], (it >> 1) & 1);
       tc_fence_after();
-      const uint32_t taddr = lane_addr + st * 128 + half * 32;
-      uint32_t r1[32], r2[32], o1[16], o2[16];
-      tmem_ld32(taddr, r1);
-      tmem_ld32(taddr + 64, r2);
+      const uint32_t taddr = lane_addr + st * 128 + grp * 16;
+      uint32_t r1[16], r2[16], o1[8], o2[8];
+      tmem_ld16(taddr, r1);
+      tmem_ld16(taddr + 64, r2);
       tmem_wait_ld();
-      const int y0 = j * C::BY + half * 32;
-      // tile-uniform: does any (query,key) pair of this half tile fall outside the mask?
+      const int y0 = j * C::BY + grp * 16;
+      // warp-uniform: does any (query,key) pair of this 128 x 16 block fall outside the mask?
       // (a streamed KEY tail is masked too: TMA zero-fills those rows, but P = exp2(0 - lse) may overflow)
       const bool masked = OWNER_K ? (CAUSAL && (y0 + off < x0 + C::BX - 1))
-                                  : ((CAUSAL && (y0 + 31 > x0 + off)) || (y0 + 32 > p.NK));
-      const float4* stat = sStat + s * C::BY + half * 32;
-      if (masked) ds_row32<TEACHER, OWNER_K, CAUSAL, true>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
-      else        ds_row32<TEACHER, OWNER_K, CAUSAL, false>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
-      // dS over the logits this thread has just consumed: K-elements [32 half, 32 half + 32) -> 16 packed columns
-      tmem_st16(taddr + 64, o2);
-      if (TEACHER) tmem_st16(taddr, o1);
+                                  : ((CAUSAL && (y0 + 15 > x0 + off)) || (y0 + 16 > p.NK));
+      const uint32_t stat = stat_base + s * C::STAT_STAGE;
+      if (masked) ds_row16<TEACHER, OWNER_K, CAUSAL, true>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
+      else        ds_row16<TEACHER, OWNER_K, CAUSAL, false>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
+      // dS over the logits this thread has just consumed: K-elements [16 grp, 16 grp + 16) -> 8 packed columns
+      tmem_st8(taddr + 64, o2);
+      if (TEACHER) tmem_st8(taddr, o1);
       tmem_wait_st();
       tc_fence_before();
       __syncwarp();
