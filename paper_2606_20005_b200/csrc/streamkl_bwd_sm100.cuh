@@ -20,8 +20,12 @@
 // layout -- padded to a multiple of 64 queries per head with values that make padded queries contribute exactly 0.
 //
 // Warp roles (640 threads): warp 0 TMA producer (X once, Y ring + the streamed queries' scalars when OWNER_K),
-// warp 1 MMA issuer, warp 2 TMEM allocator, warps 4-19 sixteen dS warps = 4 column quarters x 4 TMEM lane quarters,
-// all on the same step.  TMEM (512 columns): two S' stages of {S1' 64, S2' 64} (dS aliases them) + D1 + D2 accumulator columns.
+// warp 1 issues the S' MMAs, warp 3 issues the dX MMAs (two independent in-order streams into the tensor pipe, so a
+// ready dX never queues behind an S' that waits for its TMEM stage and vice versa), warp 2 TMEM allocator,
+// warps 4-19 sixteen dS warps = 2 step parities x 2 column halves x 4 TMEM lane quarters.
+// TMEM (512 columns): NSS S' stages of {S1' 64, S2' 64}, released as soon as the dS warps hold the logits in registers;
+// two dS stages of {dS1 32, dS2 32} packed-bf16 columns; D1 + D2 accumulator columns.  The two parity groups run
+// decoupled: one group's TMEM load / store / barrier phases overlap the other group's exp phase.
 #pragma once
 #include <cuda_bf16.h>
 #include <math_constants.h>
@@ -47,7 +51,11 @@ struct BwdCfg {
   static constexpr int SMEM_BYTES = 1024 + X_BYTES + NSTAGE * (Y_STAGE + STAT_STAGE) + AUX_BYTES;
   static constexpr int THREADS = 128 + 512;
   static constexpr uint32_t TMEM_COLS = 512;
-  static constexpr uint32_t COL_DX1 = 256, COL_DX2 = 256 + (TEACHER ? D1 : 0);   // after the two S' stages (2 x 128)
+  static constexpr int DX_COLS = D2 + (TEACHER ? D1 : 0);
+  static constexpr int NSS = (512 - 128 - DX_COLS) / 128 >= 2 ? 2 : 1;           // S' stages that fit beside dS and dX
+  static constexpr uint32_t COL_DS = NSS * 128;                                   // 2 stages x {dS1 32, dS2 32}
+  static constexpr uint32_t COL_DX1 = COL_DS + 128, COL_DX2 = COL_DX1 + (TEACHER ? D1 : 0);
+  static_assert(COL_DX2 + D2 <= 512, "TMEM budget");
 };
 
 // queries per head in the padded per-query scalar array
@@ -117,19 +125,19 @@ __device__ __forceinline__ float4 lds_f4(uint32_t saddr) {
   return v;
 }
 
-// B3 + B4 for one owner row and 16 streamed columns: logits r1,r2 (fp32 bits) -> packed bf16 dS1 (o1), dS2 (o2).
+// B3 + B4 for one owner row and NC streamed columns: logits r1,r2 (fp32 bits) -> packed bf16 dS1 (o1), dS2 (o2).
 //   OWNER_Q: the row's scalars (nL1,nL2,klog) are thread constants and g is applied in the epilogue.
-//   OWNER_K: per-column scalars come from shared memory (`stat`: shared-space address of this quarter's 8 column
+//   OWNER_K: per-column scalars come from shared memory (`stat`: shared-space address of these NC/2 column
 //            pairs, two float4 each), g is applied here.
 // MASKED: causal diagonal tiles and streamed-key tails; P (possibly inf for a zero-filled logit) is discarded by SELECT.
-template <bool TEACHER, bool OWNER_K, bool CAUSAL, bool MASKED>
-__device__ __forceinline__ void ds_row16(const uint32_t (&r1)[16], const uint32_t (&r2)[16], uint32_t (&o1)[8], uint32_t (&o2)[8],
+template <int NC, bool TEACHER, bool OWNER_K, bool CAUSAL, bool MASKED>
+__device__ __forceinline__ void ds_row(const uint32_t (&r1)[NC], const uint32_t (&r2)[NC], uint32_t (&o1)[NC / 2], uint32_t (&o2)[NC / 2],
                                          float sc1, float sc2, float nL1, float nL2, float klog, uint32_t stat, int xrow,
                                          int y0, int off, int NK) {
   const float2 vsc1 = make_float2(sc1, sc1), vsc2 = make_float2(sc2, sc2);
   float2 vn1 = make_float2(nL1, nL1), vn2 = make_float2(nL2, nL2), vk = make_float2(klog, klog), vg = make_float2(1.f, 1.f);
 #pragma unroll
-  for (int e = 0; e < 16; e += 2) {
+  for (int e = 0; e < NC; e += 2) {
     if constexpr (OWNER_K) {
       const float4 a = lds_f4(stat + e * 16), b = lds_f4(stat + e * 16 + 16);   // pair e/2: two float4
       vn1 = make_float2(a.x, a.y); vn2 = make_float2(a.z, a.w); vg = make_float2(b.x, b.y); vk = make_float2(b.z, b.w);
@@ -158,6 +166,7 @@ __device__ __forceinline__ void ds_row16(const uint32_t (&r1)[16], const uint32_
   }
 }
 
+
 template <int D1, int D2, bool CAUSAL, bool TEACHER, bool OWNER_K>
 __global__ void __launch_bounds__(BwdCfg<D1, D2, TEACHER>::THREADS, 1)
 streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid_constant__ CUtensorMap tmK1,
@@ -171,11 +180,13 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
   float4* sStat = reinterpret_cast<float4*>(sY + C::NSTAGE * C::Y_STAGE);   // NSTAGE x 64 float4
   uint64_t* bars = reinterpret_cast<uint64_t*>(reinterpret_cast<uint8_t*>(sStat) + C::NSTAGE * C::STAT_STAGE);
   uint64_t* x_full = bars;                       // 1
-  uint64_t* y_full = bars + 1;                   // NSTAGE
-  uint64_t* y_empty = y_full + C::NSTAGE;        // NSTAGE
-  uint64_t* s_full = y_empty + C::NSTAGE;        // 2 (per S' stage)
-  uint64_t* ds_full = s_full + 2;                // 2
-  uint64_t* dx_full = ds_full + 2;               // 1
+  uint64_t* y_full = bars + 1;                   // NSTAGE  (TMA bytes landed)
+  uint64_t* y_empty = y_full + C::NSTAGE;        // NSTAGE  (count 2: the S' MMAs and the dX MMAs that read the stage have retired)
+  uint64_t* s_full = y_empty + C::NSTAGE;        // 2  (per parity group) logits of the group's next step are in TMEM
+  uint64_t* s_empty = s_full + 2;                // 2  (per parity group) its 8 dS warps hold those logits in registers
+  uint64_t* ds_full = s_empty + 2;               // 2  dS stage written by its 8 dS warps
+  uint64_t* ds_empty = ds_full + 2;              // 2  dS stage consumed by the dX MMAs
+  uint64_t* dx_full = ds_empty + 2;              // 1
   uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(dx_full + 1);
 
   const CUtensorMap* tmX1 = OWNER_K ? &tmK1 : &tmQ1;
@@ -204,8 +215,11 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
   }
   if (warp == 1 && lane == 0) {
     mbar_init(x_full, 1);
-    for (int s = 0; s < C::NSTAGE; ++s) { mbar_init(&y_full[s], 1); mbar_init(&y_empty[s], 1); }
-    for (int w = 0; w < 2; ++w) { mbar_init(&s_full[w], 1); mbar_init(&ds_full[w], 16); }
+    for (int s = 0; s < C::NSTAGE; ++s) { mbar_init(&y_full[s], 1); mbar_init(&y_empty[s], 2); }
+    for (int w = 0; w < 2; ++w) {
+      mbar_init(&s_full[w], 1); mbar_init(&s_empty[w], 8);
+      mbar_init(&ds_full[w], 8); mbar_init(&ds_empty[w], 1);
+    }
     mbar_init(dx_full, 1);
     fence_mbar_init();
   }
@@ -243,30 +257,27 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
         }
       }
     } else if (warp == 1) {
-      // ===================== MMA issuer =====================
+      // ===================== S' MMA issuer =====================
       // The whole warp runs the loop (warp-uniform control flow); only the tcgen05 instructions are issued by one lane.
       constexpr uint32_t idesc_s = umma_idesc_bf16(C::BX, C::BY, 0, 0);      // S' = X Y^T   : A,B K-major from smem
-      constexpr uint32_t idesc_g1 = umma_idesc_bf16(C::BX, D1, 0, 1);        // dX1 += dS1 Y1: A from TMEM, B MN-major
-      constexpr uint32_t idesc_g2 = umma_idesc_bf16(C::BX, D2, 0, 1);
       const uint64_t dx1 = umma_smem_desc_sw128(smem_u32(sX1), 16, 1024);
       const uint64_t dx2 = umma_smem_desc_sw128(smem_u32(sX2), 16, 1024);
-      const uint64_t dyk = umma_smem_desc_sw128(smem_u32(sY), 16, 1024);          // Y as the K-major B operand of S'
-      const uint64_t dym = umma_smem_desc_sw128(smem_u32(sY), C::YBLK, 1024);     // Y as the MN-major B operand of dX:
-      //   64-column chunks YBLK apart (LBO), 8-row groups 1024 B apart (SBO); a K=16 slice = 16 streamed rows = 2048 B
+      const uint64_t dyk = umma_smem_desc_sw128(smem_u32(sY), 16, 1024);
       if (nsteps > 0) {
         mbar_wait(x_full, 0);
         tc_fence_after();
       }
-      auto issue_S = [&](int it) {
+      for (int it = 0; it < nsteps; ++it) {
         const int s = it % C::NSTAGE;
-        const uint32_t ph = (it / C::NSTAGE) & 1;
-        const int st = it & 1;
-        mbar_wait(&y_full[s], ph);
+        const int ss = it % C::NSS;
+        const int prev = it - C::NSS;                    // the step whose logits this S' stage held last
+        mbar_wait(&y_full[s], (it / C::NSTAGE) & 1);
+        // s_full / s_empty are indexed by the PARITY GROUP that consumes the step (not by the stage), so that each
+        // barrier is observed phase by phase by one group: a parity wait cannot tell phase n from phase n+2
+        if (prev >= 0) mbar_wait(&s_empty[prev & 1], (prev >> 1) & 1);   // those logits are in registers
         tc_fence_after();
-        // No "stage empty" barrier: the previous user of this S' stage is step it-2, whose dS was awaited (ds_full)
-        // before its dX MMAs were issued, and tcgen05.mma executes in issue order.
         const uint64_t dys = dyk + uint64_t((s * C::Y_STAGE) >> 4);
-        const uint32_t tS1 = tmem_base + st * 128, tS2 = tS1 + 64;
+        const uint32_t tS1 = tmem_base + ss * 128, tS2 = tS1 + 64;
         if (elect_one()) {
 #pragma unroll
           for (int kb = 0; kb < C::KB1; ++kb)
@@ -280,33 +291,39 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
             for (int k = 0; k < 4; ++k)
               umma_bf16_ss(tS2, dx2 + uint64_t((kb * C::XBLK + k * 32) >> 4),
                            dys + uint64_t(((C::KB1 + kb) * C::YBLK + k * 32) >> 4), idesc_s, (kb | k) != 0);
-          umma_commit(&s_full[st]);
+          umma_commit(&s_full[it & 1]);
+          umma_commit(&y_empty[s]);     // first of the two arrivals that free the Y stage
         }
         __syncwarp();
-      };
-      if (nsteps > 0) issue_S(0);
+      }
+    } else if (warp == 3) {
+      // ===================== dX MMA issuer =====================
+      constexpr uint32_t idesc_g1 = umma_idesc_bf16(C::BX, D1, 0, 1);        // dX1 += dS1 Y1: A from TMEM, B MN-major
+      constexpr uint32_t idesc_g2 = umma_idesc_bf16(C::BX, D2, 0, 1);
+      // Y as the MN-major B operand: 64-column chunks YBLK apart (LBO), 8-row groups 1024 B apart (SBO);
+      // a K=16 slice = 16 streamed rows = 2048 B
+      const uint64_t dym = umma_smem_desc_sw128(smem_u32(sY), C::YBLK, 1024);
       for (int it = 0; it < nsteps; ++it) {
-        if (it + 1 < nsteps) issue_S(it + 1);   // the tensor pipe works on the next logits while the dS warps work on step `it`
         const int s = it % C::NSTAGE;
         const int st = it & 1;
-        mbar_wait(&ds_full[st], (it >> 1) & 1);
+        mbar_wait(&ds_full[st], (it >> 1) & 1);   // implies the Y stage is resident (its S' MMAs ran before the dS warps did)
         tc_fence_after();
         const uint64_t dys = dym + uint64_t((s * C::Y_STAGE) >> 4);
-        const uint32_t tA = tmem_base + st * 128;
+        const uint32_t tA = tmem_base + C::COL_DS + st * 64;
         const uint32_t acc = it > 0;
         if (elect_one()) {
-          // K-slice k (16 streamed rows) of dS lives in the first 8 of warp group k's 16 columns
+          // K-slice k (16 streamed rows) of dS = 8 packed-bf16 TMEM columns
 #pragma unroll
           for (int k = 0; k < 4; ++k)
-            umma_bf16_ts(tmem_base + C::COL_DX2, tA + 64 + k * 16,
-                         dys + uint64_t((C::KB1 * C::YBLK + k * 2048) >> 4), idesc_g2, acc | (k != 0));
+            umma_bf16_ts(tmem_base + C::COL_DX2, tA + 32 + k * 8, dys + uint64_t((C::KB1 * C::YBLK + k * 2048) >> 4), idesc_g2,
+                         acc | (k != 0));
           if (TEACHER) {
 #pragma unroll
             for (int k = 0; k < 4; ++k)
-              umma_bf16_ts(tmem_base + C::COL_DX1, tA + k * 16, dys + uint64_t((k * 2048) >> 4), idesc_g1,
-                           acc | (k != 0));
+              umma_bf16_ts(tmem_base + C::COL_DX1, tA + k * 8, dys + uint64_t((k * 2048) >> 4), idesc_g1, acc | (k != 0));
           }
-          umma_commit(&y_empty[s]);
+          umma_commit(&ds_empty[st]);
+          umma_commit(&y_empty[s]);     // second arrival
           if (it + 1 == nsteps) umma_commit(dx_full);
         }
         __syncwarp();
@@ -317,7 +334,9 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
     reg_alloc<112>();
     const int sw = warp - 4;
     const int quarter = warp & 3;             // TMEM lane quarter this warp may access
-    const int grp = sw >> 2;                  // 0..3: the 16-column quarter of every streamed tile this warp group takes
+    const int grp = sw >> 2;                  // 0..3
+    const int par = grp & 1;                  // this warp group takes the steps of that parity (= its dS stage)
+    const int half = grp >> 1;                // 32-column half of every streamed tile
     const int rloc = quarter * 32 + lane;     // owner row within the tile = TMEM lane
     const int xrow = x0 + rloc;
     const float L2E = 1.4426950408889634f, LN2 = 0.6931471805599453f;
@@ -329,35 +348,38 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
       nL1 = sp[u]; nL2 = sp[2 + u]; my_g = sp[4 + u]; klog = sp[6 + u];
     }
     const uint32_t lane_addr = tmem_base + (uint32_t(quarter * 32) << 16);
-    const uint32_t stat_base = smem_u32(sStat) + grp * 16 * 16;
-    // All sixteen warps work on the same step (one owner row x 16 streamed columns per thread): while they do, the
-    // tensor pipe runs dX of the previous step and S' of the next one into the other stage.
-    for (int it = 0; it < nsteps; ++it) {
+    const uint32_t stat_base = smem_u32(sStat) + half * 32 * 16;
+    const uint32_t ds_addr = lane_addr + C::COL_DS + par * 64 + half * 16;   // dS1 here, dS2 32 columns further
+    for (int it = par; it < nsteps; it += 2) {
       const int j = j_begin + it;
       const int s = it % C::NSTAGE;
-      const int st = it & 1;
-      mbar_wait(&s_full[st], (it >> 1) & 1);
+      const int ss = it % C::NSS;
+      mbar_wait(&s_full[par], (it >> 1) & 1);
       tc_fence_after();
-      const uint32_t taddr = lane_addr + st * 128 + grp * 16;
-      uint32_t r1[16], r2[16], o1[8], o2[8];
-      tmem_ld16(taddr, r1);
-      tmem_ld16(taddr + 64, r2);
+      const uint32_t taddr = lane_addr + ss * 128 + half * 32;
+      uint32_t r1[32], r2[32], o1[16], o2[16];
+      tmem_ld32(taddr, r1);
+      tmem_ld32(taddr + 64, r2);
       tmem_wait_ld();
-      const int y0 = j * C::BY + grp * 16;
-      // warp-uniform: does any (query,key) pair of this 128 x 16 block fall outside the mask?
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&s_empty[par]);   // logits are in registers: the next S' may overwrite this stage
+      const int y0 = j * C::BY + half * 32;
+      // warp-uniform: does any (query,key) pair of this 128 x 32 block fall outside the mask?
       // (a streamed KEY tail is masked too: TMA zero-fills those rows, but P = exp2(0 - lse) may overflow)
       const bool masked = OWNER_K ? (CAUSAL && (y0 + off < x0 + C::BX - 1))
-                                  : ((CAUSAL && (y0 + 15 > x0 + off)) || (y0 + 16 > p.NK));
+                                  : ((CAUSAL && (y0 + 31 > x0 + off)) || (y0 + 32 > p.NK));
       const uint32_t stat = stat_base + s * C::STAT_STAGE;
-      if (masked) ds_row16<TEACHER, OWNER_K, CAUSAL, true>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
-      else        ds_row16<TEACHER, OWNER_K, CAUSAL, false>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
-      // dS over the logits this thread has just consumed: K-elements [16 grp, 16 grp + 16) -> 8 packed columns
-      tmem_st8(taddr + 64, o2);
-      if (TEACHER) tmem_st8(taddr, o1);
+      if (masked) ds_row<32, TEACHER, OWNER_K, CAUSAL, true>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
+      else        ds_row<32, TEACHER, OWNER_K, CAUSAL, false>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
+      mbar_wait(&ds_empty[par], ((it >> 1) & 1) ^ 1);   // the dX MMAs of step it-2 have consumed this dS stage
+      tc_fence_after();
+      tmem_st16(ds_addr + 32, o2);
+      if (TEACHER) tmem_st16(ds_addr, o1);
       tmem_wait_st();
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(&ds_full[st]);
+      if (lane == 0) mbar_arrive(&ds_full[par]);
     }
     // ---- epilogue: dX (TMEM fp32) * c_t -> bf16 -> HBM; each warp group takes a quarter of the columns
     const bool valid = xrow < NX;
