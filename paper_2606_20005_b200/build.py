@@ -56,6 +56,7 @@ def find_nvcc() -> str:
 def build_library(force: bool = False, debug_timeout: bool = False, verbose: bool = False) -> str:
     """Compile every .cu under csrc/ into paper_2606_20005_b200/libstreamkl.so; returns its path."""
     extra = ["-DSTREAMKL_DEBUG_TIMEOUT"] if debug_timeout else []
+    extra += os.environ.get("STREAMKL_NVCC_EXTRA", "").split()   # tuning macros, e.g. -DSTREAMKL_FWD_POLY_EVERY=3
     want = _digest(extra)
     if not force and os.path.exists(LIB_PATH) and os.path.exists(STAMP_PATH):
         with open(STAMP_PATH) as fh:

@@ -31,14 +31,18 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+// Suspend-time hint of every try_wait: the thread sleeps in hardware until the phase completes (or the hint expires)
+// instead of re-issuing the poll.  A tight poll loop floods the SM's MIO queue, which the MUFU instructions of the
+// softmax warps share (ncu: the exps stall on mio_throttle while an idle producer lane spins).
+constexpr uint32_t kMbarSuspendNs = 1000000u;
 __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
   uint32_t ok;
   asm volatile(
       "{\n\t.reg .pred p;\n\t"
-      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
       "selp.u32 %0, 1, 0, p;\n\t}\n"
       : "=r"(ok)
-      : "r"(smem_u32(bar)), "r"(parity)
+      : "r"(smem_u32(bar)), "r"(parity), "r"(kMbarSuspendNs)
       : "memory");
   return ok != 0;
 }
@@ -46,7 +50,7 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
 #ifdef STREAMKL_DEBUG_TIMEOUT
   for (long long it = 0; !mbar_try_wait(bar, parity); ++it)
-    if (it > (1ll << 24)) { printf("mbar timeout blk %d thr %d bar %p par %u\n", blockIdx.x, threadIdx.x, bar, parity); __trap(); }
+    if (it > (1ll << 12)) { printf("mbar timeout blk %d thr %d bar %p par %u\n", blockIdx.x, threadIdx.x, bar, parity); __trap(); }
 #else
   while (!mbar_try_wait(bar, parity)) {}
 #endif
@@ -216,6 +220,23 @@ __device__ __forceinline__ float2 mul2(float2 a, float2 b) {
   uint64_t d;
   asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(reinterpret_cast<uint64_t&>(a)), "l"(reinterpret_cast<uint64_t&>(b)));
   return reinterpret_cast<float2&>(d);
+}
+// exp2 on the FMA and ALU pipes, no MUFU (north_star: "FMA-polynomial exp2 where ncu shows MUFU is the limiter"):
+// round-to-nearest split x = n + f via the 1.5*2^23 magic constant, degree-3 minimax of 2^f on [-0.5, 0.5]
+// (relative error 7.6e-5, fitted in fp32), exponent inserted with an integer shift-add.  Two lanes per call so the
+// adds and FMAs are packed fp32x2.  Inputs are clamped at -126 (results below 2^-126 come out as ~1e-38, not 0);
+// valid for x < 2^22, meant for the x <= 0 arguments of a max-shifted softmax.
+__device__ __forceinline__ float2 ex2_poly2(float2 x) {
+  const float2 magic = make_float2(12582912.f, 12582912.f);
+  x.x = fmaxf(x.x, -126.f);
+  x.y = fmaxf(x.y, -126.f);
+  const float2 t = add2(x, magic);           // low mantissa bits of t = n (two's complement)
+  const float2 f = sub2(x, sub2(t, magic));  // f in [-0.5, 0.5]
+  float2 p = fma2(f, make_float2(0.055205512791872025f, 0.055205512791872025f), make_float2(0.24261389672756195f, 0.24261389672756195f));
+  p = fma2(p, f, make_float2(0.6932547688484192f, 0.6932547688484192f));
+  p = fma2(p, f, make_float2(0.9999276995658875f, 0.9999276995658875f));
+  return make_float2(__int_as_float((__float_as_int(t.x) << 23) + __float_as_int(p.x)),
+                     __int_as_float((__float_as_int(t.y) << 23) + __float_as_int(p.y)));
 }
 __device__ __forceinline__ float max3(float a, float b, float c) {
   float y;

@@ -276,20 +276,23 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
         // barrier is observed phase by phase by one group: a parity wait cannot tell phase n from phase n+2
         if (prev >= 0) mbar_wait(&s_empty[prev & 1], (prev >> 1) & 1);   // those logits are in registers
         tc_fence_after();
-        const uint64_t dys = dyk + uint64_t((s * C::Y_STAGE) >> 4);
+        uint64_t dys = dyk + uint64_t((s * C::Y_STAGE) >> 4), a1 = dx1, a2 = dx2;
+        // launder the descriptor bases: every MMA's descriptors are then formed as base + immediate beside it instead
+        // of sixteen loop-invariant 64-bit values being hoisted (and spilled: this warp runs on 32 registers)
+        asm volatile("" : "+l"(a1), "+l"(a2), "+l"(dys));
         const uint32_t tS1 = tmem_base + ss * 128, tS2 = tS1 + 64;
         if (elect_one()) {
 #pragma unroll
           for (int kb = 0; kb < C::KB1; ++kb)
 #pragma unroll
             for (int k = 0; k < 4; ++k)
-              umma_bf16_ss(tS1, dx1 + uint64_t((kb * C::XBLK + k * 32) >> 4), dys + uint64_t((kb * C::YBLK + k * 32) >> 4), idesc_s,
+              umma_bf16_ss(tS1, a1 + uint64_t((kb * C::XBLK + k * 32) >> 4), dys + uint64_t((kb * C::YBLK + k * 32) >> 4), idesc_s,
                            (kb | k) != 0);
 #pragma unroll
           for (int kb = 0; kb < C::KB2; ++kb)
 #pragma unroll
             for (int k = 0; k < 4; ++k)
-              umma_bf16_ss(tS2, dx2 + uint64_t((kb * C::XBLK + k * 32) >> 4),
+              umma_bf16_ss(tS2, a2 + uint64_t((kb * C::XBLK + k * 32) >> 4),
                            dys + uint64_t(((C::KB1 + kb) * C::YBLK + k * 32) >> 4), idesc_s, (kb | k) != 0);
           umma_commit(&s_full[it & 1]);
           umma_commit(&y_empty[s]);     // first of the two arrivals that free the Y stage
@@ -308,7 +311,8 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
         const int st = it & 1;
         mbar_wait(&ds_full[st], (it >> 1) & 1);   // implies the Y stage is resident (its S' MMAs ran before the dS warps did)
         tc_fence_after();
-        const uint64_t dys = dym + uint64_t((s * C::Y_STAGE) >> 4);
+        uint64_t dys = dym + uint64_t((s * C::Y_STAGE) >> 4);
+        asm volatile("" : "+l"(dys));
         const uint32_t tA = tmem_base + C::COL_DS + st * 64;
         const uint32_t acc = it > 0;
         if (elect_one()) {

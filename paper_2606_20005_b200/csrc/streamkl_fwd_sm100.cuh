@@ -19,6 +19,12 @@
 
 #include "sm100_ptx.cuh"
 
+// Share of the forward's exps evaluated by the FMA-pipe polynomial (ex2_poly2): one column pair in every
+// STREAMKL_FWD_POLY_EVERY (0 = none).  The forward is MUFU-bound 2:1 against the tensor pipe.
+#ifndef STREAMKL_FWD_POLY_EVERY
+#define STREAMKL_FWD_POLY_EVERY 4
+#endif
+
 namespace skl {
 
 template <int D1, int D2>
@@ -98,8 +104,10 @@ __device__ __forceinline__ void online_update(RowState& st, const uint32_t (&r1)
     for (int e = 0; e < NC; e += 2) {
       const float2 x1 = fma2(make_float2(__uint_as_float(r1[e]), __uint_as_float(r1[e + 1])), vsc1, vr1);
       const float2 x2 = fma2(make_float2(__uint_as_float(r2[e]), __uint_as_float(r2[e + 1])), vsc2, vr2);
-      const float2 p1 = make_float2(ex2_approx(x1.x), ex2_approx(x1.y));
-      const float2 p2 = make_float2(ex2_approx(x2.x), ex2_approx(x2.y));
+      // every STREAMKL_FWD_POLY_EVERY-th column pair takes its two exps on the FMA/ALU pipes instead of MUFU
+      const bool poly = STREAMKL_FWD_POLY_EVERY > 0 && ((e >> 1) % (STREAMKL_FWD_POLY_EVERY > 0 ? STREAMKL_FWD_POLY_EVERY : 1)) == 0;
+      const float2 p1 = poly ? ex2_poly2(x1) : make_float2(ex2_approx(x1.x), ex2_approx(x1.y));
+      const float2 p2 = poly ? ex2_poly2(x2) : make_float2(ex2_approx(x2.x), ex2_approx(x2.y));
       const int a = (e >> 1) & 1;
       s1v[a] = add2(s1v[a], p1);
       s2v[a] = add2(s2v[a], p2);
@@ -241,19 +249,25 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
           tc_fence_after();
           const uint32_t dS1 = tmem_base + (mt * 2 + st) * 128;
           const uint32_t dS2 = dS1 + 64;
+          // Per-step descriptor bases, laundered through an empty asm so that the sixteen A descriptors are formed
+          // as base + immediate next to each MMA instead of being hoisted out of the loop (32 loop-invariant 64-bit
+          // values would not fit this warp's register budget: ptxas spilled them and the issue loop, not the tensor
+          // pipe, set the pace of the kernel).
+          uint64_t a1 = dq1 + uint64_t((mt * C::KB1 * C::QBLK) >> 4), a2 = dq2 + uint64_t((mt * C::KB2 * C::QBLK) >> 4), bk = dks;
+          asm volatile("" : "+l"(a1), "+l"(a2), "+l"(bk));
           if (elect_one()) {
 #pragma unroll
             for (int kb = 0; kb < C::KB1; ++kb)
 #pragma unroll
               for (int k = 0; k < 4; ++k)
-                umma_bf16_ss(dS1, dq1 + uint64_t(((mt * C::KB1 + kb) * C::QBLK + k * 32) >> 4),
-                             dks + uint64_t((kb * C::KBLK + k * 32) >> 4), idesc, (kb | k) != 0);
+                umma_bf16_ss(dS1, a1 + uint64_t((kb * C::QBLK + k * 32) >> 4), bk + uint64_t((kb * C::KBLK + k * 32) >> 4), idesc,
+                             (kb | k) != 0);
 #pragma unroll
             for (int kb = 0; kb < C::KB2; ++kb)
 #pragma unroll
               for (int k = 0; k < 4; ++k)
-                umma_bf16_ss(dS2, dq2 + uint64_t(((mt * C::KB2 + kb) * C::QBLK + k * 32) >> 4),
-                             dks + uint64_t(((C::KB1 + kb) * C::KBLK + k * 32) >> 4), idesc, (kb | k) != 0);
+                umma_bf16_ss(dS2, a2 + uint64_t((kb * C::QBLK + k * 32) >> 4),
+                             bk + uint64_t(((C::KB1 + kb) * C::KBLK + k * 32) >> 4), idesc, (kb | k) != 0);
             umma_commit(&s_full[mt * 2 + st]);
           }
           __syncwarp();
