@@ -290,6 +290,33 @@ def time_passes(skl, cfg, dev, steps, warmup, barrier):
             "outputs": (kl, l1, l2, grads), "workspace_bytes": need}
 
 
+def profiled_traffic(cfg: W.Config, name: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of kernel `name`, from the committed ncu --set full capture
+    (profiles/*_dram_traffic.csv, taken on cfg4).  None when no capture covers this kernel / workload."""
+    import csv
+    import glob
+
+    if cfg.idx != 4:
+        return None
+    best = None
+    for path in sorted(glob.glob(os.path.join(ROOT, "profiles", "*_dram_traffic.csv"))):
+        with open(path) as fh:
+            for row in csv.DictReader(fh):
+                if row["kernel"] == name:
+                    best = float(row["dram_bytes_read"]) + float(row["dram_bytes_write"])   # the latest capture wins
+    return best
+
+
+def kernel_hbm_bytes(cfg: W.Config, name: str) -> int:
+    """Compulsory HBM bytes of ONE launch: every input once + what the kernel writes."""
+    es = 2 if cfg.dtype == "bf16" else 4
+    gd = cfg.d2 + (cfg.d1 if cfg.teacher_grads else 0)
+    if "fwd" in name:
+        return input_bytes(cfg) - cfg.BH * cfg.NQ * 4 + 12 * cfg.BH * cfg.NQ
+    rows = cfg.NK if "OWNER_K" in name else cfg.NQ
+    return input_bytes(cfg) - cfg.BH * cfg.NQ * 4 + 16 * cfg.BH * cfg.NQ + cfg.BH * rows * gd * es
+
+
 def kernel_flops(cfg: W.Config, name: str) -> float:
     """Algorithmic tensor FLOPs ONE launch of kernel `name` performs ('Algorithmic work per kernel')."""
     pairs = cfg.visible_pairs_convention()
@@ -363,7 +390,9 @@ def main():
     peak_tf = float(pk["bf16_tflops_sustained"] if step_ms * args.steps > 1000.0 else pk["bf16_tflops"])
     ach = kernel_flops(cfg, dom_name) / (dom_stat["avg_ms"] * 1e-3) / 1e12
     roofline = {"bound": "tensor", "kernel": dom_name, "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
-                "traffic": None, "peak_source": f"{pk['_source']} bf16 "
+                "traffic": profiled_traffic(cfg, dom_name), "traffic_unit": "bytes/launch (ncu dram read+write)",
+                "algorithmic_hbm_bytes": kernel_hbm_bytes(cfg, dom_name),
+                "peak_source": f"{pk['_source']} bf16 "
                 + ("sustained" if step_ms * args.steps > 1000.0 else "burst") + " (MEASURED_PEAKS.json)",
                 "share_of_step": dom_stat["avg_ms"] * dom_stat["launches_per_step"] / res["step_ms"],
                 "avg_ms": dom_stat["avg_ms"]}
