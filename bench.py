@@ -77,11 +77,34 @@ def output_bytes(cfg: W.Config) -> int:
     return b
 
 
+def rank_heads(cfg: W.Config, rank: int):
+    """The (b,h) units of rank `rank`: every rank owns a whole batch of the config's shape, batch index offset by rank*B
+    (heads are independent: no unit is shared and no data-path collective is needed)."""
+    return [(rank * cfg.B + b, h) for b in range(cfg.B) for h in range(cfg.H)]
+
+
+def max_over_ranks(x: float, world: int, device="cuda") -> float:
+    """Timing of a multi-rank run = the slowest rank's device time (one scalar all-reduce, outside the timed region)."""
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_tflops(world: int, flop_per_rank: float, step_ms: float) -> float:
+    """Weak scaling: all ranks' work / max-over-ranks time."""
+    return world * flop_per_rank / (step_ms * 1e-3) / 1e12
+
+
 def gen_inputs(cfg: W.Config, rank: int):
     """Seeded host inputs of this rank's batch: batch index b is offset by rank*B so ranks hold different data."""
     from concurrent.futures import ThreadPoolExecutor
 
-    heads = [(rank * cfg.B + b, h) for b in range(cfg.B) for h in range(cfg.H)]
+    heads = rank_heads(cfg, rank)
     with ThreadPoolExecutor(max_workers=min(16, os.cpu_count() or 1)) as ex:
         per = list(ex.map(lambda bh: W.head_inputs(cfg, *bh), heads))
     out = {}
@@ -363,13 +386,6 @@ def main():
         if world > 1:
             dist.barrier()
 
-    def max_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
-
     pk = peaks()
     host = gen_inputs(cfg, rank)
     dev = tuple(to_dev(host[k]) for k in ("Q1", "K1", "Q2", "K2", "g"))
@@ -379,9 +395,9 @@ def main():
 
     with ClockSampler(local) as clk:
         res = time_passes(skl, cfg, dev, args.steps, args.warmup, barrier)
-    step_ms = max_over_ranks(res["step_ms"])
+    step_ms = max_over_ranks(res["step_ms"], world)
     flop_f, flop_b = cfg.fwd_flop(), cfg.bwd_flop()
-    value = world * (flop_f + flop_b) / (step_ms * 1e-3) / 1e12
+    value = whole_job_tflops(world, flop_f + flop_b, step_ms)
     extra_hbm = torch.cuda.max_memory_allocated() - base_mem
 
     # ---- roofline of the dominant kernel (largest share of the step), from the events recorded inside the timed region
@@ -450,9 +466,9 @@ def main():
         for _ in range(n_e2e):
             skl.streamkl_fwd_bwd_host(pins["Q1"], pins["K1"], pins["Q2"], pins["K2"], cfg.c1, cfg.c2, cfg.causal, pins["g"],
                                       teacher=cfg.teacher_grads, out=out)
-        e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3 / n_e2e)
+        e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1e3 / n_e2e, world)
         barrier()
-        e2e = {"value": world * (flop_f + flop_b) / (e2e_ms * 1e-3) / 1e12, "unit": UNIT, "ms_per_step": e2e_ms, "steps": n_e2e,
+        e2e = {"value": whole_job_tflops(world, flop_f + flop_b, e2e_ms), "unit": UNIT, "ms_per_step": e2e_ms, "steps": n_e2e,
                "h2d_bytes_per_step": input_bytes(cfg), "d2h_bytes_per_step": output_bytes(cfg),
                "api": "streamkl_fwd_bwd_host (pinned host buffers; cudaMalloc, H2D, fwd, bwd, D2H, cudaFree inside the call)",
                "check_mean_kl": float(out["kl"].mean())}
