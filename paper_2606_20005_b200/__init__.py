@@ -13,6 +13,9 @@ from .binding import (  # noqa: F401
     streamkl_fwd,
     streamkl_fwd_bwd_host,
     streamkl_fwd_host,
+    streamkl_fwd_splitk,
+    streamkl_fwd_splitk_splits,
+    streamkl_fwd_splitk_workspace_bytes,
     streamkl_kernel_name,
     streamkl_last_launch_count,
     streamkl_profile_collect,

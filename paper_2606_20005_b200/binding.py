@@ -14,6 +14,7 @@ from .build import LIB_PATH
 
 __all__ = [
     "StreamKLError", "lib", "lib_path", "streamkl_fwd", "streamkl_bwd", "streamkl_bwd_workspace_bytes",
+    "streamkl_fwd_splitk", "streamkl_fwd_splitk_splits", "streamkl_fwd_splitk_workspace_bytes",
     "streamkl_fwd_host", "streamkl_fwd_bwd_host", "streamkl_last_launch_count", "streamkl_strerror",
     "streamkl_profile_enable", "streamkl_profile_collect", "streamkl_kernel_name",
     "streamkl_version",
@@ -55,6 +56,12 @@ def lib() -> ctypes.CDLL:
         f = getattr(L, name)
         f.argtypes = [vp] * 4 + shape + [vp] * 4 + [vp] * 4 + [vp, sz, vp]
         f.restype = ci
+    L.streamkl_fwd_splitk.argtypes = [vp] * 4 + shape + [ci] + [vp] * 3 + [vp, sz, vp]
+    L.streamkl_fwd_splitk.restype = ci
+    L.streamkl_fwd_splitk_splits.argtypes = [ci] * 5
+    L.streamkl_fwd_splitk_splits.restype = ci
+    L.streamkl_fwd_splitk_workspace_bytes.argtypes = [ci] * 4
+    L.streamkl_fwd_splitk_workspace_bytes.restype = sz
     L.streamkl_bwd_workspace_bytes.argtypes = [ci] * 7
     L.streamkl_bwd_workspace_bytes.restype = sz
     L.streamkl_fwd_host.argtypes = [ci] + [vp] * 4 + shape + [vp] * 3 + [vp]
@@ -167,6 +174,41 @@ def streamkl_fwd(Q1, K1, Q2, K2, c1, c2, causal, kl_rows=None, lse1=None, lse2=N
                 _ptr(outs[0]), _ptr(outs[1]), _ptr(outs[2]), _stream_handle(stream))
     if rc != 0:
         raise StreamKLError(rc, "streamkl_fwd")
+    return tuple(outs)
+
+
+def streamkl_fwd_splitk_splits(B, H, NQ, NK, p_target=0) -> int:
+    return int(lib().streamkl_fwd_splitk_splits(B, H, NQ, NK, int(p_target)))
+
+
+def streamkl_fwd_splitk_workspace_bytes(B, H, NQ, splits) -> int:
+    return int(lib().streamkl_fwd_splitk_workspace_bytes(B, H, NQ, int(splits)))
+
+
+def streamkl_fwd_splitk(Q1, K1, Q2, K2, c1, c2, causal, splits=0, kl_rows=None, lse1=None, lse2=None, workspace=None, stream=None):
+    """Split-K forward for small NQ (bf16).  splits <= 0: adaptive.  Returns (kl_rows, lse1, lse2)."""
+    import torch
+
+    for n, t in (("Q1", Q1), ("K1", K1), ("Q2", Q2), ("K2", K2)):
+        _check_dev(n, t, torch.bfloat16)
+    B, H, NQ, NK, d1, d2 = _shape_of(Q1, K1, Q2, K2)
+    outs = []
+    for n, t in (("kl_rows", kl_rows), ("lse1", lse1), ("lse2", lse2)):
+        if t is None:
+            t = torch.empty((B, H, NQ), dtype=torch.float32, device=Q1.device)
+        _check_dev(n, t, torch.float32)
+        outs.append(t)
+    w = int(splits) if splits > 0 else streamkl_fwd_splitk_splits(B, H, NQ, NK, 0)
+    need = streamkl_fwd_splitk_workspace_bytes(B, H, NQ, w)
+    if need > 0 and (workspace is None or workspace.numel() * workspace.element_size() < need):
+        workspace = torch.empty(need, dtype=torch.uint8, device=Q1.device)
+    ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    with torch.cuda.device(Q1.device):
+        rc = lib().streamkl_fwd_splitk(_ptr(Q1), _ptr(K1), _ptr(Q2), _ptr(K2), B, H, NQ, NK, d1, d2, float(c1), float(c2),
+                                       int(bool(causal)), w, _ptr(outs[0]), _ptr(outs[1]), _ptr(outs[2]), _ptr(workspace),
+                                       ctypes.c_size_t(ws_bytes), _stream_handle(stream))
+    if rc != 0:
+        raise StreamKLError(rc, "streamkl_fwd_splitk")
     return tuple(outs)
 
 

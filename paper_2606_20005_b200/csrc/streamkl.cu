@@ -19,11 +19,12 @@ namespace {
 thread_local int g_last_launches = 0;
 
 // ---- optional per-kernel timing (streamkl_profile_*): CUDA events recorded on the launch stream around every kernel
-enum KernelId { KID_FWD_TC = 0, KID_BWD_DQ_TC, KID_BWD_DK_TC, KID_FWD_SIMT, KID_BWD_DQ_SIMT, KID_BWD_DK_SIMT, KID_BWD_STATS, KID_COUNT };
+enum KernelId { KID_FWD_TC = 0, KID_BWD_DQ_TC, KID_BWD_DK_TC, KID_FWD_SIMT, KID_BWD_DQ_SIMT, KID_BWD_DK_SIMT, KID_BWD_STATS, KID_FWD_SPLITK_TC, KID_FWD_SPLITK_REDUCE, KID_COUNT };
 const char* const kKernelNames[KID_COUNT] = {"streamkl_fwd_sm100_kernel", "streamkl_bwd_sm100_kernel<OWNER_Q>",
                                              "streamkl_bwd_sm100_kernel<OWNER_K>", "streamkl_fwd_simt_kernel",
                                              "streamkl_bwd_simt_kernel<OWNER_Q>", "streamkl_bwd_simt_kernel<OWNER_K>",
-                                             "streamkl_bwd_stats_kernel"};
+                                             "streamkl_bwd_stats_kernel", "streamkl_fwd_sm100_kernel<SPLIT>",
+                                             "streamkl_fwd_splitk_reduce_kernel"};
 struct ProfRecord { int id; cudaEvent_t a, b; };
 thread_local bool g_prof_on = false;
 thread_local std::vector<ProfRecord>* g_prof = nullptr;
@@ -101,15 +102,17 @@ bool tc_shape(int dtype, const Shape& s) {
 }
 
 // ----------------------------------------------------------------------------------------- forward launchers
-template <int D1, int D2, bool CAUSAL>
+// splits == 1: the default kernel (grid (bsz, T_Q)).  splits > 1: split-K (grid (bsz, T_Q, W), partial
+// statistics to `part`, then the reduce kernel).
+template <int D1, int D2, bool CAUSAL, bool SPLIT = false>
 int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, float* kl, float* lse1, float* lse2,
-                  cudaStream_t stream) {
+                  cudaStream_t stream, int splits = 1, float* part = nullptr) {
   using C = skl::FwdCfg<D1, D2>;
   CUtensorMap tQ1, tK1, tQ2, tK2;
   if (!make_tmap_bf16(&tQ1, Q1, int(s.BH), s.NQ, D1, C::BM) || !make_tmap_bf16(&tK1, K1, int(s.BH), s.NK, D1, C::BK) ||
       !make_tmap_bf16(&tQ2, Q2, int(s.BH), s.NQ, D2, C::BM) || !make_tmap_bf16(&tK2, K2, int(s.BH), s.NK, D2, C::BK))
     return STREAMKL_ERR_CUDA;
-  auto kern = skl::streamkl_fwd_sm100_kernel<D1, D2, CAUSAL>;
+  auto kern = skl::streamkl_fwd_sm100_kernel<D1, D2, CAUSAL, SPLIT>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
     cudaGetLastError();
     return STREAMKL_ERR_CUDA;
@@ -120,14 +123,27 @@ int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2
   p.sc1 = s.c1 * 1.4426950408889634f;
   p.sc2 = s.c2 * 1.4426950408889634f;
   p.kl = kl; p.lse1 = lse1; p.lse2 = lse2;
-  const long long grid = (long long)p.TQ * s.BH;
+  const int TK = (s.NK + C::BK - 1) / C::BK;
+  p.chunk_steps = SPLIT ? (TK + splits - 1) / splits : TK;       // C_K = ceil(N_K / W), in whole 64-key steps
+  p.W = SPLIT ? (TK + p.chunk_steps - 1) / p.chunk_steps : 1;    // no empty trailing chunk
+  p.part = part;
+  const long long grid = (long long)p.TQ * s.BH * p.W;
   if (grid > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
   {
-    ProfScope ps(KID_FWD_TC, stream);
+    ProfScope ps(SPLIT ? KID_FWD_SPLITK_TC : KID_FWD_TC, stream);
     kern<<<dim3((unsigned)grid), C::THREADS, C::SMEM_BYTES, stream>>>(tQ1, tK1, tQ2, tK2, p);
   }
   if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
   g_last_launches += 1;
+  if (SPLIT) {
+    const long long rows = s.BH * (long long)s.NQ;
+    {
+      ProfScope ps(KID_FWD_SPLITK_REDUCE, stream);
+      skl::streamkl_fwd_splitk_reduce_kernel<<<dim3((unsigned)((rows + 127) / 128)), 128, 0, stream>>>(part, s.NQ, p.W, rows, kl, lse1, lse2);
+    }
+    if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
+    g_last_launches += 1;
+  }
   return STREAMKL_OK;
 }
 
@@ -163,7 +179,8 @@ int launch_fwd_simt(const void* Q1, const void* K1, const void* Q2, const void* 
 }
 
 int fwd_dispatch(int dtype, const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1,
-                 int d2, float c1, float c2, int causal, float* kl, float* lse1, float* lse2, cudaStream_t stream) {
+                 int d2, float c1, float c2, int causal, float* kl, float* lse1, float* lse2, cudaStream_t stream, int splits = 1,
+                 float* part = nullptr) {
   Shape s{B, H, NQ, NK, d1, d2, causal ? 1 : 0, c1, c2, (long long)B * (long long)H};
   int rc = validate_common(Q1, K1, Q2, K2, s);
   if (rc != STREAMKL_OK) return rc;
@@ -174,9 +191,13 @@ int fwd_dispatch(int dtype, const void* Q1, const void* K1, const void* Q2, cons
   if (s.BH > 65535) return STREAMKL_ERR_SHAPE;
   if (tc_shape(dtype, s)) {
 #define SKL_FWD_CASE(A, Bd)                                                                                                  \
-  if (d1 == A && d2 == Bd)                                                                                                   \
+  if (d1 == A && d2 == Bd) {                                                                                                 \
+    if (splits > 1)                                                                                                          \
+      return s.causal ? launch_fwd_tc<A, Bd, true, true>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream, splits, part)            \
+                      : launch_fwd_tc<A, Bd, false, true>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream, splits, part);          \
     return s.causal ? launch_fwd_tc<A, Bd, true>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream)                                  \
-                    : launch_fwd_tc<A, Bd, false>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream);
+                    : launch_fwd_tc<A, Bd, false>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream);                                \
+  }
     SKL_FWD_CASE(128, 128)
     SKL_FWD_CASE(128, 64)
     SKL_FWD_CASE(64, 128)
@@ -350,6 +371,39 @@ int streamkl_bwd_f32(const void* Q1, const void* K1, const void* Q2, const void*
                      streamkl_stream_t stream) {
   return bwd_dispatch(STREAMKL_F32, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2, dkl_rows, dQ1, dK1,
                       dQ2, dK2, workspace, workspace_bytes, static_cast<cudaStream_t>(stream));
+}
+
+int streamkl_fwd_splitk_splits(int B, int H, int NQ, int NK, int p_target) {
+  // adaptive split selection: P_base = bsz * T_Q; W = 1 if P_base >= P_target, else min(floor(P_target / P_base), T_K)
+  if (B <= 0 || H <= 0 || NQ <= 0 || NK <= 0) return 1;
+  if (p_target <= 0) p_target = 2 * 148;   // two CTAs' worth of work per SM of a B200 (one resident CTA per SM)
+  const long long p_base = (long long)B * H * ((NQ + 255) / 256);
+  const long long tk = (NK + 63) / 64;
+  if (p_base >= p_target) return 1;
+  const long long w = p_target / p_base;
+  return int(w < tk ? w : tk);
+}
+
+size_t streamkl_fwd_splitk_workspace_bytes(int B, int H, int NQ, int splits) {
+  if (B <= 0 || H <= 0 || NQ <= 0 || splits <= 1) return 0;
+  return size_t(B) * size_t(H) * size_t(splits) * 5 * size_t(NQ) * sizeof(float);
+}
+
+int streamkl_fwd_splitk(const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1, int d2,
+                        float c1, float c2, int causal, int splits, float* kl_rows, float* lse1, float* lse2, void* workspace,
+                        size_t workspace_bytes, streamkl_stream_t stream) {
+  if (splits <= 0) splits = streamkl_fwd_splitk_splits(B, H, NQ, NK, 0);
+  const int tk = NK > 0 ? (NK + 63) / 64 : 1;
+  if (splits > tk) splits = tk;
+  const bool tc = (d1 == 64 || d1 == 128) && (d2 == 64 || d2 == 128);
+  if (!tc || splits <= 1)   // other head dims run the (unsplit) SIMT kernel; W = 1 is the default kernel
+    return fwd_dispatch(STREAMKL_BF16, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
+                        static_cast<cudaStream_t>(stream));
+  const size_t need = streamkl_fwd_splitk_workspace_bytes(B, H, NQ, splits);
+  if (need > 0 && (!workspace || workspace_bytes < need)) return STREAMKL_ERR_WORKSPACE;
+  if (reinterpret_cast<uintptr_t>(workspace) & 15) return STREAMKL_ERR_ALIGN;
+  return fwd_dispatch(STREAMKL_BF16, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
+                      static_cast<cudaStream_t>(stream), splits, static_cast<float*>(workspace));
 }
 
 size_t streamkl_bwd_workspace_bytes(int B, int H, int NQ, int, int d1, int d2, int) {

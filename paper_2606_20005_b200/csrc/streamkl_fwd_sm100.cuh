@@ -58,6 +58,10 @@ struct FwdParams {
   float* kl;
   float* lse1;
   float* lse2;
+  // split-K: W contiguous key chunks of `chunk_steps` 64-key steps each; partial statistics
+  // (m1,l1,m2,l2,acc in the log2 domain) go to part[bh][w][5][NQ] and streamkl_fwd_splitk_reduce_kernel merges them
+  int W, chunk_steps;
+  float* part;
 };
 
 // Online update for NC keys of one query row (thread-local).  Implements Alg.1 lines 8-12 with
@@ -141,7 +145,7 @@ __device__ __forceinline__ void online_update(RowState& st, const uint32_t (&r1)
   st.m2 = m2n;
 }
 
-template <int D1, int D2, bool CAUSAL>
+template <int D1, int D2, bool CAUSAL, bool SPLIT = false>
 __global__ void __launch_bounds__(FwdCfg<D1, D2>::THREADS, 1)
 streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid_constant__ CUtensorMap tmK1,
                           const __grid_constant__ CUtensorMap tmQ2, const __grid_constant__ CUtensorMap tmK2, const FwdParams p) {
@@ -161,22 +165,26 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   // heavy (late, causal) query tiles first within each head; consecutive CTAs share a head (K stays in L2)
-  const int bh = blockIdx.x / p.TQ;
-  const int qt = p.TQ - 1 - (blockIdx.x % p.TQ);
+  const int tile = SPLIT ? int(blockIdx.x) / p.W : int(blockIdx.x);
+  const int wk = SPLIT ? int(blockIdx.x) % p.W : 0;          // key chunk of this CTA (split-K grid (b, i, w))
+  const int bh = tile / p.TQ;
+  const int qt = p.TQ - 1 - (tile % p.TQ);
   const int q0 = qt * C::BQ;
   const int off = p.NK - p.NQ;
   const int TK = (p.NK + C::BK - 1) / C::BK;
+  const int j_begin = SPLIT ? wk * p.chunk_steps : 0;        // this CTA's 64-key steps are [j_begin, j_begin + nsteps_mt)
+  const int j_end = SPLIT ? min(TK, j_begin + p.chunk_steps) : TK;
 
   int nsteps_mt[2];
 #pragma unroll
   for (int mt = 0; mt < 2; ++mt) {
     const int r0 = q0 + mt * C::BM;
-    int n = TK;
+    int n = j_end;
     if (CAUSAL) {
       const int lastkey = min(p.NK - 1, r0 + C::BM - 1 + off);
-      n = lastkey / C::BK + 1;
+      n = min(j_end, lastkey / C::BK + 1);
     }
-    nsteps_mt[mt] = (r0 < p.NQ) ? n : 0;
+    nsteps_mt[mt] = (r0 < p.NQ) ? max(0, n - j_begin) : 0;
   }
   const int nsteps = max(nsteps_mt[0], nsteps_mt[1]);
 
@@ -218,10 +226,11 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
         mbar_arrive_expect_tx(&k_full[s], C::STAGE_BYTES);
         uint8_t* st = sK + s * C::STAGE_BYTES;
 #pragma unroll
-        for (int kb = 0; kb < C::KB1; ++kb) tma_load_3d_hint(st + kb * C::KBLK, &tmK1, &k_full[s], kb * 64, j * C::BK, bh, pol_k);
+        for (int kb = 0; kb < C::KB1; ++kb)
+          tma_load_3d_hint(st + kb * C::KBLK, &tmK1, &k_full[s], kb * 64, (j_begin + j) * C::BK, bh, pol_k);
 #pragma unroll
         for (int kb = 0; kb < C::KB2; ++kb)
-          tma_load_3d_hint(st + (C::KB1 + kb) * C::KBLK, &tmK2, &k_full[s], kb * 64, j * C::BK, bh, pol_k);
+          tma_load_3d_hint(st + (C::KB1 + kb) * C::KBLK, &tmK2, &k_full[s], kb * 64, (j_begin + j) * C::BK, bh, pol_k);
       }
     }
   } else if (warp == 1) {
@@ -303,7 +312,7 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(&s_empty[mt * 2 + sg]);  // logits are in registers: MMA may refill this stage
-      const int kbase = j * C::BK + half * C::BC;
+      const int kbase = (j_begin + j) * C::BK + half * C::BC;
       const bool masked = (CAUSAL && (kbase + C::BC - 1 > first_row_limit)) || (kbase + C::BC > p.NK);
       if (masked) online_update<true, C::BC>(st, r1, r2, p.sc1, p.sc2, kbase, limit);
       else        online_update<false, C::BC>(st, r1, r2, p.sc1, p.sc2, kbase, limit);
@@ -320,9 +329,16 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
       if (half == 0 && row < p.NQ) {
         const float m1b = xch[0 * C::BM + rloc], l1b = xch[1 * C::BM + rloc], m2b = xch[2 * C::BM + rloc];
         const float l2b = xch[3 * C::BM + rloc], accb = xch[4 * C::BM + rloc];
-        const float m1 = fmaxf(st.m1, m1b), m2 = fmaxf(st.m2, m2b);   // half 0 holds key 0: its maxima are finite
-        const float wa1 = exp2f(st.m1 - m1), wb1 = exp2f(m1b - m1), wa2 = exp2f(st.m2 - m2), wb2 = exp2f(m2b - m2);
+        const float m1 = fmaxf(st.m1, m1b), m2 = fmaxf(st.m2, m2b);
+        // unsplit: half 0 holds key 0, so the maxima are finite.  A split-K chunk can lie wholly past a row's causal
+        // frontier: both halves are then (-inf, 0, 0) and the reference is 0 (R7), giving the identity partial.
+        const float r1 = (SPLIT && m1 == -CUDART_INF_F) ? 0.f : m1, r2 = (SPLIT && m2 == -CUDART_INF_F) ? 0.f : m2;
+        const float wa1 = exp2f(st.m1 - r1), wb1 = exp2f(m1b - r1), wa2 = exp2f(st.m2 - r2), wb2 = exp2f(m2b - r2);
         const float l1 = st.l1 * wa1 + l1b * wb1, l2 = st.l2 * wa2 + l2b * wb2, acc = st.acc * wa1 + accb * wb1;
+        if constexpr (SPLIT) {   // partial statistics of this key chunk (log2 domain), merged by the reduce kernel
+          float* o = p.part + (size_t(bh) * p.W + wk) * 5 * size_t(p.NQ) + row;
+          o[0] = m1; o[size_t(p.NQ)] = l1; o[2 * size_t(p.NQ)] = m2; o[3 * size_t(p.NQ)] = l2; o[4 * size_t(p.NQ)] = acc;
+        } else {
         // Alg.1 lines 13-15 in natural-log units (R6): LSE = ln2*(m + log2 l); KL = ln2*acc/l1 + LSE2 - LSE1
         const float LN2 = 0.6931471805599453f;
         const float e1 = LN2 * (m1 + log2f(l1));
@@ -331,7 +347,12 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
         p.lse1[o] = e1;
         p.lse2[o] = e2;
         p.kl[o] = fmaf(LN2, acc / l1, e2 - e1);
+        }
       }
+    } else if (SPLIT && half == 0 && row < p.NQ) {   // no step of this chunk is visible to this M-tile: identity partial
+      float* o = p.part + (size_t(bh) * p.W + wk) * 5 * size_t(p.NQ) + row;
+      o[0] = -CUDART_INF_F; o[size_t(p.NQ)] = 0.f; o[2 * size_t(p.NQ)] = -CUDART_INF_F; o[3 * size_t(p.NQ)] = 0.f;
+      o[4 * size_t(p.NQ)] = 0.f;
     }
   }
   tc_fence_before();
@@ -340,6 +361,31 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
     tc_fence_after();
     tmem_dealloc<C::TMEM_COLS>(tmem_base);
   }
+}
+
+// Split-K reduce (Eq.11; (m2,l2) merged the same way, R11): one thread per query row folds the W
+// partials in chunk order and finishes Alg.1 lines 13-15.  Chunk 0 always sees key 0, so the merged maxima are finite.
+__global__ void streamkl_fwd_splitk_reduce_kernel(const float* __restrict__ part, int NQ, int W, long long total_rows,
+                                                  float* __restrict__ kl, float* __restrict__ lse1, float* __restrict__ lse2) {
+  const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= total_rows) return;
+  const long long bh = idx / NQ;
+  const int row = int(idx % NQ);
+  const float* b = part + size_t(bh) * W * 5 * size_t(NQ) + row;
+  float m1 = b[0], l1 = b[size_t(NQ)], m2 = b[2 * size_t(NQ)], l2 = b[3 * size_t(NQ)], acc = b[4 * size_t(NQ)];
+  for (int w = 1; w < W; ++w) {
+    const float* c = b + size_t(w) * 5 * size_t(NQ);
+    const float m1b = c[0], l1b = c[size_t(NQ)], m2b = c[2 * size_t(NQ)], l2b = c[3 * size_t(NQ)], accb = c[4 * size_t(NQ)];
+    const float n1 = fmaxf(m1, m1b), n2 = fmaxf(m2, m2b);
+    const float wa1 = exp2f(m1 - n1), wb1 = exp2f(m1b - n1), wa2 = exp2f(m2 - n2), wb2 = exp2f(m2b - n2);
+    l1 = l1 * wa1 + l1b * wb1; acc = acc * wa1 + accb * wb1; l2 = l2 * wa2 + l2b * wb2;
+    m1 = n1; m2 = n2;
+  }
+  const float LN2 = 0.6931471805599453f;
+  const float e1 = LN2 * (m1 + log2f(l1)), e2 = LN2 * (m2 + log2f(l2));
+  lse1[idx] = e1;
+  lse2[idx] = e2;
+  kl[idx] = fmaf(LN2, acc / l1, e2 - e1);
 }
 
 }  // namespace skl

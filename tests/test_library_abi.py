@@ -102,3 +102,36 @@ def test_workspace_is_never_quadratic(L):
     small = L.streamkl_bwd_workspace_bytes(1, 32, 4096, 4096, 128, 128, 1)
     big = L.streamkl_bwd_workspace_bytes(1, 32, 65536, 65536, 128, 128, 1)
     assert big <= 16 * max(small, 1) + 4 * 32 * 65536 * 256 * 4  # O((NQ+NK) d), not O(NQ NK)
+
+
+def test_bwd_workspace_is_16_bytes_per_padded_query(L):
+    assert L.streamkl_bwd_workspace_bytes(1, 32, 65536, 65536, 128, 128, 1) == 32 * 65536 * 16
+    assert L.streamkl_bwd_workspace_bytes(2, 3, 100, 777, 128, 64, 0) == 6 * 128 * 16      # rows padded to 64 per head
+    assert L.streamkl_bwd_workspace_bytes(1, 1, 256, 256, 48, 80, 0) == 0                  # SIMT path: no workspace
+
+
+def test_splitk_adaptive_split_selection_follows_the_paper_rule(L):
+    """PAPER.md:249: W = 1 if P_base >= P_target else min(floor(P_target / P_base), T_K); P_base = bsz * T_Q."""
+    f = L.streamkl_fwd_splitk_splits
+    assert f(1, 16, 1, 131072, 256) == 16            # P_base = 16 -> floor(256/16)
+    assert f(1, 16, 64, 131072, 128) == 8
+    assert f(4, 64, 16, 131072, 256) == 1            # P_base = 256 >= P_target: default kernel
+    assert f(1, 1, 1, 200, 256) == 4                 # clamped by T_K = ceil(200/64)
+    assert f(1, 16, 300, 8192, 256) == 8             # T_Q = ceil(300/256) = 2 -> P_base = 32
+    assert f(1, 16, 16, 65536, 0) == 18              # default target 2 x 148 SMs
+    assert f(0, 16, 16, 65536, 0) == 1
+
+
+def test_splitk_workspace_and_argument_checks(L):
+    vp = ctypes.c_void_p
+    assert L.streamkl_fwd_splitk_workspace_bytes(1, 16, 32, 8) == 16 * 8 * 5 * 32 * 4
+    assert L.streamkl_fwd_splitk_workspace_bytes(1, 16, 32, 1) == 0
+
+    def call(ws, ws_bytes, splits=8, d1=128, NK=4096):
+        return L.streamkl_fwd_splitk(vp(16), vp(16), vp(16), vp(16), 1, 16, 32, NK, d1, 128, 0.1, 0.1, 0, splits,
+                                     vp(16), vp(16), vp(16), vp(ws), ctypes.c_size_t(ws_bytes), vp(0))
+
+    assert call(0, 0) == -5                                   # STREAMKL_ERR_WORKSPACE
+    assert call(16, 100) == -5
+    assert call(24, 1 << 20) == -3                            # misaligned workspace
+    assert call(16, 1 << 20, NK=0) in (-2, -5)                # shape errors are still reported
