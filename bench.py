@@ -330,6 +330,41 @@ def profiled_traffic(cfg: W.Config, name: str):
     return best
 
 
+SPLITK_SHAPE = dict(B=1, H=16, NQ=16, NK=131072, d1=128, d2=128)   # the paper's split-K ablation regime (bsz 16, small N_Q)
+
+
+def time_splitk(skl, iters: int = 30):
+    """Split-K forward on a decode-like shape, against the default kernel; HBM roofline (K is read once)."""
+    import torch
+
+    sh = SPLITK_SHAPE
+    cfg = W.Config(70, "splitk", sh["B"], sh["H"], sh["NQ"], sh["NK"], sh["d1"], sh["d2"], "bf16", False)
+    inp = W.all_inputs(cfg)
+    Q1, K1, Q2, K2 = (to_dev(inp[k]) for k in ("Q1", "K1", "Q2", "K2"))
+    w = skl.streamkl_fwd_splitk_splits(cfg.B, cfg.H, cfg.NQ, cfg.NK)
+    ws = torch.empty(max(1, skl.streamkl_fwd_splitk_workspace_bytes(cfg.B, cfg.H, cfg.NQ, w)), dtype=torch.uint8, device="cuda")
+    outs = skl.streamkl_fwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, False)
+
+    def timed(fn):
+        for _ in range(3):
+            fn()
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(iters):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / iters
+
+    ms_split = timed(lambda: skl.streamkl_fwd_splitk(Q1, K1, Q2, K2, cfg.c1, cfg.c2, False, w, *outs, workspace=ws))
+    ms_default = timed(lambda: skl.streamkl_fwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, False, *outs))
+    bytes_alg = input_bytes(cfg) - cfg.BH * cfg.NQ * 4 + 12 * cfg.BH * cfg.NQ
+    return {"shape": sh, "splits": w, "ms": ms_split, "default_kernel_ms": ms_default, "speedup_over_default": ms_default / ms_split,
+            "tflops": cfg.fwd_flop() / (ms_split * 1e-3) / 1e12, "algorithmic_hbm_bytes": bytes_alg,
+            "hbm_gbs": bytes_alg / (ms_split * 1e-3) / 1e9, "l2": "inputs (1.07 GB) larger than L2, no flush"}
+
+
 def kernel_hbm_bytes(cfg: W.Config, name: str) -> int:
     """Compulsory HBM bytes of ONE launch: every input once + what the kernel writes."""
     es = 2 if cfg.dtype == "bf16" else 4
@@ -436,6 +471,10 @@ def main():
             "bwd_tflops": c3.bwd_flop() / (r3["bwd_ms"] * 1e-3) / 1e12,
             "fwd_frac_of_measured_bf16_burst": c3.fwd_flop() / (r3["fwd_ms"] * 1e-3) / 1e12 / float(pk["bf16_tflops"])}
         del d3, h3, r3
+        sk = time_splitk(skl)
+        sk["roofline"] = {"bound": "hbm", "achieved": sk["hbm_gbs"], "peak": float(pk["hbm_gbs"]), "unit": "GB/s",
+                          "frac": sk["hbm_gbs"] / float(pk["hbm_gbs"])}
+        also["split-K forward (bsz=16, NQ=16, NK=131072, d=128/128, no mask)"] = sk
 
     # ---- e2e: host buffers through streamkl_fwd_bwd_host (copies inside the timed region)
     e2e = None

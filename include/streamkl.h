@@ -85,8 +85,8 @@ int streamkl_fwd_splitk(const void* Q1, const void* K1, const void* Q2, const vo
                         float* kl_rows, float* lse1, float* lse2,
                         void* workspace, size_t workspace_bytes, streamkl_stream_t stream);
 /* Adaptive split selection, pure host arithmetic: P_base = B*H*ceil(NQ/256) CTAs of the default kernel;
- * returns 1 if P_base >= p_target, else min(floor(p_target/P_base), ceil(NK/64)).  p_target <= 0 means 296 = 2 x the
- * 148 SMs of a B200 (the paper's "typically 128 or 256" was for 108/132-SM parts). */
+ * returns 1 if P_base >= p_target, else min(floor(p_target/P_base), ceil(NK/64)).  p_target <= 0 means 148 = one CTA
+ * per SM of a B200, i.e. one full wave (the paper's "typically 128 or 256" was for 108/132-SM parts). */
 int streamkl_fwd_splitk_splits(int B, int H, int NQ, int NK, int p_target);
 /* B*H*splits*5*NQ floats; 0 when splits <= 1. */
 size_t streamkl_fwd_splitk_workspace_bytes(int B, int H, int NQ, int splits);

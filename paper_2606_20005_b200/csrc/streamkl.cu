@@ -376,7 +376,7 @@ int streamkl_bwd_f32(const void* Q1, const void* K1, const void* Q2, const void*
 int streamkl_fwd_splitk_splits(int B, int H, int NQ, int NK, int p_target) {
   // adaptive split selection: P_base = bsz * T_Q; W = 1 if P_base >= P_target, else min(floor(P_target / P_base), T_K)
   if (B <= 0 || H <= 0 || NQ <= 0 || NK <= 0) return 1;
-  if (p_target <= 0) p_target = 2 * 148;   // two CTAs' worth of work per SM of a B200 (one resident CTA per SM)
+  if (p_target <= 0) p_target = 148;   // one CTA per SM of a B200 = one full wave (measured best: profiles/r01d_splitk.md)
   const long long p_base = (long long)B * H * ((NQ + 255) / 256);
   const long long tk = (NK + 63) / 64;
   if (p_base >= p_target) return 1;
