@@ -509,7 +509,7 @@ def main():
         barrier()
         e2e = {"value": whole_job_tflops(world, flop_f + flop_b, e2e_ms), "unit": UNIT, "ms_per_step": e2e_ms, "steps": n_e2e,
                "h2d_bytes_per_step": input_bytes(cfg), "d2h_bytes_per_step": output_bytes(cfg),
-               "api": "streamkl_fwd_bwd_host (pinned host buffers; cudaMalloc, H2D, fwd, bwd, D2H, cudaFree inside the call)",
+               "api": "streamkl_fwd_bwd_host (pinned host buffers; pooled device scratch, H2D, fwd, bwd, D2H inside the call, head groups pipelined over three streams)",
                "check_mean_kl": float(out["kl"].mean())}
 
     # ---- cpu baseline: the oracle as it stands, bounded sample, rank 0 at N=1 only

@@ -116,8 +116,9 @@ size_t streamkl_bwd_workspace_bytes(int B, int H, int NQ, int NK, int d1, int d2
 
 /*
  * End-to-end variants with HOST buffers (same argument meaning; `dtype` = STREAMKL_BF16 | STREAMKL_F32).
- * They cudaMalloc scratch for inputs/outputs, copy host->device, run the kernels above, copy device->host,
- * free, and synchronise `stream` before returning.  Host buffers may be pageable or pinned.
+ * They take device scratch for inputs/outputs from the stream-ordered pool, copy host->device, run the kernels above,
+ * copy device->host, and synchronise `stream` before returning.  Host buffers may be pageable or pinned (pinned
+ * buffers are what lets the copies overlap the kernels).
  * streamkl_fwd_bwd_host runs forward then backward on the same resident inputs (one "step" of the hot path);
  * pass dQ1 = dK1 = NULL for Setting 1 only.
  */
@@ -128,6 +129,15 @@ int streamkl_fwd_bwd_host(int dtype, const void* Q1, const void* K1, const void*
                           int B, int H, int NQ, int NK, int d1, int d2, float c1, float c2, int causal,
                           const float* dkl_rows, float* kl_rows, float* lse1, float* lse2,
                           void* dQ1, void* dK1, void* dQ2, void* dK2, streamkl_stream_t stream);
+
+/*
+ * The *_host entry points cut the batch into groups of whole heads (heads are independent) and overlap the upload of
+ * one group and the download of another with the kernels of a third on internal streams; results are bit-identical to
+ * one ungrouped call.  Their device scratch comes from the device's stream-ordered memory pool and stays cached there
+ * between calls (no cudaMalloc/cudaFree per call); streamkl_host_trim() synchronises the device and returns that cached
+ * memory to the driver.
+ */
+int streamkl_host_trim(void);
 
 /* Number of kernels the last successful streamkl_* call on this thread launched (for launch accounting). */
 int streamkl_last_launch_count(void);

@@ -14,6 +14,7 @@ from .binding import (  # noqa: F401
     streamkl_fwd_bwd_host,
     streamkl_fwd_host,
     streamkl_fwd_splitk,
+    streamkl_host_trim,
     streamkl_fwd_splitk_splits,
     streamkl_fwd_splitk_workspace_bytes,
     streamkl_kernel_name,

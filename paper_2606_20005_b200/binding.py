@@ -15,7 +15,7 @@ from .build import LIB_PATH
 __all__ = [
     "StreamKLError", "lib", "lib_path", "streamkl_fwd", "streamkl_bwd", "streamkl_bwd_workspace_bytes",
     "streamkl_fwd_splitk", "streamkl_fwd_splitk_splits", "streamkl_fwd_splitk_workspace_bytes",
-    "streamkl_fwd_host", "streamkl_fwd_bwd_host", "streamkl_last_launch_count", "streamkl_strerror",
+    "streamkl_fwd_host", "streamkl_fwd_bwd_host", "streamkl_host_trim", "streamkl_last_launch_count", "streamkl_strerror",
     "streamkl_profile_enable", "streamkl_profile_collect", "streamkl_kernel_name",
     "streamkl_version",
 ]
@@ -68,6 +68,8 @@ def lib() -> ctypes.CDLL:
     L.streamkl_fwd_host.restype = ci
     L.streamkl_fwd_bwd_host.argtypes = [ci] + [vp] * 4 + shape + [vp] + [vp] * 3 + [vp] * 4 + [vp]
     L.streamkl_fwd_bwd_host.restype = ci
+    L.streamkl_host_trim.argtypes = []
+    L.streamkl_host_trim.restype = ci
     L.streamkl_last_launch_count.argtypes = []
     L.streamkl_last_launch_count.restype = ci
     L.streamkl_profile_enable.argtypes = [ci]
@@ -90,6 +92,12 @@ def streamkl_strerror(code: int) -> str:
 
 def streamkl_version() -> str:
     return lib().streamkl_version().decode()
+
+
+def streamkl_host_trim() -> None:
+    rc = lib().streamkl_host_trim()
+    if rc != 0:
+        raise StreamKLError(rc, "streamkl_host_trim")
 
 
 def streamkl_last_launch_count() -> int:

@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <cuda_bf16.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdint>
 #include <cstring>
@@ -338,12 +339,50 @@ int bwd_dispatch(int dtype, const void* Q1, const void* K1, const void* Q2, cons
   return STREAMKL_ERR_DTYPE;
 }
 
-// RAII device scratch for the *_host entry points
-struct DevBuf {
-  void* p = nullptr;
-  ~DevBuf() { if (p) cudaFree(p); }
-  bool alloc(size_t n) { return n == 0 || cudaMalloc(&p, n) == cudaSuccess; }
+// Device scratch of the *_host entry points, taken from the device's stream-ordered pool.  The pool keeps freed blocks
+// (release threshold = max), so a host call after the first one pays no cudaMalloc / cudaFree; streamkl_host_trim()
+// hands the memory back to the driver.
+struct AsyncScratch {
+  cudaStream_t st;
+  std::vector<void*> ptrs;
+  bool ok = true;
+  explicit AsyncScratch(cudaStream_t s) : st(s) {
+    int dev = 0;
+    cudaMemPool_t pool;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+      unsigned long long thr = ~0ull;
+      cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+    }
+    cudaGetLastError();
+  }
+  void* get(size_t n) {
+    if (n == 0) return nullptr;
+    void* p = nullptr;
+    if (cudaMallocAsync(&p, n, st) != cudaSuccess) { cudaGetLastError(); ok = false; return nullptr; }
+    ptrs.push_back(p);
+    return p;
+  }
+  ~AsyncScratch() {
+    for (void* p : ptrs) cudaFreeAsync(p, st);
+    cudaStreamSynchronize(st);
+  }
 };
+
+// Two helper streams per host thread: uploads and downloads of one head group overlap the kernels of another.
+struct HostStreams {
+  cudaStream_t in = nullptr, out = nullptr, cmp = nullptr;
+  bool ok = false;
+  HostStreams() {
+    ok = cudaStreamCreateWithFlags(&in, cudaStreamNonBlocking) == cudaSuccess &&
+         cudaStreamCreateWithFlags(&out, cudaStreamNonBlocking) == cudaSuccess &&
+         cudaStreamCreateWithFlags(&cmp, cudaStreamNonBlocking) == cudaSuccess;
+    if (!ok) cudaGetLastError();
+  }
+};
+HostStreams& host_streams() {
+  thread_local HostStreams hs;
+  return hs;
+}
 
 }  // namespace
 
@@ -441,42 +480,122 @@ int streamkl_fwd_bwd_host(int dtype, const void* Q1, const void* K1, const void*
   }
   if (!device_is_sm100()) return STREAMKL_ERR_CUDA;
   const size_t es = dtype == STREAMKL_BF16 ? 2 : 4;
-  const size_t nq1 = size_t(s.BH) * NQ * d1 * es, nk1 = size_t(s.BH) * NK * d1 * es;
-  const size_t nq2 = size_t(s.BH) * NQ * d2 * es, nk2 = size_t(s.BH) * NK * d2 * es;
-  const size_t nrow = size_t(s.BH) * NQ * sizeof(float);
-  DevBuf bQ1, bK1, bQ2, bK2, bkl, bl1, bl2, bg, gQ1, gK1, gQ2, gK2, bws;
-  const size_t ws_bytes = want_bwd ? streamkl_bwd_workspace_bytes(B, H, NQ, NK, d1, d2, dQ1 != nullptr) : 0;
-  if (!bQ1.alloc(nq1) || !bK1.alloc(nk1) || !bQ2.alloc(nq2) || !bK2.alloc(nk2) || !bkl.alloc(nrow) || !bl1.alloc(nrow) ||
-      !bl2.alloc(nrow)) { cudaGetLastError(); return STREAMKL_ERR_CUDA; }
-  if (want_bwd && (!bws.alloc(ws_bytes) || !bg.alloc(nrow) || !gQ2.alloc(nq2) || !gK2.alloc(nk2) || (dQ1 && (!gQ1.alloc(nq1) || !gK1.alloc(nk1))))) {
+  const bool teacher = dQ1 != nullptr;
+  // per-head sizes: heads are independent, so the batch is cut into groups of whole heads and the upload of group g+1
+  // and the download of group g-1 overlap the kernels of group g (three streams, events between them)
+  const size_t hq1 = size_t(NQ) * d1 * es, hk1 = size_t(NK) * d1 * es, hq2 = size_t(NQ) * d2 * es, hk2 = size_t(NK) * d2 * es;
+  const size_t hrow = size_t(NQ) * sizeof(float);
+  const size_t hws = want_bwd ? streamkl_bwd_workspace_bytes(1, 1, NQ, NK, d1, d2, teacher) : 0;
+  const long long BH = s.BH;
+  long long gs = BH;   // heads per group
+  if (BH > 1 && (size_t(d1) * es) % 16 == 0 && (size_t(d2) * es) % 16 == 0 && size_t(BH) * (hq1 + hk1 + hq2 + hk2) >= (64u << 20)) {
+    const long long tq = (NQ + 255) / 256;
+    const long long fill = (2 * 148 + tq - 1) / (tq > 0 ? tq : 1);   // enough CTAs per launch for two waves
+    gs = (BH + 7) / 8;
+    if (gs < fill) gs = fill;
+    if (gs > BH) gs = BH;
+  }
+  const int G = int((BH + gs - 1) / gs);
+  HostStreams& hs = host_streams();
+  if (!hs.ok) return STREAMKL_ERR_CUDA;
+
+  AsyncScratch sc(stream);
+  uint8_t* bQ1 = static_cast<uint8_t*>(sc.get(BH * hq1));
+  uint8_t* bK1 = static_cast<uint8_t*>(sc.get(BH * hk1));
+  uint8_t* bQ2 = static_cast<uint8_t*>(sc.get(BH * hq2));
+  uint8_t* bK2 = static_cast<uint8_t*>(sc.get(BH * hk2));
+  uint8_t* bkl = static_cast<uint8_t*>(sc.get(BH * hrow));
+  uint8_t* bl1 = static_cast<uint8_t*>(sc.get(BH * hrow));
+  uint8_t* bl2 = static_cast<uint8_t*>(sc.get(BH * hrow));
+  uint8_t *bg = nullptr, *gQ1 = nullptr, *gK1 = nullptr, *gQ2 = nullptr, *gK2 = nullptr, *bws = nullptr;
+  if (want_bwd) {
+    bg = static_cast<uint8_t*>(sc.get(BH * hrow));
+    gQ2 = static_cast<uint8_t*>(sc.get(BH * hq2));
+    gK2 = static_cast<uint8_t*>(sc.get(BH * hk2));
+    bws = static_cast<uint8_t*>(sc.get(BH * hws));
+    if (teacher) {
+      gQ1 = static_cast<uint8_t*>(sc.get(BH * hq1));
+      gK1 = static_cast<uint8_t*>(sc.get(BH * hk1));
+    }
+  }
+  if (!sc.ok) return STREAMKL_ERR_CUDA;
+  std::vector<cudaEvent_t> ev(size_t(2 * G + 4), nullptr);
+  bool ok = true;
+  for (cudaEvent_t& e : ev) ok = ok && cudaEventCreateWithFlags(&e, cudaEventDisableTiming) == cudaSuccess;
+  auto cleanup = [&]() { for (cudaEvent_t e : ev) if (e) cudaEventDestroy(e); };
+  if (!ok) { cudaGetLastError(); cleanup(); return STREAMKL_ERR_CUDA; }
+  cudaEvent_t ev_start = ev[size_t(2 * G)], ev_in_done = ev[size_t(2 * G + 1)], ev_cmp_done = ev[size_t(2 * G + 2)], ev_out_done = ev[size_t(2 * G + 3)];
+  // the scratch was allocated in order on `stream`: everything else starts after that point
+  ok = ok && cudaEventRecord(ev_start, stream) == cudaSuccess && cudaStreamWaitEvent(hs.in, ev_start, 0) == cudaSuccess &&
+       cudaStreamWaitEvent(hs.cmp, ev_start, 0) == cudaSuccess && cudaStreamWaitEvent(hs.out, ev_start, 0) == cudaSuccess;
+  auto cp = [&](void* dst, const void* src, size_t n, cudaMemcpyKind kind, cudaStream_t st) {
+    return n == 0 || cudaMemcpyAsync(dst, src, n, kind, st) == cudaSuccess;
+  };
+  const uint8_t *hQ1 = static_cast<const uint8_t*>(Q1), *hK1 = static_cast<const uint8_t*>(K1);
+  const uint8_t *hQ2 = static_cast<const uint8_t*>(Q2), *hK2 = static_cast<const uint8_t*>(K2);
+  int launches = 0;
+  rc = STREAMKL_OK;
+  for (int g = 0; g < G && ok && rc == STREAMKL_OK; ++g) {
+    const size_t h0 = size_t(g) * size_t(gs);
+    const int hn = int(std::min<long long>(gs, BH - (long long)h0));
+    // ---- upload (stream `in`)
+    ok = ok && cp(bQ1 + h0 * hq1, hQ1 + h0 * hq1, hn * hq1, cudaMemcpyHostToDevice, hs.in) &&
+         cp(bK1 + h0 * hk1, hK1 + h0 * hk1, hn * hk1, cudaMemcpyHostToDevice, hs.in) &&
+         cp(bQ2 + h0 * hq2, hQ2 + h0 * hq2, hn * hq2, cudaMemcpyHostToDevice, hs.in) &&
+         cp(bK2 + h0 * hk2, hK2 + h0 * hk2, hn * hk2, cudaMemcpyHostToDevice, hs.in);
+    if (want_bwd) ok = ok && cp(bg + h0 * hrow, reinterpret_cast<const uint8_t*>(dkl_rows) + h0 * hrow, hn * hrow, cudaMemcpyHostToDevice, hs.in);
+    ok = ok && cudaEventRecord(ev[size_t(2 * g)], hs.in) == cudaSuccess && cudaStreamWaitEvent(hs.cmp, ev[size_t(2 * g)], 0) == cudaSuccess;
+    if (!ok) break;
+    // ---- kernels (stream `cmp`): the group is a batch of hn heads
+    if (s.NQ > 0) {
+      rc = fwd_dispatch(dtype, bQ1 + h0 * hq1, bK1 + h0 * hk1, bQ2 + h0 * hq2, bK2 + h0 * hk2, 1, hn, NQ, NK, d1, d2, c1, c2, causal,
+                        reinterpret_cast<float*>(bkl + h0 * hrow), reinterpret_cast<float*>(bl1 + h0 * hrow),
+                        reinterpret_cast<float*>(bl2 + h0 * hrow), hs.cmp);
+      if (rc != STREAMKL_OK) break;
+      launches += g_last_launches;
+    }
+    if (want_bwd) {
+      rc = bwd_dispatch(dtype, bQ1 + h0 * hq1, bK1 + h0 * hk1, bQ2 + h0 * hq2, bK2 + h0 * hk2, 1, hn, NQ, NK, d1, d2, c1, c2, causal,
+                        reinterpret_cast<float*>(bkl + h0 * hrow), reinterpret_cast<float*>(bl1 + h0 * hrow),
+                        reinterpret_cast<float*>(bl2 + h0 * hrow), reinterpret_cast<float*>(bg + h0 * hrow),
+                        teacher ? gQ1 + h0 * hq1 : nullptr, teacher ? gK1 + h0 * hk1 : nullptr, gQ2 + h0 * hq2, gK2 + h0 * hk2,
+                        hws ? bws + h0 * hws : nullptr, hn * hws, hs.cmp);
+      if (rc != STREAMKL_OK) break;
+      launches += g_last_launches;
+    }
+    ok = ok && cudaEventRecord(ev[size_t(2 * g + 1)], hs.cmp) == cudaSuccess && cudaStreamWaitEvent(hs.out, ev[size_t(2 * g + 1)], 0) == cudaSuccess;
+    // ---- download (stream `out`)
+    if (s.NQ > 0)
+      ok = ok && cp(reinterpret_cast<uint8_t*>(kl_rows) + h0 * hrow, bkl + h0 * hrow, hn * hrow, cudaMemcpyDeviceToHost, hs.out) &&
+           cp(reinterpret_cast<uint8_t*>(lse1) + h0 * hrow, bl1 + h0 * hrow, hn * hrow, cudaMemcpyDeviceToHost, hs.out) &&
+           cp(reinterpret_cast<uint8_t*>(lse2) + h0 * hrow, bl2 + h0 * hrow, hn * hrow, cudaMemcpyDeviceToHost, hs.out);
+    if (want_bwd) {
+      ok = ok && cp(static_cast<uint8_t*>(dQ2) + h0 * hq2, gQ2 + h0 * hq2, hn * hq2, cudaMemcpyDeviceToHost, hs.out) &&
+           cp(static_cast<uint8_t*>(dK2) + h0 * hk2, gK2 + h0 * hk2, hn * hk2, cudaMemcpyDeviceToHost, hs.out);
+      if (teacher)
+        ok = ok && cp(static_cast<uint8_t*>(dQ1) + h0 * hq1, gQ1 + h0 * hq1, hn * hq1, cudaMemcpyDeviceToHost, hs.out) &&
+             cp(static_cast<uint8_t*>(dK1) + h0 * hk1, gK1 + h0 * hk1, hn * hk1, cudaMemcpyDeviceToHost, hs.out);
+    }
+  }
+  // join: `stream` continues (and the scratch is returned to the pool) only after all three helper streams are done
+  cudaEventRecord(ev_in_done, hs.in); cudaEventRecord(ev_cmp_done, hs.cmp); cudaEventRecord(ev_out_done, hs.out);
+  cudaStreamWaitEvent(stream, ev_in_done, 0); cudaStreamWaitEvent(stream, ev_cmp_done, 0); cudaStreamWaitEvent(stream, ev_out_done, 0);
+  const bool synced = cudaStreamSynchronize(stream) == cudaSuccess;
+  cleanup();
+  if (rc != STREAMKL_OK) { cudaGetLastError(); return rc; }
+  if (!ok || !synced) { cudaGetLastError(); return STREAMKL_ERR_CUDA; }
+  g_last_launches = launches;
+  return STREAMKL_OK;
+}
+
+int streamkl_host_trim(void) {
+  int dev = 0;
+  cudaMemPool_t pool;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetDefaultMemPool(&pool, dev) != cudaSuccess ||
+      cudaDeviceSynchronize() != cudaSuccess || cudaMemPoolTrimTo(pool, 0) != cudaSuccess) {
     cudaGetLastError();
     return STREAMKL_ERR_CUDA;
   }
-  auto up = [&](void* d, const void* h, size_t n) { return n == 0 || cudaMemcpyAsync(d, h, n, cudaMemcpyHostToDevice, stream) == cudaSuccess; };
-  auto down = [&](void* h, const void* d, size_t n) { return n == 0 || cudaMemcpyAsync(h, d, n, cudaMemcpyDeviceToHost, stream) == cudaSuccess; };
-  if (!up(bQ1.p, Q1, nq1) || !up(bK1.p, K1, nk1) || !up(bQ2.p, Q2, nq2) || !up(bK2.p, K2, nk2)) return STREAMKL_ERR_CUDA;
-  if (want_bwd && !up(bg.p, dkl_rows, nrow)) return STREAMKL_ERR_CUDA;
-  int launches = 0;
-  if (s.NQ > 0) {
-    rc = fwd_dispatch(dtype, bQ1.p, bK1.p, bQ2.p, bK2.p, B, H, NQ, NK, d1, d2, c1, c2, causal, static_cast<float*>(bkl.p),
-                      static_cast<float*>(bl1.p), static_cast<float*>(bl2.p), stream);
-    if (rc != STREAMKL_OK) { cudaStreamSynchronize(stream); return rc; }
-    launches += g_last_launches;
-  }
-  if (want_bwd) {
-    rc = bwd_dispatch(dtype, bQ1.p, bK1.p, bQ2.p, bK2.p, B, H, NQ, NK, d1, d2, c1, c2, causal, static_cast<float*>(bkl.p),
-                      static_cast<float*>(bl1.p), static_cast<float*>(bl2.p), static_cast<float*>(bg.p), gQ1.p, gK1.p, gQ2.p, gK2.p,
-                      bws.p, ws_bytes, stream);
-    if (rc != STREAMKL_OK) { cudaStreamSynchronize(stream); return rc; }
-    launches += g_last_launches;
-  }
-  bool ok = down(kl_rows, bkl.p, nrow) && down(lse1, bl1.p, nrow) && down(lse2, bl2.p, nrow);
-  if (want_bwd) {
-    ok = ok && down(dQ2, gQ2.p, nq2) && down(dK2, gK2.p, nk2);
-    if (dQ1) ok = ok && down(dQ1, gQ1.p, nq1) && down(dK1, gK1.p, nk1);
-  }
-  if (cudaStreamSynchronize(stream) != cudaSuccess || !ok) { cudaGetLastError(); return STREAMKL_ERR_CUDA; }
-  g_last_launches = launches;
   return STREAMKL_OK;
 }
 

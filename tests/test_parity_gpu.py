@@ -169,3 +169,21 @@ def test_host_entry_point_matches_device_path():
     assert np.array_equal(bits_to_f64(out["dK2"]), to_f64(dK2))
     kl_h, l1_h, l2_h = skl.streamkl_fwd_host(inp["Q1"], inp["K1"], inp["Q2"], inp["K2"], cfg.c1, cfg.c2, cfg.causal)
     assert np.array_equal(kl_h, out["kl"]) and np.array_equal(l1_h, out["lse1"]) and np.array_equal(l2_h, out["lse2"])
+
+
+def test_host_entry_point_pipelined_head_groups_match_device_path():
+    """cfg 2 at full size (32 heads, 136 MB of inputs): the host entry point splits the batch into head groups and overlaps
+    copies with kernels; every group must land where one ungrouped device call puts it, bit for bit."""
+    import paper_2606_20005_b200 as skl
+
+    cfg = W.CONFIGS[2]
+    inp = W.all_inputs(cfg)
+    out = skl.streamkl_fwd_bwd_host(inp["Q1"], inp["K1"], inp["Q2"], inp["K2"], cfg.c1, cfg.c2, cfg.causal, inp["g"], teacher=True)
+    assert skl.streamkl_last_launch_count() > 4          # more than one group's worth of {fwd, stats, dQ, dK}
+    Q1, K1, Q2, K2 = (to_torch(inp[k]) for k in ("Q1", "K1", "Q2", "K2"))
+    kl, l1, l2 = skl.streamkl_fwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, cfg.causal)
+    dQ1, dK1, dQ2, dK2 = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, cfg.causal, kl, l1, l2, to_torch(inp["g"]), teacher=True)
+    assert np.array_equal(out["kl"], kl.cpu().numpy()) and np.array_equal(out["lse2"], l2.cpu().numpy())
+    for name, t in (("dQ1", dQ1), ("dK1", dK1), ("dQ2", dQ2), ("dK2", dK2)):
+        assert np.array_equal(bits_to_f64(out[name]), to_f64(t)), name
+    skl.streamkl_host_trim()
