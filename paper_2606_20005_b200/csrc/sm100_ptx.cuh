@@ -224,12 +224,12 @@ __device__ __forceinline__ float2 mul2(float2 a, float2 b) {
 // exp2 on the FMA and ALU pipes, no MUFU (north_star: "FMA-polynomial exp2 where ncu shows MUFU is the limiter"):
 // round-to-nearest split x = n + f via the 1.5*2^23 magic constant, degree-3 minimax of 2^f on [-0.5, 0.5]
 // (relative error 7.6e-5, fitted in fp32), exponent inserted with an integer shift-add.  Two lanes per call so the
-// adds and FMAs are packed fp32x2.  Inputs are clamped at -126 (results below 2^-126 come out as ~1e-38, not 0);
-// valid for x < 2^22, meant for the x <= 0 arguments of a max-shifted softmax.
+// adds and FMAs are packed fp32x2.  Inputs are clamped to [-126, 127] (results below 2^-126 come out as ~1e-38, not 0;
+// above 2^127 as ~1.7e38); meant for the x <= 0 arguments of a max-shifted softmax.
 __device__ __forceinline__ float2 ex2_poly2(float2 x) {
   const float2 magic = make_float2(12582912.f, 12582912.f);
-  x.x = fmaxf(x.x, -126.f);
-  x.y = fmaxf(x.y, -126.f);
+  x.x = fminf(fmaxf(x.x, -126.f), 127.f);   // upper clamp: a stale softmax reference must show up as a huge p, not wrap
+  x.y = fminf(fmaxf(x.y, -126.f), 127.f);
   const float2 t = add2(x, magic);           // low mantissa bits of t = n (two's complement)
   const float2 f = sub2(x, sub2(t, magic));  // f in [-0.5, 0.5]
   float2 p = fma2(f, make_float2(0.055205512791872025f, 0.055205512791872025f), make_float2(0.24261389672756195f, 0.24261389672756195f));

@@ -25,6 +25,12 @@
 #define STREAMKL_FWD_POLY_EVERY 4
 #endif
 
+// 1: unmasked tiles are evaluated against the row's current reference and the row maximum is only recomputed when a
+// tile sum shows the reference is stale (online_update_lazy); 0: Alg.1 literally (row maximum every tile).
+#ifndef STREAMKL_FWD_LAZY_MAX
+#define STREAMKL_FWD_LAZY_MAX 1
+#endif
+
 namespace skl {
 
 template <int D1, int D2>
@@ -143,6 +149,56 @@ __device__ __forceinline__ void online_update(RowState& st, const uint32_t (&r1)
   st.acc = fmaf(st.acc, a1, fmaf(ref1 - ref2, sum1, dsum));    // line 12
   st.m1 = m1n;
   st.m2 = m2n;
+}
+
+// Unmasked tiles, lazy reference.  Alg.1 keeps m_t = the running MAXIMUM, but Eq.8-10 hold for ANY per-row reference
+// m_t as long as (l_t, acc) are expressed relative to it: the maximum is only there to keep exp() in range.  So the tile
+// is first evaluated against the reference the row already has -- no row-max reduction, no alpha, and the exps can
+// start as soon as the logits are in registers.  All p >= 0, hence max p <= sum p: if both tile sums stay below 2^20
+// nothing can have overflowed and the tile is committed as is.  Otherwise (first tile: reference -inf gives sum = inf;
+// or a logit more than ~20 log2-units above the reference) the reference is raised to the true maximum exactly as
+// Alg.1 lines 8-12 do (rescale l, acc by alpha) and the tile is evaluated again; then every p <= 1.
+template <int NC>
+__device__ __forceinline__ void online_update_lazy(RowState& st, const uint32_t (&r1)[NC], const uint32_t (&r2)[NC], float sc1, float sc2) {
+  const float2 vsc1 = make_float2(sc1, sc1), vsc2 = make_float2(sc2, sc2);
+#pragma unroll 1
+  for (int attempt = 0;; ++attempt) {
+    const float2 vr1 = make_float2(-st.m1, -st.m1), vr2 = make_float2(-st.m2, -st.m2);
+    float2 s1v[2] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f)}, s2v[2] = {s1v[0], s1v[0]}, ddv[2] = {s1v[0], s1v[0]};
+#pragma unroll
+    for (int e = 0; e < NC; e += 2) {
+      const float2 x1 = fma2(make_float2(__uint_as_float(r1[e]), __uint_as_float(r1[e + 1])), vsc1, vr1);
+      const float2 x2 = fma2(make_float2(__uint_as_float(r2[e]), __uint_as_float(r2[e + 1])), vsc2, vr2);
+      const bool poly = STREAMKL_FWD_POLY_EVERY > 0 && ((e >> 1) % (STREAMKL_FWD_POLY_EVERY > 0 ? STREAMKL_FWD_POLY_EVERY : 1)) == 0;
+      const float2 p1 = poly ? ex2_poly2(x1) : make_float2(ex2_approx(x1.x), ex2_approx(x1.y));
+      const float2 p2 = poly ? ex2_poly2(x2) : make_float2(ex2_approx(x2.x), ex2_approx(x2.y));
+      const int a = (e >> 1) & 1;
+      s1v[a] = add2(s1v[a], p1);
+      s2v[a] = add2(s2v[a], p2);
+      ddv[a] = fma2(p1, sub2(x1, x2), ddv[a]);
+    }
+    const float sum1 = (s1v[0].x + s1v[0].y) + (s1v[1].x + s1v[1].y);
+    const float sum2 = (s2v[0].x + s2v[0].y) + (s2v[1].x + s2v[1].y);
+    const float dsum = (ddv[0].x + ddv[0].y) + (ddv[1].x + ddv[1].y);
+    if ((sum1 <= 1048576.f && sum2 <= 1048576.f) || attempt >= 1) {   // (false for inf / NaN sums on the first attempt)
+      st.l1 += sum1;                                                   // line 11 with alpha = 1
+      st.l2 += sum2;
+      st.acc += fmaf(st.m1 - st.m2, sum1, dsum);                       // line 12: sum p1 (s1' - s2')
+      return;
+    }
+    float mx1a = -CUDART_INF_F, mx1b = -CUDART_INF_F, mx2a = -CUDART_INF_F, mx2b = -CUDART_INF_F;
+#pragma unroll
+    for (int e = 0; e < NC; e += 4) {
+      mx1a = max3(mx1a, __uint_as_float(r1[e]), __uint_as_float(r1[e + 1]));
+      mx1b = max3(mx1b, __uint_as_float(r1[e + 2]), __uint_as_float(r1[e + 3]));
+      mx2a = max3(mx2a, __uint_as_float(r2[e]), __uint_as_float(r2[e + 1]));
+      mx2b = max3(mx2b, __uint_as_float(r2[e + 2]), __uint_as_float(r2[e + 3]));
+    }
+    const float m1n = fmaxf(st.m1, fmaxf(mx1a, mx1b) * sc1), m2n = fmaxf(st.m2, fmaxf(mx2a, mx2b) * sc2);   // finite: the tile is unmasked
+    const float a1 = ex2_approx(st.m1 - m1n), a2 = ex2_approx(st.m2 - m2n);                                // m = -inf gives 0
+    st.l1 *= a1; st.acc *= a1; st.l2 *= a2;
+    st.m1 = m1n; st.m2 = m2n;
+  }
 }
 
 template <int D1, int D2, bool CAUSAL, bool SPLIT = false>
@@ -315,7 +371,11 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
       const int kbase = (j_begin + j) * C::BK + half * C::BC;
       const bool masked = (CAUSAL && (kbase + C::BC - 1 > first_row_limit)) || (kbase + C::BC > p.NK);
       if (masked) online_update<true, C::BC>(st, r1, r2, p.sc1, p.sc2, kbase, limit);
+#if STREAMKL_FWD_LAZY_MAX
+      else        online_update_lazy<C::BC>(st, r1, r2, p.sc1, p.sc2);
+#else
       else        online_update<false, C::BC>(st, r1, r2, p.sc1, p.sc2, kbase, limit);
+#endif
     }
     if (n > 0) {
       // merge the two column halves of each row (Eq.11 with (m2,l2) carried too, R11).  The exchange buffer aliases this
