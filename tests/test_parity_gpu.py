@@ -187,3 +187,35 @@ def test_host_entry_point_pipelined_head_groups_match_device_path():
     for name, t in (("dQ1", dQ1), ("dK1", dK1), ("dQ2", dQ2), ("dK2", dK2)):
         assert np.array_equal(bits_to_f64(out[name]), to_f64(t)), name
     skl.streamkl_host_trim()
+
+
+def test_device_entry_points_are_graph_capturable_and_deterministic():
+    """streamkl_fwd + streamkl_bwd only enqueue kernels on the caller's stream (no allocation, no sync): they can be
+    captured into a CUDA graph, and replaying it reproduces the eager results bit for bit (tile ownership: no atomics)."""
+    import torch
+
+    import paper_2606_20005_b200 as skl
+
+    cfg = W.shrink(W.CONFIGS[2], H=3, NQ=1100, NK=1100)
+    inp = W.all_inputs(cfg)
+    Q1, K1, Q2, K2 = (to_torch(inp[k]) for k in ("Q1", "K1", "Q2", "K2"))
+    g = to_torch(inp["g"])
+    kl, l1, l2 = skl.streamkl_fwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, True)
+    eager = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, True, kl, l1, l2, g, teacher=True)
+    ws = torch.empty(skl.streamkl_bwd_workspace_bytes(cfg.B, cfg.H, cfg.NQ, cfg.NK, cfg.d1, cfg.d2, True), dtype=torch.uint8, device="cuda")
+    outs = [torch.zeros_like(t) for t in (kl, l1, l2)]
+    grads = [torch.zeros_like(t) for t in eager]
+    torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        skl.streamkl_fwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, True, *outs)
+        skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, True, outs[0], outs[1], outs[2], g, teacher=True, dQ1=grads[0],
+                         dK1=grads[1], dQ2=grads[2], dK2=grads[3], workspace=ws)
+    for _ in range(2):
+        for t in outs + grads:
+            t.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(outs[0], kl) and torch.equal(outs[1], l1) and torch.equal(outs[2], l2)
+        for a, b in zip(grads, eager):
+            assert torch.equal(a, b)
