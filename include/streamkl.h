@@ -111,7 +111,22 @@ int streamkl_bwd_f32(const void* Q1, const void* K1, const void* Q2, const void*
                      void* dQ1, void* dK1, void* dQ2, void* dK2,
                      void* workspace, size_t workspace_bytes, streamkl_stream_t stream);       /* fp32 */
 
-/* Bytes of device scratch streamkl_bwd needs for this shape (O((NQ+NK)*d) at most, never O(NQ*NK)). */
+/*
+ * Backward strategy, per calling thread.  The tcgen05 path has two:
+ *   STREAMKL_BWD_SEPARATE : a Q-owner kernel (dQ) and a K-owner kernel (dK); every output tile has one owner, no atomics,
+ *                           bit-reproducible.  The only strategy when teacher gradients are requested.
+ *   STREAMKL_BWD_FUSED    : Setting 1 only (dQ1 = dK1 = NULL): one K-owner kernel visits every tile pair once, keeps dK2 in
+ *                           place and adds its dQ2 contributions with fp32 atomics into the workspace, then one rounding to
+ *                           bf16.  Half the logit recomputation and exps; dQ2 reproducible only up to fp32 summation order.
+ *   STREAMKL_BWD_AUTO     : (default) FUSED when it applies and NQ <= 512 (the measured crossover on B200; the paper's rule
+ *                           T_Q*C <= T_K, with the crossover found independent of T_K), else SEPARATE.
+ * Returns STREAMKL_OK, or STREAMKL_ERR_SHAPE for an unknown mode.
+ */
+enum { STREAMKL_BWD_AUTO = 0, STREAMKL_BWD_SEPARATE = 1, STREAMKL_BWD_FUSED = 2 };
+int streamkl_set_bwd_mode(int mode);
+
+/* Bytes of device scratch streamkl_bwd needs for this shape (O((NQ+NK)*d) at most, never O(NQ*NK)): 16 B per query of
+ * packed per-query scalars, plus -- without teacher gradients -- the fp32 dQ2 accumulator of the fused strategy. */
 size_t streamkl_bwd_workspace_bytes(int B, int H, int NQ, int NK, int d1, int d2, int want_teacher_grads);
 
 /*

@@ -15,6 +15,10 @@ from .binding import (  # noqa: F401
     streamkl_fwd_host,
     streamkl_fwd_splitk,
     streamkl_host_trim,
+    streamkl_set_bwd_mode,
+    STREAMKL_BWD_AUTO,
+    STREAMKL_BWD_SEPARATE,
+    STREAMKL_BWD_FUSED,
     streamkl_fwd_splitk_splits,
     streamkl_fwd_splitk_workspace_bytes,
     streamkl_kernel_name,

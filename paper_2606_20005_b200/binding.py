@@ -15,12 +15,14 @@ from .build import LIB_PATH
 __all__ = [
     "StreamKLError", "lib", "lib_path", "streamkl_fwd", "streamkl_bwd", "streamkl_bwd_workspace_bytes",
     "streamkl_fwd_splitk", "streamkl_fwd_splitk_splits", "streamkl_fwd_splitk_workspace_bytes",
-    "streamkl_fwd_host", "streamkl_fwd_bwd_host", "streamkl_host_trim", "streamkl_last_launch_count", "streamkl_strerror",
+    "streamkl_fwd_host", "streamkl_fwd_bwd_host", "streamkl_host_trim", "streamkl_set_bwd_mode",
+    "STREAMKL_BWD_AUTO", "STREAMKL_BWD_SEPARATE", "STREAMKL_BWD_FUSED", "streamkl_last_launch_count", "streamkl_strerror",
     "streamkl_profile_enable", "streamkl_profile_collect", "streamkl_kernel_name",
     "streamkl_version",
 ]
 
 STREAMKL_BF16, STREAMKL_F32 = 0, 1
+STREAMKL_BWD_AUTO, STREAMKL_BWD_SEPARATE, STREAMKL_BWD_FUSED = 0, 1, 2
 
 
 class StreamKLError(RuntimeError):
@@ -68,6 +70,8 @@ def lib() -> ctypes.CDLL:
     L.streamkl_fwd_host.restype = ci
     L.streamkl_fwd_bwd_host.argtypes = [ci] + [vp] * 4 + shape + [vp] + [vp] * 3 + [vp] * 4 + [vp]
     L.streamkl_fwd_bwd_host.restype = ci
+    L.streamkl_set_bwd_mode.argtypes = [ci]
+    L.streamkl_set_bwd_mode.restype = ci
     L.streamkl_host_trim.argtypes = []
     L.streamkl_host_trim.restype = ci
     L.streamkl_last_launch_count.argtypes = []
@@ -92,6 +96,13 @@ def streamkl_strerror(code: int) -> str:
 
 def streamkl_version() -> str:
     return lib().streamkl_version().decode()
+
+
+def streamkl_set_bwd_mode(mode: int) -> None:
+    """STREAMKL_BWD_AUTO | STREAMKL_BWD_SEPARATE (deterministic) | STREAMKL_BWD_FUSED (Setting 1, dQ2 by fp32 atomics)."""
+    rc = lib().streamkl_set_bwd_mode(int(mode))
+    if rc != 0:
+        raise StreamKLError(rc, "streamkl_set_bwd_mode")
 
 
 def streamkl_host_trim() -> None:

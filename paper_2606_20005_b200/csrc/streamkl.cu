@@ -13,19 +13,22 @@
 #include "../../include/streamkl.h"
 #include "streamkl_fwd_sm100.cuh"
 #include "streamkl_bwd_sm100.cuh"
+#include "streamkl_bwd_fused_sm100.cuh"
 #include "streamkl_simt.cuh"
 
 namespace {
 
 thread_local int g_last_launches = 0;
+thread_local int g_bwd_mode = STREAMKL_BWD_AUTO;
 
 // ---- optional per-kernel timing (streamkl_profile_*): CUDA events recorded on the launch stream around every kernel
-enum KernelId { KID_FWD_TC = 0, KID_BWD_DQ_TC, KID_BWD_DK_TC, KID_FWD_SIMT, KID_BWD_DQ_SIMT, KID_BWD_DK_SIMT, KID_BWD_STATS, KID_FWD_SPLITK_TC, KID_FWD_SPLITK_REDUCE, KID_COUNT };
+enum KernelId { KID_FWD_TC = 0, KID_BWD_DQ_TC, KID_BWD_DK_TC, KID_FWD_SIMT, KID_BWD_DQ_SIMT, KID_BWD_DK_SIMT, KID_BWD_STATS, KID_FWD_SPLITK_TC, KID_FWD_SPLITK_REDUCE, KID_BWD_FUSED_TC, KID_BWD_DQ_CONVERT, KID_COUNT };
 const char* const kKernelNames[KID_COUNT] = {"streamkl_fwd_sm100_kernel", "streamkl_bwd_sm100_kernel<OWNER_Q>",
                                              "streamkl_bwd_sm100_kernel<OWNER_K>", "streamkl_fwd_simt_kernel",
                                              "streamkl_bwd_simt_kernel<OWNER_Q>", "streamkl_bwd_simt_kernel<OWNER_K>",
                                              "streamkl_bwd_stats_kernel", "streamkl_fwd_sm100_kernel<SPLIT>",
-                                             "streamkl_fwd_splitk_reduce_kernel"};
+                                             "streamkl_fwd_splitk_reduce_kernel", "streamkl_bwd_fused_sm100_kernel",
+                                             "streamkl_bwd_dq_convert_kernel"};
 struct ProfRecord { int id; cudaEvent_t a, b; };
 thread_local bool g_prof_on = false;
 thread_local std::vector<ProfRecord>* g_prof = nullptr;
@@ -268,6 +271,48 @@ int launch_bwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2
   return STREAMKL_OK;
 }
 
+size_t stats_bytes_aligned(long long BH, int NQ) { return (size_t(BH) * size_t(skl::bwd_stats_padded_rows(NQ)) * 16 + 255) & ~size_t(255); }
+
+// Setting 1 in one visit: zero the fp32 dQ2 accumulator, run the fused K-owner kernel, convert dQ2.
+template <int D1, int D2, bool CAUSAL>
+int launch_bwd_fused(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, const float4* stats, float* dq_acc,
+                     void* dQ2, void* dK2, cudaStream_t stream) {
+  using C = skl::BwdFusedCfg<D1, D2>;
+  CUtensorMap tQ1, tK1, tQ2, tK2;
+  if (!make_tmap_bf16(&tQ1, Q1, int(s.BH), s.NQ, D1, C::BY) || !make_tmap_bf16(&tK1, K1, int(s.BH), s.NK, D1, C::BX) ||
+      !make_tmap_bf16(&tQ2, Q2, int(s.BH), s.NQ, D2, C::BY) || !make_tmap_bf16(&tK2, K2, int(s.BH), s.NK, D2, C::BX))
+    return STREAMKL_ERR_CUDA;
+  auto kern = skl::streamkl_bwd_fused_sm100_kernel<D1, D2, CAUSAL>;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
+    cudaGetLastError();
+    return STREAMKL_ERR_CUDA;
+  }
+  const size_t n = size_t(s.BH) * s.NQ * D2;
+  if (cudaMemsetAsync(dq_acc, 0, n * sizeof(float), stream) != cudaSuccess) { cudaGetLastError(); return STREAMKL_ERR_CUDA; }
+  skl::BwdFusedParams p;
+  p.NQ = s.NQ; p.NK = s.NK; p.BH = int(s.BH);
+  p.TX = (s.NK + C::BX - 1) / C::BX;
+  p.c1 = s.c1; p.c2 = s.c2;
+  p.stats = stats; p.dq_acc = dq_acc;
+  p.dK2 = static_cast<__nv_bfloat16*>(dK2);
+  const long long grid = (long long)p.TX * s.BH;
+  if (grid > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
+  {
+    ProfScope ps(KID_BWD_FUSED_TC, stream);
+    kern<<<dim3((unsigned)grid), C::THREADS, C::SMEM_BYTES, stream>>>(tQ1, tK1, tQ2, tK2, p);
+  }
+  if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
+  const long long n4 = (long long)(n / 4);
+  {
+    ProfScope ps(KID_BWD_DQ_CONVERT, stream);
+    skl::streamkl_bwd_dq_convert_kernel<<<dim3((unsigned)((n4 + 255) / 256)), 256, 0, stream>>>(reinterpret_cast<const float4*>(dq_acc),
+                                                                                             static_cast<uint2*>(dQ2), s.c2, n4);
+  }
+  if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
+  g_last_launches += 2;
+  return STREAMKL_OK;
+}
+
 template <int D1, int D2>
 int bwd_tc_both(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, const float* kl, const float* lse1,
                 const float* lse2, const float* dkl, void* dQ1, void* dK1, void* dQ2, void* dK2, void* workspace, cudaStream_t st) {
@@ -285,6 +330,16 @@ int bwd_tc_both(const void* Q1, const void* K1, const void* Q2, const void* K2, 
     }
     if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
     g_last_launches += 1;
+  }
+  // Strategy (PAPER.md:321 picks fused iff T_Q*C <= T_K with an empirically tuned C).  Measured on B200
+  // (profiles/r01f_fused_bwd.md): the one-visit kernel wins 1.3-3.0x while the Q-owner grid is small (T_Q <= 4 tiles of 128
+  // queries), is level at T_Q = 8 and loses a few per cent beyond, where its fp32 atomics (64 KB per 128x128 tile pair)
+  // run into the L2's atomic throughput; the crossover did not move with T_K (128 vs 1024), so the rule is on T_Q alone.
+  const bool fused = !t && (g_bwd_mode == STREAMKL_BWD_FUSED || (g_bwd_mode == STREAMKL_BWD_AUTO && (s.NQ + 127) / 128 <= 4));
+  if (fused) {   // Setting 1: one visit, dQ2 through fp32 atomics
+    float* dq_acc = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) + stats_bytes_aligned(s.BH, s.NQ));
+    return s.causal ? launch_bwd_fused<D1, D2, true>(Q1, K1, Q2, K2, s, stats, dq_acc, dQ2, dK2, st)
+                    : launch_bwd_fused<D1, D2, false>(Q1, K1, Q2, K2, s, stats, dq_acc, dQ2, dK2, st);
   }
 #define SKL_BWD(CA, TE)                                                                                                   \
   rc = launch_bwd_tc<D1, D2, CA, TE, false>(Q1, K1, Q2, K2, s, stats, dQ1, dQ2, st);                                      \
@@ -445,12 +500,21 @@ int streamkl_fwd_splitk(const void* Q1, const void* K1, const void* Q2, const vo
                       static_cast<cudaStream_t>(stream), splits, static_cast<float*>(workspace));
 }
 
-size_t streamkl_bwd_workspace_bytes(int B, int H, int NQ, int, int d1, int d2, int) {
+size_t streamkl_bwd_workspace_bytes(int B, int H, int NQ, int, int d1, int d2, int want_teacher) {
   // both gradients are produced by tile ownership: no fp32 accumulation workspace.  The tcgen05 kernels read the
   // per-query scalars (lse1, lse2, dkl, kl) from a packed copy: 16 B per query, rows padded to 64 per head -- O(NQ).
   if (B <= 0 || H <= 0 || NQ <= 0) return 0;
   if (!((d1 == 64 || d1 == 128) && (d2 == 64 || d2 == 128))) return 0;
-  return size_t(B) * size_t(H) * size_t(skl::bwd_stats_padded_rows(NQ)) * 16;
+  const long long BH = (long long)B * H;
+  if (want_teacher) return size_t(BH) * size_t(skl::bwd_stats_padded_rows(NQ)) * 16;
+  // Setting 1: + the fp32 dQ2 accumulator of the one-visit kernel (O(NQ d2)), whatever mode is selected at call time
+  return stats_bytes_aligned(BH, NQ) + size_t(BH) * size_t(NQ) * size_t(d2) * sizeof(float);
+}
+
+int streamkl_set_bwd_mode(int mode) {
+  if (mode != STREAMKL_BWD_AUTO && mode != STREAMKL_BWD_SEPARATE && mode != STREAMKL_BWD_FUSED) return STREAMKL_ERR_SHAPE;
+  g_bwd_mode = mode;
+  return STREAMKL_OK;
 }
 
 int streamkl_fwd_host(int dtype, const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1,

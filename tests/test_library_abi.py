@@ -106,7 +106,9 @@ def test_workspace_is_never_quadratic(L):
 
 def test_bwd_workspace_is_16_bytes_per_padded_query(L):
     assert L.streamkl_bwd_workspace_bytes(1, 32, 65536, 65536, 128, 128, 1) == 32 * 65536 * 16
-    assert L.streamkl_bwd_workspace_bytes(2, 3, 100, 777, 128, 64, 0) == 6 * 128 * 16      # rows padded to 64 per head
+    assert L.streamkl_bwd_workspace_bytes(2, 3, 100, 777, 128, 64, 1) == 6 * 128 * 16      # rows padded to 64 per head
+    # Setting 1: + the fp32 dQ2 accumulator of the fused strategy (scalars padded to 256 B)
+    assert L.streamkl_bwd_workspace_bytes(2, 3, 100, 777, 128, 64, 0) == 6 * 128 * 16 + 6 * 100 * 64 * 4
     assert L.streamkl_bwd_workspace_bytes(1, 1, 256, 256, 48, 80, 0) == 0                  # SIMT path: no workspace
 
 
@@ -135,3 +137,8 @@ def test_splitk_workspace_and_argument_checks(L):
     assert call(16, 100) == -5
     assert call(24, 1 << 20) == -3                            # misaligned workspace
     assert call(16, 1 << 20, NK=0) in (-2, -5)                # shape errors are still reported
+
+
+def test_bwd_mode_selector(L):
+    assert L.streamkl_set_bwd_mode(1) == 0 and L.streamkl_set_bwd_mode(2) == 0 and L.streamkl_set_bwd_mode(0) == 0
+    assert L.streamkl_set_bwd_mode(7) == -2

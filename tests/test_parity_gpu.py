@@ -160,6 +160,7 @@ def test_host_entry_point_matches_device_path():
 
     cfg = W.shrink(W.CONFIGS[3], H=2, NQ=512, NK=512)
     inp = W.all_inputs(cfg)
+    skl.streamkl_set_bwd_mode(skl.STREAMKL_BWD_SEPARATE)   # bit-for-bit comparison: the atomic-free strategy
     out = skl.streamkl_fwd_bwd_host(inp["Q1"], inp["K1"], inp["Q2"], inp["K2"], cfg.c1, cfg.c2, cfg.causal, inp["g"], teacher=False)
     Q1, K1, Q2, K2 = (to_torch(inp[k]) for k in ("Q1", "K1", "Q2", "K2"))
     kl, l1, l2 = skl.streamkl_fwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, cfg.causal)
@@ -169,6 +170,7 @@ def test_host_entry_point_matches_device_path():
     assert np.array_equal(bits_to_f64(out["dK2"]), to_f64(dK2))
     kl_h, l1_h, l2_h = skl.streamkl_fwd_host(inp["Q1"], inp["K1"], inp["Q2"], inp["K2"], cfg.c1, cfg.c2, cfg.causal)
     assert np.array_equal(kl_h, out["kl"]) and np.array_equal(l1_h, out["lse1"]) and np.array_equal(l2_h, out["lse2"])
+    skl.streamkl_set_bwd_mode(skl.STREAMKL_BWD_AUTO)
 
 
 def test_host_entry_point_pipelined_head_groups_match_device_path():
@@ -219,3 +221,49 @@ def test_device_entry_points_are_graph_capturable_and_deterministic():
         assert torch.equal(outs[0], kl) and torch.equal(outs[1], l1) and torch.equal(outs[2], l2)
         for a, b in zip(grads, eager):
             assert torch.equal(a, b)
+
+
+@pytest.mark.parametrize("d1,d2", [(128, 128), (128, 64), (64, 128), (64, 64)])
+@pytest.mark.parametrize("causal", [False, True])
+def test_setting1_fused_and_separate_strategies_agree_with_the_oracle(d1, d2, causal):
+    """Setting 1 (teacher frozen) through both backward strategies: the one-visit kernel with fp32-atomic
+    dQ2 and the two deterministic owner kernels; ragged sizes, several K-owner tiles, several 64-query steps."""
+    import paper_2606_20005_b200 as skl
+
+    cfg = W.Config(50 + d1 // 64 * 2 + d2 // 64, "setting1", 1, 3, 457, 901, d1, d2, "bf16", causal, teacher_grads=False)
+    inp = W.all_inputs(cfg)
+    Q1, K1, Q2, K2 = (to_torch(inp[k]) for k in ("Q1", "K1", "Q2", "K2"))
+    g = to_torch(inp["g"])
+    ref = attention_kl(*(bits_to_f64(inp[k]) for k in ("Q1", "K1", "Q2", "K2")), cfg.c1, cfg.c2, cfg.causal,
+                       g=inp["g"].astype(np.float64), teacher=False)
+    kl, l1, l2 = skl.streamkl_fwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, cfg.causal)
+    res = {}
+    try:
+        for mode in (skl.STREAMKL_BWD_FUSED, skl.STREAMKL_BWD_SEPARATE):
+            skl.streamkl_set_bwd_mode(mode)
+            _, _, dQ2, dK2 = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, cfg.causal, kl, l1, l2, g, teacher=False)
+            check_grad(to_f64(dQ2), ref["dQ2"], f"mode {mode} dQ2")
+            check_grad(to_f64(dK2), ref["dK2"], f"mode {mode} dK2")
+            res[mode] = (to_f64(dQ2), to_f64(dK2), skl.streamkl_last_launch_count())
+    finally:
+        skl.streamkl_set_bwd_mode(skl.STREAMKL_BWD_AUTO)
+    assert res[skl.STREAMKL_BWD_FUSED][2] == 3 and res[skl.STREAMKL_BWD_SEPARATE][2] == 3   # {stats, fused, convert} / {stats, dQ, dK}
+
+
+def test_setting1_fused_mixed_sign_upstream_gradient_and_tiny_sizes():
+    """dkl_rows of both signs (and zeros); NQ, NK below one tile."""
+    import torch
+
+    import paper_2606_20005_b200 as skl
+
+    for NQ, NK in ((1, 1), (5, 300), (130, 70)):
+        cfg = W.Config(58, "setting1-sign", 1, 2, NQ, NK, 128, 128, "bf16", False, teacher_grads=False)
+        inp = W.all_inputs(cfg)
+        gnp = inp["g"] - 1.0
+        gnp[..., ::3] = 0.0
+        Q1, K1, Q2, K2 = (to_torch(inp[k]) for k in ("Q1", "K1", "Q2", "K2"))
+        ref = attention_kl(*(bits_to_f64(inp[k]) for k in ("Q1", "K1", "Q2", "K2")), cfg.c1, cfg.c2, False, g=gnp.astype(np.float64), teacher=False)
+        kl, l1, l2 = skl.streamkl_fwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, False)
+        _, _, dQ2, dK2 = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, False, kl, l1, l2, torch.from_numpy(gnp).cuda(), teacher=False)
+        check_grad(to_f64(dQ2), ref["dQ2"], f"{NQ}x{NK} dQ2")
+        check_grad(to_f64(dK2), ref["dK2"], f"{NQ}x{NK} dK2")
