@@ -267,3 +267,31 @@ def test_setting1_fused_mixed_sign_upstream_gradient_and_tiny_sizes():
         _, _, dQ2, dK2 = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, False, kl, l1, l2, torch.from_numpy(gnp).cuda(), teacher=False)
         check_grad(to_f64(dQ2), ref["dQ2"], f"{NQ}x{NK} dQ2")
         check_grad(to_f64(dK2), ref["dK2"], f"{NQ}x{NK} dK2")
+
+
+def test_one_million_keys_and_many_small_heads():
+    """Index arithmetic at the extremes: NK = 2^20 + 3 keys (8 query rows: forward, split-K forward, both Setting-1 backward
+    strategies, Setting-2 backward), and 1024 heads of a 130 x 190 problem in one call."""
+    import paper_2606_20005_b200 as skl
+
+    cfg = W.Config(46, "1M-keys", 1, 2, 8, (1 << 20) + 3, 128, 64, "bf16", False)
+    inp = W.all_inputs(cfg)
+    Q1, K1, Q2, K2 = (to_torch(inp[k]) for k in ("Q1", "K1", "Q2", "K2"))
+    g = to_torch(inp["g"])
+    ref = attention_kl(*(bits_to_f64(inp[k]) for k in ("Q1", "K1", "Q2", "K2")), cfg.c1, cfg.c2, False, g=inp["g"].astype(np.float64), teacher=True)
+    kl, l1, l2 = skl.streamkl_fwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, False)
+    check_fwd(to_f64(kl), to_f64(l1), to_f64(l2), ref, "1M fwd")
+    ks, l1s, l2s = skl.streamkl_fwd_splitk(Q1, K1, Q2, K2, cfg.c1, cfg.c2, False)
+    check_fwd(to_f64(ks), to_f64(l1s), to_f64(l2s), ref, "1M split-K")
+    dQ1, dK1, dQ2, dK2 = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, False, kl, l1, l2, g, teacher=True)
+    for name, t in (("dQ1", dQ1), ("dK1", dK1), ("dQ2", dQ2), ("dK2", dK2)):
+        check_grad(to_f64(t), ref[name], "1M " + name)
+    try:
+        for mode in (skl.STREAMKL_BWD_FUSED, skl.STREAMKL_BWD_SEPARATE):
+            skl.streamkl_set_bwd_mode(mode)
+            _, _, dQ2, dK2 = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, False, kl, l1, l2, g, teacher=False)
+            check_grad(to_f64(dQ2), ref["dQ2"], f"1M mode {mode} dQ2")
+            check_grad(to_f64(dK2), ref["dK2"], f"1M mode {mode} dK2")
+    finally:
+        skl.streamkl_set_bwd_mode(skl.STREAMKL_BWD_AUTO)
+    run_case(W.Config(47, "many-heads", 32, 32, 130, 190, 64, 128, "bf16", True))
