@@ -454,6 +454,13 @@ def main():
         "fwd_frac_of_measured_bf16_burst": flop_f / (res["fwd_ms"] * 1e-3) / 1e12 / float(pk["bf16_tflops"]),
         "fwd_frac_of_spec_2250": flop_f / (res["fwd_ms"] * 1e-3) / 1e12 / SPEC_BF16_TFLOPS,
         "fwd_exp_per_s": 2.0 * cfg.visible_pairs_convention() / (res["fwd_ms"] * 1e-3),
+        # exps per second against MUFU's 16 ex2/clk/SM x 148 SMs at the SM clock observed during the timed region
+        "fwd_frac_of_mufu_peak_at_observed_clock": (2.0 * cfg.visible_pairs_convention() / (res["fwd_ms"] * 1e-3))
+        / (16.0 * 148.0 * 1e6 * (clk.summary().get("sm_mhz") or 1965.0)),
+        "fwd_frac_of_measured_bf16_sustained": flop_f / (res["fwd_ms"] * 1e-3) / 1e12 / float(pk["bf16_tflops_sustained"]),
+        "bwd_frac_of_measured_bf16_sustained": flop_b / (res["bwd_ms"] * 1e-3) / 1e12 / float(pk["bf16_tflops_sustained"]),
+        "bwd_executed_tflops": sum(kernel_flops(cfg, k) * v["launches_per_step"] for k, v in res["kernels"].items()
+                                   if "bwd_sm100" in k) / (res["bwd_ms"] * 1e-3) / 1e12,
         "kernels": res["kernels"],
         "extra_hbm_bytes": {"total_peak_over_inputs": int(extra_hbm), "outputs": output_bytes(cfg),
                             "workspace": int(res["workspace_bytes"])},
