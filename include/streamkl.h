@@ -71,12 +71,12 @@ int streamkl_fwd_f32(const void* Q1, const void* K1, const void* Q2, const void*
 
 /*
  * Split-K forward for small NQ (Eq.11; bf16, d1,d2 in {64,128}).  The key range is cut into W
- * contiguous chunks of C_K = 64*ceil(ceil(NK/64)/W) keys (the paper's ceil(NK/W), rounded up to whole 64-key tiles);
+ * contiguous chunks of C_K = 128*ceil(ceil(NK/128)/W) keys (the paper's ceil(NK/W), rounded up to whole 128-key tiles);
  * the grid becomes (bsz, T_Q, W); every CTA writes its chunk's partial statistics (m1,l1,m2,l2,acc) -- 5 floats per
  * row and chunk -- to `workspace`, and a reduce kernel merges them with Eq.11 ((m2,l2) merged the same way) and
  * finishes Alg.1 lines 13-15.  Same outputs as streamkl_fwd up to fp32 summation order.
  *   splits    : W; <= 0 selects it adaptively (streamkl_fwd_splitk_splits with the default target); clamped to
- *               ceil(NK/64); W = 1 launches the default kernel and touches no workspace.
+ *               ceil(NK/128); W = 1 launches the default kernel and touches no workspace.
  *   workspace : device scratch of at least streamkl_fwd_splitk_workspace_bytes(B,H,NQ,W) bytes, 16-byte aligned.
  * Other head dims run the unsplit SIMT kernel.  Error behaviour as streamkl_fwd, plus STREAMKL_ERR_WORKSPACE.
  */
@@ -84,8 +84,8 @@ int streamkl_fwd_splitk(const void* Q1, const void* K1, const void* Q2, const vo
                         int B, int H, int NQ, int NK, int d1, int d2, float c1, float c2, int causal, int splits,
                         float* kl_rows, float* lse1, float* lse2,
                         void* workspace, size_t workspace_bytes, streamkl_stream_t stream);
-/* Adaptive split selection, pure host arithmetic: P_base = B*H*ceil(NQ/256) CTAs of the default kernel;
- * returns 1 if P_base >= p_target, else min(floor(p_target/P_base), ceil(NK/64)).  p_target <= 0 means 148 = one CTA
+/* Adaptive split selection, pure host arithmetic: P_base = B*H*ceil(NQ/128) CTAs of the default kernel;
+ * returns 1 if P_base >= p_target, else min(floor(p_target/P_base), ceil(NK/128)).  p_target <= 0 means 148 = one CTA
  * per SM of a B200, i.e. one full wave (the paper's "typically 128 or 256" was for 108/132-SM parts). */
 int streamkl_fwd_splitk_splits(int B, int H, int NQ, int NK, int p_target);
 /* B*H*splits*5*NQ floats; 0 when splits <= 1. */

@@ -128,7 +128,7 @@ int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2
   p.sc2 = s.c2 * 1.4426950408889634f;
   p.kl = kl; p.lse1 = lse1; p.lse2 = lse2;
   const int TK = (s.NK + C::BK - 1) / C::BK;
-  p.chunk_steps = SPLIT ? (TK + splits - 1) / splits : TK;       // C_K = ceil(N_K / W), in whole 64-key steps
+  p.chunk_steps = SPLIT ? (TK + splits - 1) / splits : TK;       // C_K = ceil(N_K / W), in whole BK-key steps
   p.W = SPLIT ? (TK + p.chunk_steps - 1) / p.chunk_steps : 1;    // no empty trailing chunk
   p.part = part;
   const long long grid = (long long)p.TQ * s.BH * p.W;
@@ -471,8 +471,9 @@ int streamkl_fwd_splitk_splits(int B, int H, int NQ, int NK, int p_target) {
   // adaptive split selection: P_base = bsz * T_Q; W = 1 if P_base >= P_target, else min(floor(P_target / P_base), T_K)
   if (B <= 0 || H <= 0 || NQ <= 0 || NK <= 0) return 1;
   if (p_target <= 0) p_target = 148;   // one CTA per SM of a B200 = one full wave (measured best: profiles/r01d_splitk.md)
-  const long long p_base = (long long)B * H * ((NQ + 255) / 256);
-  const long long tk = (NK + 63) / 64;
+  using C = skl::FwdCfg<128, 128>;   // tile sizes of the forward kernel (the same for every head-dim pair)
+  const long long p_base = (long long)B * H * ((NQ + C::BQ - 1) / C::BQ);
+  const long long tk = (NK + C::BK - 1) / C::BK;
   if (p_base >= p_target) return 1;
   const long long w = p_target / p_base;
   return int(w < tk ? w : tk);
@@ -487,7 +488,7 @@ int streamkl_fwd_splitk(const void* Q1, const void* K1, const void* Q2, const vo
                         float c1, float c2, int causal, int splits, float* kl_rows, float* lse1, float* lse2, void* workspace,
                         size_t workspace_bytes, streamkl_stream_t stream) {
   if (splits <= 0) splits = streamkl_fwd_splitk_splits(B, H, NQ, NK, 0);
-  const int tk = NK > 0 ? (NK + 63) / 64 : 1;
+  const int tk = NK > 0 ? (NK + skl::FwdCfg<128, 128>::BK - 1) / skl::FwdCfg<128, 128>::BK : 1;
   if (splits > tk) splits = tk;
   const bool tc = (d1 == 64 || d1 == 128) && (d2 == 64 || d2 == 128);
   if (!tc || splits <= 1)   // other head dims run the (unsplit) SIMT kernel; W = 1 is the default kernel

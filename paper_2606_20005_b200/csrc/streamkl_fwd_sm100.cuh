@@ -1,18 +1,18 @@
 // streamkl_fwd_sm100.cuh -- StreamKL forward (Algorithm 1) for sm_100a.
 //
-// One CTA owns 256 query rows of one (b,h) (two 128-row M-tiles) and streams 64-key tiles:
+// One CTA owns NMT 128-row M-tiles of one (b,h) and streams BK-key tiles, NMT * BK = 128 (STREAMKL_FWD_BK = 128: one
+// M-tile, 128-key steps, N=128 logit MMAs -- the default; 64: two M-tiles sharing 64-key tiles):
 //   warp 0      TMA producer : Q1,Q2 once; K1_j,K2_j through an NSTAGE ring          (F1, F2 of DESIGN.md)
 //   warp 1      MMA issuer   : S1 = Q1 K1_j^T, S2 = Q2 K2_j^T, tcgen05.mma -> TMEM    (F3)
 //   warp 2      TMEM allocator
-//   warps 4-19  sixteen softmax warps = 2 M-tiles x 2 column halves x 4 TMEM lane quarters          (F4, F5, F6)
-// TMEM (512 columns): per M-tile two stages of {S1 (64 cols), S2 (64 cols)}.  A softmax thread owns ONE query row and
-// ONE 32-column half of every key tile: it pulls its 32+32 logits into registers, releases the TMEM stage at once (so
+//   warps 4-19  sixteen softmax warps = NMT M-tiles x BK/32 column groups x 4 TMEM lane quarters    (F4, F5, F6)
+// TMEM (512 columns): per M-tile two stages of {S1 (BK cols), S2 (BK cols)}.  A softmax thread owns ONE query row and
+// ONE 32-column group of every key tile: it pulls its 32+32 logits into registers, releases the TMEM stage at once (so
 // the next tile's MMA overlaps the exp work) and performs the online update of its own partial (m1,l1,m2,l2,acc) --
-// Eq.9-10 -- entirely thread-locally in the log2 domain (exp2 instead of exp; R6).  The two
-// column halves of a row are independent partial statistics over disjoint key sets; they are merged once, after the
+// Eq.9-10 -- entirely thread-locally in the log2 domain (exp2 instead of exp; R6).  The
+// column groups of a row are independent partial statistics over disjoint key sets; they are merged once, after the
 // last tile, with the associative merge of Eq.11 (carrying (m2,l2) too: R11).  Four softmax warps per
-// SM sub-partition (instead of two) keep the MUFU pipe fed while other warps sit in their no-exp phases (TMEM load,
-// running-max reduction): DESIGN.md "forward kernel".
+// SM sub-partition keep the MUFU pipe fed while other warps sit in their no-exp phases (TMEM load, barrier waits).
 #pragma once
 #include <cuda_bf16.h>
 #include <math_constants.h>
@@ -27,6 +27,13 @@
 
 // 1: unmasked tiles are evaluated against the row's current reference and the row maximum is only recomputed when a
 // tile sum shows the reference is stale (online_update_lazy); 0: Alg.1 literally (row maximum every tile).
+// Keys per step = N of the logit MMAs.  64: two 128-row M-tiles per CTA share every K tile (half the L2->SM traffic), but
+// an N=64 SS MMA is shared-memory-bound at 48 cycles instead of 32.  128: one M-tile per CTA, N=128 MMAs at
+// the full tensor rate.
+#ifndef STREAMKL_FWD_BK
+#define STREAMKL_FWD_BK 128
+#endif
+
 #ifndef STREAMKL_FWD_LAZY_MAX
 #define STREAMKL_FWD_LAZY_MAX 1
 #endif
@@ -37,9 +44,10 @@ template <int D1, int D2>
 struct FwdCfg {
   static_assert(D1 % 64 == 0 && D2 % 64 == 0 && D1 <= 128 && D2 <= 128, "tcgen05 path: d in {64,128}");
   static constexpr int BM = 128;             // rows per M-tile (TMEM lanes)
-  static constexpr int NMT = 2;              // M-tiles per CTA
+  static constexpr int BK = STREAMKL_FWD_BK; // keys per step = N of the logit MMAs
+  static_assert(BK == 64 || BK == 128, "TMEM holds 2 stages x {S1,S2} x BK columns for NMT M-tiles: NMT * BK = 128");
+  static constexpr int NMT = 128 / BK;       // M-tiles per CTA
   static constexpr int BQ = BM * NMT;        // query rows per CTA
-  static constexpr int BK = 64;              // keys per step
   static constexpr int KB1 = D1 / 64, KB2 = D2 / 64;  // 128-byte K-blocks per row
   static constexpr int QBLK = BM * 128;      // bytes of one [128 rows x 64 bf16] swizzled block
   static constexpr int KBLK = BK * 128;      // bytes of one [64 rows x 64 bf16] swizzled block
@@ -51,14 +59,15 @@ struct FwdCfg {
   static constexpr int NSTAGE = NSTAGE_RAW > 6 ? 6 : NSTAGE_RAW;
   static_assert(NSTAGE >= 2, "need at least a double-buffered K ring");
   static constexpr int SMEM_BYTES = 1024 + Q_BYTES + NSTAGE * STAGE_BYTES + AUX_BYTES;
-  static constexpr int NHALF = 2;            // column halves of a key tile (one softmax thread per row and half)
-  static constexpr int BC = BK / NHALF;      // columns per softmax thread and step
+  static constexpr int NHALF = BK / 32;      // column groups of a key tile (one softmax thread per row and group)
+  static constexpr int BC = BK / NHALF;      // columns per softmax thread and step (32)
   static constexpr int THREADS = 128 + NMT * NHALF * 128;
+  static_assert(THREADS == 640, "sixteen softmax warps");
   static constexpr uint32_t TMEM_COLS = 512;
 };
 
 struct FwdParams {
-  int NQ, NK, TQ;       // TQ = number of 256-row super tiles per head
+  int NQ, NK, TQ;       // TQ = number of BQ-row CTA tiles per head
   int BH;
   float sc1, sc2;       // c_t * log2(e)
   float* kl;
@@ -231,9 +240,9 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
   const int j_begin = SPLIT ? wk * p.chunk_steps : 0;        // this CTA's 64-key steps are [j_begin, j_begin + nsteps_mt)
   const int j_end = SPLIT ? min(TK, j_begin + p.chunk_steps) : TK;
 
-  int nsteps_mt[2];
+  int nsteps_mt[2] = {0, 0};
 #pragma unroll
-  for (int mt = 0; mt < 2; ++mt) {
+  for (int mt = 0; mt < C::NMT; ++mt) {
     const int r0 = q0 + mt * C::BM;
     int n = j_end;
     if (CAUSAL) {
@@ -312,8 +321,8 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
         if (j < nsteps_mt[mt]) {
           mbar_wait(&s_empty[mt * 2 + st], sph ^ 1);
           tc_fence_after();
-          const uint32_t dS1 = tmem_base + (mt * 2 + st) * 128;
-          const uint32_t dS2 = dS1 + 64;
+          const uint32_t dS1 = tmem_base + (mt * 2 + st) * (2 * C::BK);
+          const uint32_t dS2 = dS1 + C::BK;
           // Per-step descriptor bases, laundered through an empty asm so that the sixteen A descriptors are formed
           // as base + immediate next to each MMA instead of being hoisted out of the loop (32 loop-invariant 64-bit
           // values would not fit this warp's register budget: ptxas spilled them and the issue loop, not the tensor
@@ -347,8 +356,8 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
     reg_alloc<112>();    // needs 16*512 = 8192 registers from the pool the other warpgroup released
     const int sw = warp - 4;
     const int quarter = warp & 3;          // TMEM lane quarter this warp may access
-    const int mt = (sw >> 2) & 1;
-    const int half = sw >> 3;              // which 32-column half of every key tile
+    const int mt = (sw >> 2) % C::NMT;
+    const int half = (sw >> 2) / C::NMT;   // which 32-column group of every key tile (0 .. NHALF-1)
     const int rloc = quarter * 32 + lane;
     const int row = q0 + mt * C::BM + rloc;
     const int limit = CAUSAL ? min(p.NK - 1, row + off) : p.NK - 1;  // last visible key of this row
@@ -360,7 +369,7 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
       const uint32_t sph = (j >> 1) & 1;
       mbar_wait(&s_full[mt * 2 + sg], sph);
       tc_fence_after();
-      const uint32_t taddr = tmem_base + (uint32_t(quarter * 32) << 16) + (mt * 2 + sg) * 128 + half * C::BC;
+      const uint32_t taddr = tmem_base + (uint32_t(quarter * 32) << 16) + (mt * 2 + sg) * (2 * C::BK) + half * C::BC;
       uint32_t r1[C::BC], r2[C::BC];
       tmem_ld32(taddr, r1);
       tmem_ld32(taddr + C::BK, r2);
@@ -378,17 +387,30 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
 #endif
     }
     if (n > 0) {
-      // merge the two column halves of each row (Eq.11 with (m2,l2) carried too, R11).  The exchange buffer aliases this
+      // merge the column groups of each row (Eq.11 with (m2,l2) carried too, R11).  The exchange buffer aliases this
       // M-tile's own Q1 block: every MMA that reads it has completed (the last s_full of this M-tile has been observed).
       float* xch = reinterpret_cast<float*>(sQ1 + mt * C::KB1 * C::QBLK);
-      if (half == 1) {
-        xch[0 * C::BM + rloc] = st.m1; xch[1 * C::BM + rloc] = st.l1; xch[2 * C::BM + rloc] = st.m2;
-        xch[3 * C::BM + rloc] = st.l2; xch[4 * C::BM + rloc] = st.acc;
+      if (half > 0) {
+        float* x = xch + (half - 1) * 5 * C::BM;
+        x[0 * C::BM + rloc] = st.m1; x[1 * C::BM + rloc] = st.l1; x[2 * C::BM + rloc] = st.m2;
+        x[3 * C::BM + rloc] = st.l2; x[4 * C::BM + rloc] = st.acc;
       }
-      asm volatile("bar.sync %0, 256;" ::"r"(1 + mt) : "memory");
+      asm volatile("bar.sync %0, %1;" ::"r"(1 + mt), "n"(C::NHALF * 128) : "memory");
       if (half == 0 && row < p.NQ) {
-        const float m1b = xch[0 * C::BM + rloc], l1b = xch[1 * C::BM + rloc], m2b = xch[2 * C::BM + rloc];
-        const float l2b = xch[3 * C::BM + rloc], accb = xch[4 * C::BM + rloc];
+#pragma unroll
+        for (int hb = 1; hb < C::NHALF - 1; ++hb) {   // fold groups 1 .. NHALF-2 into this thread's state; the last one below
+          const float* x = xch + (hb - 1) * 5 * C::BM;
+          const float m1b = x[0 * C::BM + rloc], l1b = x[1 * C::BM + rloc], m2b = x[2 * C::BM + rloc];
+          const float l2b = x[3 * C::BM + rloc], accb = x[4 * C::BM + rloc];
+          const float m1 = fmaxf(st.m1, m1b), m2 = fmaxf(st.m2, m2b);
+          const float r1 = (m1 == -CUDART_INF_F) ? 0.f : m1, r2 = (m2 == -CUDART_INF_F) ? 0.f : m2;
+          const float wa1 = exp2f(st.m1 - r1), wb1 = exp2f(m1b - r1), wa2 = exp2f(st.m2 - r2), wb2 = exp2f(m2b - r2);
+          st.l1 = st.l1 * wa1 + l1b * wb1; st.l2 = st.l2 * wa2 + l2b * wb2; st.acc = st.acc * wa1 + accb * wb1;
+          st.m1 = m1; st.m2 = m2;
+        }
+        const float* xl = xch + (C::NHALF - 2) * 5 * C::BM;
+        const float m1b = xl[0 * C::BM + rloc], l1b = xl[1 * C::BM + rloc], m2b = xl[2 * C::BM + rloc];
+        const float l2b = xl[3 * C::BM + rloc], accb = xl[4 * C::BM + rloc];
         const float m1 = fmaxf(st.m1, m1b), m2 = fmaxf(st.m2, m2b);
         // unsplit: half 0 holds key 0, so the maxima are finite.  A split-K chunk can lie wholly past a row's causal
         // frontier: both halves are then (-inf, 0, 0) and the reference is 0 (R7), giving the identity partial.

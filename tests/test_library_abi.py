@@ -118,8 +118,8 @@ def test_splitk_adaptive_split_selection_follows_the_paper_rule(L):
     assert f(1, 16, 1, 131072, 256) == 16            # P_base = 16 -> floor(256/16)
     assert f(1, 16, 64, 131072, 128) == 8
     assert f(4, 64, 16, 131072, 256) == 1            # P_base = 256 >= P_target: default kernel
-    assert f(1, 1, 1, 200, 256) == 4                 # clamped by T_K = ceil(200/64)
-    assert f(1, 16, 300, 8192, 256) == 8             # T_Q = ceil(300/256) = 2 -> P_base = 32
+    assert f(1, 1, 1, 200, 256) == 2                 # clamped by T_K = ceil(200/128)
+    assert f(1, 16, 300, 8192, 256) == 5             # T_Q = ceil(300/128) = 3 -> P_base = 48
     assert f(1, 16, 16, 65536, 0) == 9               # default target: 148 CTAs = one per SM
     assert f(0, 16, 16, 65536, 0) == 1
 

@@ -1,6 +1,6 @@
 """GPU parity of the split-K forward (Eq.11) against the float64 definition, element by element:
 small N_Q (the regime it exists for), long and ragged N_K, every head-dim pair, causal and not, split counts from 2 to
-one chunk per 64-key tile (incl. chunks that lie wholly past a row's causal frontier), and the adaptive choice."""
+one chunk per key tile (incl. chunks that lie wholly past a row's causal frontier), and the adaptive choice."""
 from __future__ import annotations
 
 import numpy as np
@@ -44,7 +44,7 @@ def test_splitk_head_dim_pairs(d1, d2):
 
 @pytest.mark.parametrize("splits", [2, 3, 1000])
 def test_splitk_split_counts_up_to_one_tile_per_chunk(splits):
-    """splits=1000 is clamped to ceil(NK/64) chunks of one 64-key step each; causal rows then meet empty chunks."""
+    """splits=1000 is clamped to one chunk per key tile; causal rows then meet empty chunks."""
     run_splitk(W.Config(62, "splitk-w", 1, 2, 48, 1024 + 40, 128, 64, "bf16", True), splits)
 
 
