@@ -32,6 +32,21 @@
 
 #include "sm100_ptx.cuh"
 
+// Share of the backward's exps evaluated by the FMA-pipe polynomial (ex2_poly2): one column pair in every N (0 = none),
+// per kernel flavour.  Measured on B200: the student-only kernels are MUFU-bound (their tensor work is
+// light) and gain 7-10 % from a quarter of the exps on the FMA pipe.  With teacher gradients the K owner alone gains
+// (62.4 -> 57.3 ms on cfg 4) but draws more power, and under the 1000 W cap the forward and the Q owner then lose what it
+// won (step 164.0 vs 163.8-165.6 ms): off.
+#ifndef STREAMKL_BWD_POLY_STUDENT
+#define STREAMKL_BWD_POLY_STUDENT 4
+#endif
+#ifndef STREAMKL_BWD_POLY_TEACHER_K
+#define STREAMKL_BWD_POLY_TEACHER_K 0
+#endif
+#ifndef STREAMKL_BWD_POLY_TEACHER_Q
+#define STREAMKL_BWD_POLY_TEACHER_Q 0
+#endif
+
 namespace skl {
 
 template <int D1, int D2, bool TEACHER>
@@ -144,8 +159,11 @@ __device__ __forceinline__ void ds_row(const uint32_t (&r1)[NC], const uint32_t 
     }
     const float2 x1 = fma2(make_float2(__uint_as_float(r1[e]), __uint_as_float(r1[e + 1])), vsc1, vn1);
     const float2 x2 = fma2(make_float2(__uint_as_float(r2[e]), __uint_as_float(r2[e + 1])), vsc2, vn2);
-    const float2 p1 = make_float2(ex2_approx(x1.x), ex2_approx(x1.y));   // P1 = exp(s1 - lse1)   (Alg.2 line 7)
-    const float2 p2 = make_float2(ex2_approx(x2.x), ex2_approx(x2.y));
+    // P_t = exp(s_t - lse_t) (Alg.2 line 7); one column pair in every STREAMKL_BWD_POLY_EVERY on the FMA/ALU pipes
+    constexpr int PE = TEACHER ? (OWNER_K ? STREAMKL_BWD_POLY_TEACHER_K : STREAMKL_BWD_POLY_TEACHER_Q) : STREAMKL_BWD_POLY_STUDENT;
+    const bool poly = PE > 0 && ((e >> 1) % (PE > 0 ? PE : 1)) == 0;
+    const float2 p1 = poly ? ex2_poly2(x1) : make_float2(ex2_approx(x1.x), ex2_approx(x1.y));
+    const float2 p2 = poly ? ex2_poly2(x2) : make_float2(ex2_approx(x2.x), ex2_approx(x2.y));
     float2 a2 = sub2(p2, p1);                                            // dS2 / g (Alg.2 line 8): fp32 subtract, rounded once below
     if constexpr (OWNER_K) a2 = mul2(a2, vg);
     float2 a1 = make_float2(0.f, 0.f);
