@@ -39,7 +39,8 @@ struct ProfScope {  // brackets ONE kernel launch; a no-op unless profiling is e
     if (!g_prof_on) return;
     if (!g_prof) g_prof = new std::vector<ProfRecord>();
     cudaEvent_t a = nullptr;
-    if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { cudaGetLastError(); b = nullptr; return; }
+    if (cudaEventCreate(&a) != cudaSuccess) { cudaGetLastError(); return; }
+    if (cudaEventCreate(&b) != cudaSuccess) { cudaGetLastError(); cudaEventDestroy(a); b = nullptr; return; }
     cudaEventRecord(a, st);
     g_prof->push_back({id, a, b});
   }
@@ -271,6 +272,13 @@ int launch_bwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2
   return STREAMKL_OK;
 }
 
+// Strategy selection of the Setting-1 backward (see bwd_tc_both): the one-visit kernel iff no teacher gradients are wanted and
+// the mode is FUSED, or AUTO with at most four 128-query tiles per head.  streamkl_bwd_workspace_bytes applies the same rule,
+// so the fp32 dQ2 accumulator is only asked for when the strategy that will run needs it.
+bool bwd_fused_selected(int NQ, bool teacher) {
+  return !teacher && (g_bwd_mode == STREAMKL_BWD_FUSED || (g_bwd_mode == STREAMKL_BWD_AUTO && (NQ + 127) / 128 <= 4));
+}
+
 size_t stats_bytes_aligned(long long BH, int NQ) { return (size_t(BH) * size_t(skl::bwd_stats_padded_rows(NQ)) * 16 + 255) & ~size_t(255); }
 
 // Setting 1 in one visit: zero the fp32 dQ2 accumulator, run the fused K-owner kernel, convert dQ2.
@@ -335,7 +343,7 @@ int bwd_tc_both(const void* Q1, const void* K1, const void* Q2, const void* K2, 
   // (profiles/r01f_fused_bwd.md): the one-visit kernel wins 1.3-3.0x while the Q-owner grid is small (T_Q <= 4 tiles of 128
   // queries), is level at T_Q = 8 and loses a few per cent beyond, where its fp32 atomics (64 KB per 128x128 tile pair)
   // run into the L2's atomic throughput; the crossover did not move with T_K (128 vs 1024), so the rule is on T_Q alone.
-  const bool fused = !t && (g_bwd_mode == STREAMKL_BWD_FUSED || (g_bwd_mode == STREAMKL_BWD_AUTO && (s.NQ + 127) / 128 <= 4));
+  const bool fused = bwd_fused_selected(s.NQ, t);
   if (fused) {   // Setting 1: one visit, dQ2 through fp32 atomics
     float* dq_acc = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) + stats_bytes_aligned(s.BH, s.NQ));
     return s.causal ? launch_bwd_fused<D1, D2, true>(Q1, K1, Q2, K2, s, stats, dq_acc, dQ2, dK2, st)
@@ -507,8 +515,8 @@ size_t streamkl_bwd_workspace_bytes(int B, int H, int NQ, int, int d1, int d2, i
   if (B <= 0 || H <= 0 || NQ <= 0) return 0;
   if (!((d1 == 64 || d1 == 128) && (d2 == 64 || d2 == 128))) return 0;
   const long long BH = (long long)B * H;
-  if (want_teacher) return size_t(BH) * size_t(skl::bwd_stats_padded_rows(NQ)) * 16;
-  // Setting 1: + the fp32 dQ2 accumulator of the one-visit kernel (O(NQ d2)), whatever mode is selected at call time
+  if (!bwd_fused_selected(NQ, want_teacher != 0)) return size_t(BH) * size_t(skl::bwd_stats_padded_rows(NQ)) * 16;
+  // one-visit Setting-1 kernel (mode FUSED, or AUTO with NQ <= 512): + its fp32 dQ2 accumulator, O(NQ d2)
   return stats_bytes_aligned(BH, NQ) + size_t(BH) * size_t(NQ) * size_t(d2) * sizeof(float);
 }
 
@@ -554,7 +562,7 @@ int streamkl_fwd_bwd_host(int dtype, const void* Q1, const void* K1, const void*
   const long long BH = s.BH;
   long long gs = BH;   // heads per group
   if (BH > 1 && (size_t(d1) * es) % 16 == 0 && (size_t(d2) * es) % 16 == 0 && size_t(BH) * (hq1 + hk1 + hq2 + hk2) >= (64u << 20)) {
-    const long long tq = (NQ + 255) / 256;
+    const long long tq = (NQ + skl::FwdCfg<128, 128>::BQ - 1) / skl::FwdCfg<128, 128>::BQ;   // forward CTAs per head
     const long long fill = (2 * 148 + tq - 1) / (tq > 0 ? tq : 1);   // enough CTAs per launch for two waves
     gs = (BH + 7) / 8;
     if (gs < fill) gs = fill;

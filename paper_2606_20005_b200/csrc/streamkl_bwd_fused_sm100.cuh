@@ -276,7 +276,9 @@ streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const 
       if (lane == 0) mbar_arrive(&s_empty[par]);
       if (last >= 0) drain(last);             // the previous step of this group: its dQ2^T MMAs have had a whole step to finish
       const int y0 = j * C::BY + half * 32;
-      const bool masked = CAUSAL && (y0 + off < x0 + C::BX - 1);
+      // warp-uniform: causal diagonal blocks, and the owner tile's KEY tail (TMA zero-fills those rows, P = exp2(0 - lse) may
+      // be inf there, and unlike the separate K-owner kernel this kernel CONTRACTS over the owned keys: dQ2^T = K2^T dS2)
+      const bool masked = (CAUSAL && (y0 + off < x0 + C::BX - 1)) || (x0 + C::BX > p.NK);
       const uint32_t stat = stat_base + s * C::STAT_STAGE;
       if (masked) ds_row<32, false, true, CAUSAL, true>(r1, r2, o1, o2, sc1, sc2, 0.f, 0.f, 0.f, stat, xrow, y0, off, p.NK);
       else        ds_row<32, false, true, CAUSAL, false>(r1, r2, o1, o2, sc1, sc2, 0.f, 0.f, 0.f, stat, xrow, y0, off, p.NK);

@@ -174,7 +174,7 @@ __device__ __forceinline__ void ds_row(const uint32_t (&r1)[NC], const uint32_t 
     if constexpr (MASKED) {
       const int y = y0 + e;
       bool ok0, ok1;
-      if constexpr (OWNER_K) { ok0 = !CAUSAL || xrow <= y + off; ok1 = !CAUSAL || xrow <= y + 1 + off; }
+      if constexpr (OWNER_K) { ok0 = (xrow < NK) && (!CAUSAL || xrow <= y + off); ok1 = (xrow < NK) && (!CAUSAL || xrow <= y + 1 + off); }
       else { ok0 = (y < NK) && (!CAUSAL || y <= xrow + off); ok1 = (y + 1 < NK) && (!CAUSAL || y + 1 <= xrow + off); }
       a2.x = ok0 ? a2.x : 0.f; a2.y = ok1 ? a2.y : 0.f;
       a1.x = ok0 ? a1.x : 0.f; a1.y = ok1 ? a1.y : 0.f;

@@ -3,7 +3,8 @@
 Tolerances (bf16 inputs, fp32 accumulation; R17 applies the same numbers to fp32 inputs):
   per-row KL   |err| <= 2e-3 + 1e-2*|ref|
   lse          |err| <= 1e-3
-  gradients    cosine similarity >= 0.999 and max|g - ref| / max|ref| <= 3e-2   (R16: per tensor)
+  gradients    cosine similarity >= 0.999 and max|g - ref| / max|ref| <= 3e-2   (R16), evaluated PER (batch, head):
+               a head with small gradients must not hide behind a head with large ones (check_grad_heads)
 """
 from __future__ import annotations
 
@@ -72,3 +73,20 @@ def check_grad(got, ref, what=""):
     assert cos >= GRAD_COS, f"{what}: cosine {cos:.6f} < {GRAD_COS}"
     assert rel <= GRAD_MAXREL, f"{what}: max|err|/max|ref| {rel:.3e} > {GRAD_MAXREL}"
     return cos, rel
+
+
+def check_grad_heads(got, ref, what=""):
+    """The gradient bars applied to every (batch, head) slice of [..., N, d] tensors separately; returns the worst
+    (min cosine, max relative error) over the heads."""
+    got = np.asarray(got, dtype=np.float64)
+    ref = np.asarray(ref, dtype=np.float64)
+    assert got.shape == ref.shape, f"{what}: shape {got.shape} vs {ref.shape}"
+    if got.ndim <= 2:
+        return check_grad(got, ref, what)
+    g3 = got.reshape((-1,) + got.shape[-2:])
+    r3 = ref.reshape((-1,) + ref.shape[-2:])
+    worst_cos, worst_rel = 1.0, 0.0
+    for i in range(g3.shape[0]):
+        cos, rel = check_grad(g3[i], r3[i], f"{what} [head {i}]")
+        worst_cos, worst_rel = min(worst_cos, cos), max(worst_rel, rel)
+    return worst_cos, worst_rel

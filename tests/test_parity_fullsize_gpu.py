@@ -3,9 +3,12 @@ shapes, whole batch in one call), against the float64 oracle on outputs the orac
 
   * kl / lse1 / lse2 / dQ rows: a sample of query rows per sampled head (first, last, every 128/256-row tile boundary
     +-1 near both ends, seeded random rows) -- `attention_kl_rows` is exact for any row subset.
-  * dK: exact where a bounded row set determines it -- the whole head for cfg 2/3/5 (one head each), and for cfg 4 the
-    last 1024 keys of a head (under the causal mask only the last 1024 query rows see them, so 1024 oracle rows give
-    those dK rows exactly: interior tiles, the masked diagonal tiles and the tail of the K-owner loop).
+  * dK: the whole head for cfg 2/3/5 (one head each).  cfg 4 (the bench workload; ">= 2 whole heads, first
+    and last -- needed for dK, which sums over all rows"): heads 0 and 31 in full -- every kl / lse / dQ row and all of
+    dK1, dK2, i.e. also the early key tiles whose K-owner CTAs stream all 1024 query tiles.  The oracle is called block by
+    block on the causal prefix the block can see (rows r0..r1-1 of a causal NQ = NK head see keys < r1 only: passing
+    Q[:r1], K[:r1] to the unmodified definition gives the same rows and the same dK contributions, the masked remainder
+    contributes exact zeros), several blocks at a time on the host's threads.
   * properties that hold at any size, on EVERY head: all outputs finite, KL >= -2e-3 (R14), column sums of dK vanish
     (sum_j dS[i,j] = 0 per row).
 Tolerances are parity_util's (BASELINE.json north_star).
@@ -103,7 +106,50 @@ def whole_head_dk(cfg, head_inp, hidx, dK1, dK2):
         assert cos >= GRAD_COS and rel <= GRAD_MAXREL, f"cfg{cfg.idx} head {hidx} {name}: cos {cos:.6f} rel {rel:.3e}"
 
 
-def fullsize_case(idx: int, row_heads, n_random: int, dk_whole_head=None, dk_tail_rows: int = 0):
+def whole_head_causal_by_prefix_blocks(cfg, head_inp, hidx, kl, l1, l2, dQ1, dK1, dQ2, dK2, row_block=256, workers=8):
+    """Every output of head `hidx` of a causal NQ = NK config against the definition (see the module docstring)."""
+    import torch
+
+    assert cfg.causal and cfg.NQ == cfg.NK
+    Q1, K1, Q2, K2 = (W.widen_f64(head_inp[k]) for k in ("Q1", "K1", "Q2", "K2"))
+    g = head_inp["g"].astype(np.float64)
+    N = cfg.NQ
+    ref = {"kl": np.empty(N), "lse1": np.empty(N), "lse2": np.empty(N), "dQ2": np.empty((N, cfg.d2)), "dK2": np.zeros((N, cfg.d2))}
+    if cfg.teacher_grads:
+        ref["dQ1"] = np.empty((N, cfg.d1))
+        ref["dK1"] = np.zeros((N, cfg.d1))
+
+    def block(r0):
+        r1 = min(N, r0 + row_block)
+        rows = np.arange(r0, r1)
+        return r0, r1, attention_kl_rows(Q1[:r1], K1[:r1], Q2[:r1], K2[:r1], cfg.c1, cfg.c2, True, rows, g[:r1], cfg.teacher_grads)
+
+    with ThreadPoolExecutor(max_workers=workers) as ex:
+        for r0, r1, part in ex.map(block, range(0, N, row_block)):
+            for k in ("kl", "lse1", "lse2", "dQ2") + (("dQ1",) if cfg.teacher_grads else ()):
+                ref[k][r0:r1] = part[k]
+            ref["dK2"][:r1] += part["dK2_part"]
+            if cfg.teacher_grads:
+                ref["dK1"][:r1] += part["dK1_part"]
+    b, h = divmod(hidx, cfg.H)
+    got_kl, got_l1, got_l2 = (to_f64(t[b, h]) for t in (kl, l1, l2))
+    assert np.abs(got_l1 - ref["lse1"]).max() <= LSE_ATOL, f"cfg{cfg.idx} head {hidx}: lse1 (all rows)"
+    assert np.abs(got_l2 - ref["lse2"]).max() <= LSE_ATOL, f"cfg{cfg.idx} head {hidx}: lse2 (all rows)"
+    assert (np.abs(got_kl - ref["kl"]) <= KL_ATOL + KL_RTOL * np.abs(ref["kl"])).all(), f"cfg{cfg.idx} head {hidx}: kl (all rows)"
+    res = {}
+    for name, t in (("dQ2", dQ2), ("dK2", dK2), ("dQ1", dQ1), ("dK1", dK1)):
+        if t is None:
+            continue
+        cos, rel = grad_metrics(to_f64(t[b, h]), ref[name])
+        assert cos >= GRAD_COS and rel <= GRAD_MAXREL, f"cfg{cfg.idx} head {hidx} {name} (whole head): cos {cos:.6f} rel {rel:.3e}"
+        if name.startswith("dK"):   # the longest K-owner loops: the first key tiles, seen by every query row
+            cos, rel = grad_metrics(to_f64(t[b, h][:256]), ref[name][:256])
+            assert cos >= GRAD_COS and rel <= GRAD_MAXREL, f"cfg{cfg.idx} head {hidx} {name} first 256 keys: cos {cos:.6f} rel {rel:.3e}"
+        res[name] = (cos, rel)
+    return res
+
+
+def fullsize_case(idx: int, row_heads, n_random: int, dk_whole_head=None, dk_tail_rows: int = 0, whole_heads=()):
     cfg = W.CONFIGS[idx]
     inp, per = gen_all(cfg)
     kl, l1, l2, dQ1, dK1, dQ2, dK2 = run_gpu(cfg, inp)
@@ -112,6 +158,8 @@ def fullsize_case(idx: int, row_heads, n_random: int, dk_whole_head=None, dk_tai
         check_rows(cfg, per[hidx], hidx, sample_rows(cfg.NQ, n_random, 1000 * idx + hidx), kl, l1, l2, dQ1, dQ2)
     if dk_whole_head is not None:
         whole_head_dk(cfg, per[dk_whole_head], dk_whole_head, dK1, dK2)
+    for hidx in whole_heads:
+        whole_head_causal_by_prefix_blocks(cfg, per[hidx], hidx, kl, l1, l2, dQ1, dK1, dQ2, dK2)
     if dk_tail_rows:
         assert cfg.causal and cfg.NQ == cfg.NK
         hidx = row_heads[-1]
@@ -140,8 +188,9 @@ def test_cfg3_fullsize():
 
 
 def test_cfg4_fullsize():
-    """B=1,H=32,65536^2,d=128/128,causal (the bench workload): rows of heads 0 and 31, dK of the last 1024 keys of head 31."""
-    fullsize_case(4, row_heads=[0, 31], n_random=40, dk_tail_rows=1024)
+    """B=1,H=32,65536^2,d=128/128,causal (the bench workload): sampled rows of heads 7 and 20; heads 0 and 31 WHOLE (every
+    kl/lse/dQ row, all of dK1 and dK2 -- SURVEY 8(c) C4), plus the global properties on every head."""
+    fullsize_case(4, row_heads=[7, 20], n_random=40, whole_heads=(0, 31))
 
 
 def test_cfg5_fullsize():

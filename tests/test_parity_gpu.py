@@ -8,7 +8,7 @@ import pytest
 
 import workloads as W
 from oracle.streamkl_oracle import attention_kl
-from parity_util import bits_to_f64, check_fwd, check_grad, to_f64, to_torch
+from parity_util import bits_to_f64, check_fwd, check_grad, check_grad_heads, to_f64, to_torch
 
 pytestmark = pytest.mark.gpu
 
@@ -30,11 +30,11 @@ def run_case(cfg: W.Config, teacher=None, check_bwd=True):
         return stats
     dQ1, dK1, dQ2, dK2 = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, cfg.causal, kl, l1, l2, g, teacher=teacher)
     assert skl.streamkl_last_launch_count() >= 1
-    check_grad(to_f64(dQ2), ref["dQ2"], cfg.name + " dQ2")
-    check_grad(to_f64(dK2), ref["dK2"], cfg.name + " dK2")
+    check_grad_heads(to_f64(dQ2), ref["dQ2"], cfg.name + " dQ2")
+    check_grad_heads(to_f64(dK2), ref["dK2"], cfg.name + " dK2")
     if teacher:
-        check_grad(to_f64(dQ1), ref["dQ1"], cfg.name + " dQ1")
-        check_grad(to_f64(dK1), ref["dK1"], cfg.name + " dK1")
+        check_grad_heads(to_f64(dQ1), ref["dQ1"], cfg.name + " dQ1")
+        check_grad_heads(to_f64(dK1), ref["dK1"], cfg.name + " dK1")
     else:
         assert dQ1 is None and dK1 is None
     return stats
@@ -242,8 +242,8 @@ def test_setting1_fused_and_separate_strategies_agree_with_the_oracle(d1, d2, ca
         for mode in (skl.STREAMKL_BWD_FUSED, skl.STREAMKL_BWD_SEPARATE):
             skl.streamkl_set_bwd_mode(mode)
             _, _, dQ2, dK2 = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, cfg.causal, kl, l1, l2, g, teacher=False)
-            check_grad(to_f64(dQ2), ref["dQ2"], f"mode {mode} dQ2")
-            check_grad(to_f64(dK2), ref["dK2"], f"mode {mode} dK2")
+            check_grad_heads(to_f64(dQ2), ref["dQ2"], f"mode {mode} dQ2")
+            check_grad_heads(to_f64(dK2), ref["dK2"], f"mode {mode} dK2")
             res[mode] = (to_f64(dQ2), to_f64(dK2), skl.streamkl_last_launch_count())
     finally:
         skl.streamkl_set_bwd_mode(skl.STREAMKL_BWD_AUTO)
@@ -265,8 +265,8 @@ def test_setting1_fused_mixed_sign_upstream_gradient_and_tiny_sizes():
         ref = attention_kl(*(bits_to_f64(inp[k]) for k in ("Q1", "K1", "Q2", "K2")), cfg.c1, cfg.c2, False, g=gnp.astype(np.float64), teacher=False)
         kl, l1, l2 = skl.streamkl_fwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, False)
         _, _, dQ2, dK2 = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, False, kl, l1, l2, torch.from_numpy(gnp).cuda(), teacher=False)
-        check_grad(to_f64(dQ2), ref["dQ2"], f"{NQ}x{NK} dQ2")
-        check_grad(to_f64(dK2), ref["dK2"], f"{NQ}x{NK} dK2")
+        check_grad_heads(to_f64(dQ2), ref["dQ2"], f"{NQ}x{NK} dQ2")
+        check_grad_heads(to_f64(dK2), ref["dK2"], f"{NQ}x{NK} dK2")
 
 
 def test_one_million_keys_and_many_small_heads():
@@ -285,13 +285,13 @@ def test_one_million_keys_and_many_small_heads():
     check_fwd(to_f64(ks), to_f64(l1s), to_f64(l2s), ref, "1M split-K")
     dQ1, dK1, dQ2, dK2 = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, False, kl, l1, l2, g, teacher=True)
     for name, t in (("dQ1", dQ1), ("dK1", dK1), ("dQ2", dQ2), ("dK2", dK2)):
-        check_grad(to_f64(t), ref[name], "1M " + name)
+        check_grad_heads(to_f64(t), ref[name], "1M " + name)
     try:
         for mode in (skl.STREAMKL_BWD_FUSED, skl.STREAMKL_BWD_SEPARATE):
             skl.streamkl_set_bwd_mode(mode)
             _, _, dQ2, dK2 = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, False, kl, l1, l2, g, teacher=False)
-            check_grad(to_f64(dQ2), ref["dQ2"], f"1M mode {mode} dQ2")
-            check_grad(to_f64(dK2), ref["dK2"], f"1M mode {mode} dK2")
+            check_grad_heads(to_f64(dQ2), ref["dQ2"], f"1M mode {mode} dQ2")
+            check_grad_heads(to_f64(dK2), ref["dK2"], f"1M mode {mode} dK2")
     finally:
         skl.streamkl_set_bwd_mode(skl.STREAMKL_BWD_AUTO)
     run_case(W.Config(47, "many-heads", 32, 32, 130, 190, 64, 128, "bf16", True))
