@@ -1,17 +1,19 @@
 #!/usr/bin/env python
 """bench.py -- StreamKL hot path on B200: one JSON line per run (driver contract).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4|cfg3|cfg2|cfg5] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4|cfg3|cfg2|cfg5] [--bwd-mode auto|separate|fused]
+                    [--impl reference]
 
 A "step" is ONE pass of the whole hot path over one batch of the workload: streamkl_fwd (F1-F6 of DESIGN.md) followed
 by streamkl_bwd (B1-B6; teacher gradients too where the config asks for them).  The default workload is BASELINE.json's
 64K configuration (configs[3]: B=1, H=32, NQ=NK=65536, d=128/128, bf16, causal), the larger of the two sizes the metric
-is quoted on; the 16K one (configs[2]) is timed beside it and reported under "also".
+is quoted on; the 16K one (configs[2]), cfg 2, cfg 5, a split-K shape and the backward-strategy table are timed beside it
+and reported under "also".
   value   = algorithmic TFLOP/s of the step (fwd 2*pairs*(d1+d2) + bwd 2*pairs*((d1+d2)+2*d2+2*d1), pairs = NQ*NK/2 causal),
             all ranks' work / max-over-ranks device time, inputs resident in HBM.
   e2e     = the same metric through streamkl_fwd_bwd_host: pinned HOST buffers, host<->device copies inside the timed region.
-  roofline= the dominant kernel's achieved tensor TFLOP/s (its algorithmic FLOPs / its average CUDA-event duration inside
-            the timed region) against the measured dense bf16 peak of MEASURED_PEAKS.json.
+  roofline= the dominant kernel's achieved tensor TFLOP/s (its algorithmic one-visit FLOPs / its average CUDA-event duration
+            inside the timed region; the executed FLOPs beside it) against the measured dense bf16 peak of MEASURED_PEAKS.json.
   cpu_baseline = the float64 oracle, as it stands, timed on this box's host cores on a bounded row sample of the workload.
 With N > 1 (torchrun) every rank runs its own batch of the same shape (heads are independent: no collective on the data
 path) -> "scaling": "weak".  `--impl reference` times the oracle alone (rank 0), same metric and config.
@@ -291,7 +293,7 @@ def time_passes(skl, cfg, dev, steps, warmup, barrier):
     barrier()
     torch.cuda.synchronize()
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
-    skl.streamkl_profile_enable(True)
+    skl.streamkl_profile_enable(max(2, 8 * steps))   # event pairs for every launch of the region, created now
     launches = 0
     ev[0].record()
     for _ in range(steps):
@@ -376,13 +378,70 @@ def kernel_hbm_bytes(cfg: W.Config, name: str) -> int:
 
 
 def kernel_flops(cfg: W.Config, name: str) -> float:
-    """Algorithmic tensor FLOPs ONE launch of kernel `name` performs ('Algorithmic work per kernel')."""
+    """EXECUTED tensor FLOPs of ONE launch of kernel `name`: every backward kernel recomputes both logit
+    tiles and runs the gradient GEMMs of what it differentiates (owner kernels: one per distribution; a one-visit pass: two)."""
     pairs = cfg.visible_pairs_convention()
     if "fwd" in name:
         return 2.0 * pairs * (cfg.d1 + cfg.d2)
     t = cfg.teacher_grads
-    # each backward kernel recomputes both logit tiles and runs one gradient GEMM per distribution it differentiates
+    if "fused" in name:   # averaged over the student pass (2 d2) and, with teacher gradients, the teacher pass (2 d1)
+        return 2.0 * pairs * ((cfg.d1 + cfg.d2) + (cfg.d2 + cfg.d1 if t else 2 * cfg.d2))
     return 2.0 * pairs * ((cfg.d1 + cfg.d2) + cfg.d2 + (cfg.d1 if t else 0))
+
+
+def kernel_flops_one_visit(cfg: W.Config, name: str, launches_of_bwd_kernels: float) -> float:
+    """SURVEY 8(d)'s ALGORITHMIC count credited to one launch: the gradient GEMMs it runs, plus its share of ONE logit
+    recomputation per tile pair -- the recompute is needed once per pair however many kernels repeat it, so it is split
+    evenly over the backward tensor-core launches of the step (two owner kernels: half each)."""
+    pairs = cfg.visible_pairs_convention()
+    if "fwd" in name:
+        return 2.0 * pairs * (cfg.d1 + cfg.d2)
+    return kernel_flops(cfg, name) - 2.0 * pairs * (cfg.d1 + cfg.d2) * (1.0 - 1.0 / max(1.0, launches_of_bwd_kernels))
+
+
+BWD_MODES = {"auto": 0, "separate": 1, "fused": 2}
+
+
+def time_bwd_strategies(skl, iters: int = 20):
+    """Backward strategy table (Fig.13): separate owner kernels vs the one-visit kernels,
+    both settings, small-to-medium N_Q, bsz 16, N_K = 16384, d = 128/128, no mask.  ms per streamkl_bwd call."""
+    import torch
+
+    out = {}
+    for NQ in (16, 128, 256, 512, 1024, 4096):
+        cfg = W.Config(71, "bwd-strategy", 1, 16, NQ, 16384, 128, 128, "bf16", False)
+        inp = W.all_inputs(cfg)
+        Q1, K1, Q2, K2 = (to_dev(inp[k]) for k in ("Q1", "K1", "Q2", "K2"))
+        g = to_dev(inp["g"])
+        kl, l1, l2 = skl.streamkl_fwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, False)
+        row = {}
+        for teacher in (False, True):
+            for mode in ("separate", "fused"):
+                skl.streamkl_set_bwd_mode(BWD_MODES[mode])
+                try:
+                    ws = torch.empty(max(1, skl.streamkl_bwd_workspace_bytes(cfg.B, cfg.H, NQ, cfg.NK, cfg.d1, cfg.d2, teacher)), dtype=torch.uint8, device="cuda")
+                    grads = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, False, kl, l1, l2, g, teacher=teacher, workspace=ws)
+
+                    def call():
+                        skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, False, kl, l1, l2, g, teacher=teacher, dQ1=grads[0], dK1=grads[1],
+                                         dQ2=grads[2], dK2=grads[3], workspace=ws)
+
+                    for _ in range(3):
+                        call()
+                    torch.cuda.synchronize()
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record()
+                    for _ in range(iters):
+                        call()
+                    b.record()
+                    torch.cuda.synchronize()
+                    row[f"{'setting2' if teacher else 'setting1'}_{mode}_ms"] = a.elapsed_time(b) / iters
+                finally:
+                    skl.streamkl_set_bwd_mode(BWD_MODES["auto"])
+        for st in ("setting1", "setting2"):
+            row[f"{st}_fused_speedup"] = row[f"{st}_separate_ms"] / row[f"{st}_fused_ms"]
+        out[f"NQ={NQ}"] = row
+    return {"shape": "bsz=16 (B=1,H=16), NK=16384, d=128/128, bf16, no mask", "auto_rule": "one-visit kernels iff NQ <= 512 (Setting 1) / NQ <= 256 (Setting 2)", "rows": out}
 
 
 def main():
@@ -392,7 +451,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="streamkl", choices=["streamkl", "reference"])
     ap.add_argument("--workload", default="cfg4", choices=sorted(WORKLOADS))
-    ap.add_argument("--no-also", action="store_true", help="skip the secondary 16K measurement")
+    ap.add_argument("--no-also", action="store_true", help="skip the secondary measurements (cfg3, cfg2, cfg5, split-K, strategy table)")
+    ap.add_argument("--bwd-mode", default="auto", choices=sorted(BWD_MODES), help="backward strategy of the timed step (streamkl_set_bwd_mode)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiling runs)")
     args = ap.parse_args()
@@ -422,6 +482,7 @@ def main():
             dist.barrier()
 
     pk = peaks()
+    skl.streamkl_set_bwd_mode(BWD_MODES[args.bwd_mode])
     host = gen_inputs(cfg, rank)
     dev = tuple(to_dev(host[k]) for k in ("Q1", "K1", "Q2", "K2", "g"))
     torch.cuda.synchronize()
@@ -435,16 +496,23 @@ def main():
     value = whole_job_tflops(world, flop_f + flop_b, step_ms)
     extra_hbm = torch.cuda.max_memory_allocated() - base_mem
 
-    # ---- roofline of the dominant kernel (largest share of the step), from the events recorded inside the timed region
+    # ---- roofline of the dominant kernel (largest share of the step), from the events recorded inside the timed region.
+    # `frac` uses SURVEY 8(d)'s algorithmic (one-visit) FLOPs of that kernel; `frac_executed` what it actually executes.
     dom = max(res["kernels"].items(), key=lambda kv: kv[1]["avg_ms"] * kv[1]["launches_per_step"])
     dom_name, dom_stat = dom
-    peak_tf = float(pk["bf16_tflops_sustained"] if step_ms * args.steps > 1000.0 else pk["bf16_tflops"])
-    ach = kernel_flops(cfg, dom_name) / (dom_stat["avg_ms"] * 1e-3) / 1e12
+    n_bwd_tc = sum(v["launches_per_step"] for k, v in res["kernels"].items() if "bwd" in k and "sm100" in k)
+    sustained = step_ms * args.steps > 1000.0
+    peak_tf = float(pk["bf16_tflops_sustained"] if sustained else pk["bf16_tflops"])
+    ach = kernel_flops_one_visit(cfg, dom_name, n_bwd_tc) / (dom_stat["avg_ms"] * 1e-3) / 1e12
+    ach_x = kernel_flops(cfg, dom_name) / (dom_stat["avg_ms"] * 1e-3) / 1e12
     roofline = {"bound": "tensor", "kernel": dom_name, "achieved": ach, "peak": peak_tf, "unit": "TFLOP/s", "frac": ach / peak_tf,
-                "traffic": profiled_traffic(cfg, dom_name), "traffic_unit": "bytes/launch (ncu dram read+write)",
+                "achieved_executed": ach_x, "frac_executed": ach_x / peak_tf,
+                "flop_count": "achieved/frac: algorithmic (one-visit) FLOPs of this kernel, the logit recompute shared by the step's "
+                              "backward kernels credited once; *_executed: the FLOPs the kernel executes",
+                "traffic": profiled_traffic(cfg, dom_name),
+                "traffic_unit": "bytes/launch, ncu dram read+write of this kernel from the committed capture under profiles/ (not measured in this run)",
                 "algorithmic_hbm_bytes": kernel_hbm_bytes(cfg, dom_name),
-                "peak_source": f"{pk['_source']} bf16 "
-                + ("sustained" if step_ms * args.steps > 1000.0 else "burst") + " (MEASURED_PEAKS.json)",
+                "peak_source": f"{pk['_source']} bf16 " + ("sustained" if sustained else "burst") + " (MEASURED_PEAKS.json)",
                 "share_of_step": dom_stat["avg_ms"] * dom_stat["launches_per_step"] / res["step_ms"],
                 "avg_ms": dom_stat["avg_ms"]}
 
@@ -460,7 +528,8 @@ def main():
         "fwd_frac_of_measured_bf16_sustained": flop_f / (res["fwd_ms"] * 1e-3) / 1e12 / float(pk["bf16_tflops_sustained"]),
         "bwd_frac_of_measured_bf16_sustained": flop_b / (res["bwd_ms"] * 1e-3) / 1e12 / float(pk["bf16_tflops_sustained"]),
         "bwd_executed_tflops": sum(kernel_flops(cfg, k) * v["launches_per_step"] for k, v in res["kernels"].items()
-                                   if "bwd_sm100" in k) / (res["bwd_ms"] * 1e-3) / 1e12,
+                                   if "bwd" in k and "sm100" in k) / (res["bwd_ms"] * 1e-3) / 1e12,
+        "bwd_mode": args.bwd_mode,
         "kernels": res["kernels"],
         "extra_hbm_bytes": {"total_peak_over_inputs": int(extra_hbm), "outputs": output_bytes(cfg),
                             "workspace": int(res["workspace_bytes"])},
@@ -469,19 +538,27 @@ def main():
     # ---- secondary: the 16K configuration the metric also names
     also = {}
     if not args.no_also and args.workload == "cfg4":
-        c3 = W.CONFIGS[3]
-        h3 = gen_inputs(c3, rank)
-        d3 = tuple(to_dev(h3[k]) for k in ("Q1", "K1", "Q2", "K2", "g"))
-        r3 = time_passes(skl, c3, d3, max(args.steps, 10), args.warmup, barrier)
-        also["cfg3 indexer 16K (H=32, d=128/64, causal, dQ2,dK2 only)"] = {
-            "fwd_ms": r3["fwd_ms"], "bwd_ms": r3["bwd_ms"], "fwd_tflops": c3.fwd_flop() / (r3["fwd_ms"] * 1e-3) / 1e12,
-            "bwd_tflops": c3.bwd_flop() / (r3["bwd_ms"] * 1e-3) / 1e12,
-            "fwd_frac_of_measured_bf16_burst": c3.fwd_flop() / (r3["fwd_ms"] * 1e-3) / 1e12 / float(pk["bf16_tflops"])}
-        del d3, h3, r3
+        labels = {3: "cfg3 indexer 16K (H=32, d=128/64, causal, dQ2,dK2 only)", 2: "cfg2 near-identical 4K (H=32, d=128/128, causal, all four grads)",
+                  5: "cfg5 skewed (B=4,H=16, 2048x131072, d=128/64, no mask, Q1 x4, all four grads)"}
+        for idx in (3, 2, 5):
+            c = W.CONFIGS[idx]
+            h = gen_inputs(c, rank)
+            d = tuple(to_dev(h[k]) for k in ("Q1", "K1", "Q2", "K2", "g"))
+            r = time_passes(skl, c, d, max(args.steps, 10), args.warmup, barrier)
+            also[labels[idx]] = {
+                "step_ms": r["step_ms"], "fwd_ms": r["fwd_ms"], "bwd_ms": r["bwd_ms"],
+                "step_tflops": (c.fwd_flop() + c.bwd_flop()) / (r["step_ms"] * 1e-3) / 1e12,
+                "fwd_tflops": c.fwd_flop() / (r["fwd_ms"] * 1e-3) / 1e12, "bwd_tflops": c.bwd_flop() / (r["bwd_ms"] * 1e-3) / 1e12,
+                "fwd_frac_of_measured_bf16_burst": c.fwd_flop() / (r["fwd_ms"] * 1e-3) / 1e12 / float(pk["bf16_tflops"]),
+                "workspace_bytes": int(r["workspace_bytes"]),
+                "kernels_ms": {k: v["avg_ms"] for k, v in r["kernels"].items()}}
+            del d, h, r
+            torch.cuda.empty_cache()
         sk = time_splitk(skl)
         sk["roofline"] = {"bound": "hbm", "achieved": sk["hbm_gbs"], "peak": float(pk["hbm_gbs"]), "unit": "GB/s",
                           "frac": sk["hbm_gbs"] / float(pk["hbm_gbs"])}
         also["split-K forward (bsz=16, NQ=16, NK=131072, d=128/128, no mask)"] = sk
+        also["backward strategies (separate owner kernels vs one-visit kernels)"] = time_bwd_strategies(skl)
 
     # ---- e2e: host buffers through streamkl_fwd_bwd_host (copies inside the timed region)
     e2e = None

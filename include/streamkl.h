@@ -23,8 +23,10 @@
  *    retains them, and only enqueues work on `stream` (asynchronous; device faults surface at the caller's next
  *    synchronisation).  `*_host` entry points take HOST pointers, allocate their own device scratch, copy in,
  *    run, copy back and synchronise before returning.
- *  - Return value: 0 (STREAMKL_OK) or a negative STREAMKL_ERR_* code.  A failed call enqueues nothing and
- *    writes nothing.  The library never throws, prints or exits.  There is no CPU fallback: on a machine without
+ *  - Return value: 0 (STREAMKL_OK) or a negative STREAMKL_ERR_* code.  Argument errors (every code but
+ *    STREAMKL_ERR_CUDA) are detected before anything is enqueued: such a call enqueues nothing and writes nothing.  A
+ *    STREAMKL_ERR_CUDA (tensor-map encode, launch or copy failure) can surface after earlier kernels of the same call were
+ *    enqueued; the outputs are then unspecified.  The library never throws, prints or exits.  There is no CPU fallback: on a machine without
  *    an sm_100 GPU every compute entry point returns STREAMKL_ERR_CUDA.
  *  - Thread-safe for concurrent calls on distinct streams.
  *  - Shapes: B,H >= 0 (B*H == 0 or NQ == 0 is a successful no-op), NK >= 1, 1 <= d1,d2 <= 256,
@@ -98,7 +100,8 @@ size_t streamkl_fwd_splitk_workspace_bytes(int B, int H, int NQ, int splits);
  *   dQ1 [B][H][NQ][d1], dK1 [B][H][NK][d1] : both NULL => teacher frozen (Setting 1 only); both non-NULL =>
  *                                            Setting 2 gradients too.  Exactly one NULL is STREAMKL_ERR_NULLPTR.
  *   workspace : device scratch of at least streamkl_bwd_workspace_bytes(...) bytes (may be NULL when that is 0).
- * dK is accumulated atomic-free by K-tile ownership; dQ by Q-tile ownership (deterministic, no atomics).
+ * dK is always accumulated atomic-free by K-tile ownership.  dQ: by Q-tile ownership (deterministic, no atomics) under
+ * STREAMKL_BWD_SEPARATE; by fp32 atomics under the one-visit strategy, which the default mode selects for small NQ (below).
  */
 int streamkl_bwd(const void* Q1, const void* K1, const void* Q2, const void* K2,
                  int B, int H, int NQ, int NK, int d1, int d2, float c1, float c2, int causal,
@@ -114,19 +117,24 @@ int streamkl_bwd_f32(const void* Q1, const void* K1, const void* Q2, const void*
 /*
  * Backward strategy, per calling thread.  The tcgen05 path has two:
  *   STREAMKL_BWD_SEPARATE : a Q-owner kernel (dQ) and a K-owner kernel (dK); every output tile has one owner, no atomics,
- *                           bit-reproducible.  The only strategy when teacher gradients are requested.
- *   STREAMKL_BWD_FUSED    : Setting 1 only (dQ1 = dK1 = NULL): one K-owner kernel visits every tile pair once, keeps dK2 in
- *                           place and adds its dQ2 contributions with fp32 atomics into the workspace, then one rounding to
- *                           bf16.  Half the logit recomputation and exps; dQ2 reproducible only up to fp32 summation order.
- *   STREAMKL_BWD_AUTO     : (default) FUSED when it applies and NQ <= 512 (the measured crossover on B200; the paper's rule
- *                           T_Q*C <= T_K, with the crossover found independent of T_K), else SEPARATE.
+ *                           bit-reproducible.
+ *   STREAMKL_BWD_FUSED    : one-visit K-owner kernels: a pass visits every tile pair once, keeps dK in place and adds its dQ
+ *                           contributions with fp32 atomics into the workspace, then one rounding to the output dtype.  One
+ *                           pass for the student (dQ2, dK2: all of Setting 1 -- half the logit recomputation and exps of the
+ *                           separate kernels), a second one for the teacher when dQ1, dK1 are requested.  dQ is reproducible
+ *                           only up to fp32 summation order.
+ *   STREAMKL_BWD_AUTO     : (default) FUSED below the measured crossover on B200 -- NQ <= 512 without teacher gradients,
+ *                           NQ <= 256 with them (the paper's rule T_Q*C <= T_K, with the crossover found
+ *                           independent of T_K) -- else SEPARATE.  NOTE: AUTO is therefore NOT bit-reproducible for small NQ;
+ *                           select STREAMKL_BWD_SEPARATE where that matters.
  * Returns STREAMKL_OK, or STREAMKL_ERR_SHAPE for an unknown mode.
  */
 enum { STREAMKL_BWD_AUTO = 0, STREAMKL_BWD_SEPARATE = 1, STREAMKL_BWD_FUSED = 2 };
 int streamkl_set_bwd_mode(int mode);
 
-/* Bytes of device scratch streamkl_bwd needs for this shape (O((NQ+NK)*d) at most, never O(NQ*NK)): 16 B per query of
- * packed per-query scalars, plus -- without teacher gradients -- the fp32 dQ2 accumulator of the fused strategy. */
+/* Bytes of device scratch streamkl_bwd needs for this shape UNDER THE CALLING THREAD'S CURRENT MODE (O((NQ+NK)*d) at most,
+ * never O(NQ*NK)): 16 B per query of packed per-query scalars, plus -- only when the one-visit strategy will run (mode FUSED,
+ * or AUTO below its crossover) -- the fp32 dQ2 (and dQ1) accumulators, each region padded to 256 B. */
 size_t streamkl_bwd_workspace_bytes(int B, int H, int NQ, int NK, int d1, int d2, int want_teacher_grads);
 
 /*
@@ -158,10 +166,11 @@ int streamkl_host_trim(void);
 int streamkl_last_launch_count(void);
 
 /*
- * Per-kernel timing, a measurement aid (bench.py's roofline block uses it).  streamkl_profile_enable(1) makes every
+ * Per-kernel timing, a measurement aid (bench.py's roofline block uses it).  streamkl_profile_enable(on != 0) makes every
  * later kernel launch from the calling thread record a CUDA event on the launch stream immediately before and after
- * the kernel; streamkl_profile_collect() synchronises those events, writes up to max_records (kernel id, milliseconds)
- * pairs in launch order, forgets them and returns how many it wrote (or a negative STREAMKL_ERR_* code).
+ * the kernel (on > 1 additionally creates `on` event pairs up front, so that none is created inside a timed region; events
+ * are pooled and reused); streamkl_profile_collect() synchronises those events, writes up to max_records (kernel id,
+ * milliseconds) pairs in launch order, forgets them and returns how many it wrote (or a negative STREAMKL_ERR_* code).
  * streamkl_kernel_name() maps a kernel id to the kernel's name (static string).  Disabled by default; when disabled
  * the launch path does not touch events at all.
  */

@@ -115,8 +115,9 @@ def streamkl_last_launch_count() -> int:
     return int(lib().streamkl_last_launch_count())
 
 
-def streamkl_profile_enable(on: bool) -> None:
-    lib().streamkl_profile_enable(int(bool(on)))
+def streamkl_profile_enable(on) -> None:
+    """on = False/0: off; True/1: on; n > 1: on, with n event pairs created up front (none created inside a timed region)."""
+    lib().streamkl_profile_enable(int(on))
 
 
 def streamkl_profile_collect(max_records: int = 4096):
@@ -138,6 +139,13 @@ def streamkl_bwd_workspace_bytes(B, H, NQ, NK, d1, d2, want_teacher_grads) -> in
 
 
 # ------------------------------------------------------------------------------------------ device entry points
+def _keep_alive_on(t, stream):
+    """A scratch tensor allocated here (on torch's current stream) is used by kernels enqueued on `stream` and dropped when the
+    call returns: tell the caching allocator, so that the block is not handed to other work while those kernels still run."""
+    if stream is not None:   # a torch.cuda.Stream other than (possibly) the current one
+        t.record_stream(stream)
+
+
 def _check_dev(name, t, dtype=None):
     import torch
 
@@ -221,6 +229,7 @@ def streamkl_fwd_splitk(Q1, K1, Q2, K2, c1, c2, causal, splits=0, kl_rows=None, 
     need = streamkl_fwd_splitk_workspace_bytes(B, H, NQ, w)
     if need > 0 and (workspace is None or workspace.numel() * workspace.element_size() < need):
         workspace = torch.empty(need, dtype=torch.uint8, device=Q1.device)
+        _keep_alive_on(workspace, stream)
     ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
     with torch.cuda.device(Q1.device):
         rc = lib().streamkl_fwd_splitk(_ptr(Q1), _ptr(K1), _ptr(Q2), _ptr(K2), B, H, NQ, NK, d1, d2, float(c1), float(c2),
@@ -258,6 +267,7 @@ def streamkl_bwd(Q1, K1, Q2, K2, c1, c2, causal, kl_rows, lse1, lse2, dkl_rows, 
     need = streamkl_bwd_workspace_bytes(B, H, NQ, NK, d1, d2, teacher)
     if need > 0 and (workspace is None or workspace.numel() * workspace.element_size() < need):
         workspace = torch.empty(need, dtype=torch.uint8, device=Q1.device)
+        _keep_alive_on(workspace, stream)
     ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
     if Q1.dtype == torch.bfloat16:
         fn = lib().streamkl_bwd

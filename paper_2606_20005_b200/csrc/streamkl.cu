@@ -32,15 +32,29 @@ const char* const kKernelNames[KID_COUNT] = {"streamkl_fwd_sm100_kernel", "strea
 struct ProfRecord { int id; cudaEvent_t a, b; };
 thread_local bool g_prof_on = false;
 thread_local std::vector<ProfRecord>* g_prof = nullptr;
+thread_local std::vector<cudaEvent_t>* g_prof_pool = nullptr;   // idle events: created outside the timed region, reused
+
+cudaEvent_t prof_event() {
+  if (g_prof_pool && !g_prof_pool->empty()) { cudaEvent_t e = g_prof_pool->back(); g_prof_pool->pop_back(); return e; }
+  cudaEvent_t e = nullptr;
+  if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+  return e;
+}
+void prof_release(cudaEvent_t e) {
+  if (!e) return;
+  if (!g_prof_pool) g_prof_pool = new std::vector<cudaEvent_t>();
+  g_prof_pool->push_back(e);
+}
 
 struct ProfScope {  // brackets ONE kernel launch; a no-op unless profiling is enabled on this thread
   cudaStream_t st; cudaEvent_t b = nullptr;
   ProfScope(int id, cudaStream_t s) : st(s) {
     if (!g_prof_on) return;
     if (!g_prof) g_prof = new std::vector<ProfRecord>();
-    cudaEvent_t a = nullptr;
-    if (cudaEventCreate(&a) != cudaSuccess) { cudaGetLastError(); return; }
-    if (cudaEventCreate(&b) != cudaSuccess) { cudaGetLastError(); cudaEventDestroy(a); b = nullptr; return; }
+    cudaEvent_t a = prof_event();
+    if (!a) return;
+    b = prof_event();
+    if (!b) { prof_release(a); return; }
     cudaEventRecord(a, st);
     g_prof->push_back({id, a, b});
   }
@@ -272,37 +286,41 @@ int launch_bwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2
   return STREAMKL_OK;
 }
 
-// Strategy selection of the Setting-1 backward (see bwd_tc_both): the one-visit kernel iff no teacher gradients are wanted and
-// the mode is FUSED, or AUTO with at most four 128-query tiles per head.  streamkl_bwd_workspace_bytes applies the same rule,
-// so the fp32 dQ2 accumulator is only asked for when the strategy that will run needs it.
+// Strategy selection of the backward (see bwd_tc_both): the one-visit kernels iff the mode is FUSED, or AUTO below the measured
+// crossover (bench.py "backward strategies", profiles/r02_bwd_strategies.md): at most four 128-query tiles per head for
+// Setting 1 (one pass: half the recomputation), at most two for Setting 2 (two passes: same work as the owner kernels, the
+// gain is the fuller K-owner grid).  streamkl_bwd_workspace_bytes applies the same rule, so the fp32 dQ accumulators are
+// only asked for when the strategy that will run needs them.
 bool bwd_fused_selected(int NQ, bool teacher) {
-  return !teacher && (g_bwd_mode == STREAMKL_BWD_FUSED || (g_bwd_mode == STREAMKL_BWD_AUTO && (NQ + 127) / 128 <= 4));
+  return g_bwd_mode == STREAMKL_BWD_FUSED || (g_bwd_mode == STREAMKL_BWD_AUTO && (NQ + 127) / 128 <= (teacher ? 2 : 4));
 }
+size_t fused_acc_bytes_aligned(long long BH, int NQ, int d) { return (size_t(BH) * size_t(NQ) * size_t(d) * sizeof(float) + 255) & ~size_t(255); }
 
 size_t stats_bytes_aligned(long long BH, int NQ) { return (size_t(BH) * size_t(skl::bwd_stats_padded_rows(NQ)) * 16 + 255) & ~size_t(255); }
 
-// Setting 1 in one visit: zero the fp32 dQ2 accumulator, run the fused K-owner kernel, convert dQ2.
-template <int D1, int D2, bool CAUSAL>
+// One one-visit pass: zero the fp32 dQ accumulator, run the fused K-owner kernel, convert dQ.
+// TPASS = false: student (dS2 -> dQ2, dK2); true: teacher (dS1 -> dQ1, dK1).
+template <int D1, int D2, bool CAUSAL, bool TPASS>
 int launch_bwd_fused(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, const float4* stats, float* dq_acc,
-                     void* dQ2, void* dK2, cudaStream_t stream) {
-  using C = skl::BwdFusedCfg<D1, D2>;
+                     void* dQ, void* dK, cudaStream_t stream) {
+  using C = skl::BwdFusedCfg<D1, D2, TPASS>;
   CUtensorMap tQ1, tK1, tQ2, tK2;
   if (!make_tmap_bf16(&tQ1, Q1, int(s.BH), s.NQ, D1, C::BY) || !make_tmap_bf16(&tK1, K1, int(s.BH), s.NK, D1, C::BX) ||
       !make_tmap_bf16(&tQ2, Q2, int(s.BH), s.NQ, D2, C::BY) || !make_tmap_bf16(&tK2, K2, int(s.BH), s.NK, D2, C::BX))
     return STREAMKL_ERR_CUDA;
-  auto kern = skl::streamkl_bwd_fused_sm100_kernel<D1, D2, CAUSAL>;
+  auto kern = skl::streamkl_bwd_fused_sm100_kernel<D1, D2, CAUSAL, TPASS>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
     cudaGetLastError();
     return STREAMKL_ERR_CUDA;
   }
-  const size_t n = size_t(s.BH) * s.NQ * D2;
+  const size_t n = size_t(s.BH) * s.NQ * C::DG;
   if (cudaMemsetAsync(dq_acc, 0, n * sizeof(float), stream) != cudaSuccess) { cudaGetLastError(); return STREAMKL_ERR_CUDA; }
   skl::BwdFusedParams p;
   p.NQ = s.NQ; p.NK = s.NK; p.BH = int(s.BH);
   p.TX = (s.NK + C::BX - 1) / C::BX;
   p.c1 = s.c1; p.c2 = s.c2;
   p.stats = stats; p.dq_acc = dq_acc;
-  p.dK2 = static_cast<__nv_bfloat16*>(dK2);
+  p.dK = static_cast<__nv_bfloat16*>(dK);
   const long long grid = (long long)p.TX * s.BH;
   if (grid > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
   {
@@ -313,8 +331,8 @@ int launch_bwd_fused(const void* Q1, const void* K1, const void* Q2, const void*
   const long long n4 = (long long)(n / 4);
   {
     ProfScope ps(KID_BWD_DQ_CONVERT, stream);
-    skl::streamkl_bwd_dq_convert_kernel<<<dim3((unsigned)((n4 + 255) / 256)), 256, 0, stream>>>(reinterpret_cast<const float4*>(dq_acc),
-                                                                                             static_cast<uint2*>(dQ2), s.c2, n4);
+    skl::streamkl_bwd_dq_convert_kernel<<<dim3((unsigned)((n4 + 255) / 256)), 256, 0, stream>>>(
+        reinterpret_cast<const float4*>(dq_acc), static_cast<uint2*>(dQ), TPASS ? s.c1 * 0.6931471805599453f : s.c2, n4);
   }
   if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
   g_last_launches += 2;
@@ -340,14 +358,20 @@ int bwd_tc_both(const void* Q1, const void* K1, const void* Q2, const void* K2, 
     g_last_launches += 1;
   }
   // Strategy (PAPER.md:321 picks fused iff T_Q*C <= T_K with an empirically tuned C).  Measured on B200
-  // (profiles/r01f_fused_bwd.md): the one-visit kernel wins 1.3-3.0x while the Q-owner grid is small (T_Q <= 4 tiles of 128
-  // queries), is level at T_Q = 8 and loses a few per cent beyond, where its fp32 atomics (64 KB per 128x128 tile pair)
-  // run into the L2's atomic throughput; the crossover did not move with T_K (128 vs 1024), so the rule is on T_Q alone.
+  // (profiles/r01f_fused_bwd.md, r02_bwd_strategies.md): the one-visit kernels win while the Q-owner grid is small (Setting 1:
+  // 1.3-3.0x up to T_Q = 4 tiles of 128 queries, level at 8; Setting 2: 1.3-1.5x up to T_Q = 2, 0.8x at 4) and lose beyond,
+  // where their fp32 atomics (64 KB per 128x128 tile pair and pass) run into the L2's atomic throughput; the crossover did
+  // not move with T_K (128 vs 1024), so the rule is on T_Q alone.
   const bool fused = bwd_fused_selected(s.NQ, t);
-  if (fused) {   // Setting 1: one visit, dQ2 through fp32 atomics
-    float* dq_acc = reinterpret_cast<float*>(static_cast<uint8_t*>(workspace) + stats_bytes_aligned(s.BH, s.NQ));
-    return s.causal ? launch_bwd_fused<D1, D2, true>(Q1, K1, Q2, K2, s, stats, dq_acc, dQ2, dK2, st)
-                    : launch_bwd_fused<D1, D2, false>(Q1, K1, Q2, K2, s, stats, dq_acc, dQ2, dK2, st);
+  if (fused) {   // one visit per differentiated distribution, dQ through fp32 atomics
+    uint8_t* w = static_cast<uint8_t*>(workspace) + stats_bytes_aligned(s.BH, s.NQ);
+    float* acc2 = reinterpret_cast<float*>(w);
+    float* acc1 = reinterpret_cast<float*>(w + fused_acc_bytes_aligned(s.BH, s.NQ, D2));
+    rc = s.causal ? launch_bwd_fused<D1, D2, true, false>(Q1, K1, Q2, K2, s, stats, acc2, dQ2, dK2, st)
+                  : launch_bwd_fused<D1, D2, false, false>(Q1, K1, Q2, K2, s, stats, acc2, dQ2, dK2, st);
+    if (rc != STREAMKL_OK || !t) return rc;
+    return s.causal ? launch_bwd_fused<D1, D2, true, true>(Q1, K1, Q2, K2, s, stats, acc1, dQ1, dK1, st)
+                    : launch_bwd_fused<D1, D2, false, true>(Q1, K1, Q2, K2, s, stats, acc1, dQ1, dK1, st);
   }
 #define SKL_BWD(CA, TE)                                                                                                   \
   rc = launch_bwd_tc<D1, D2, CA, TE, false>(Q1, K1, Q2, K2, s, stats, dQ1, dQ2, st);                                      \
@@ -516,8 +540,8 @@ size_t streamkl_bwd_workspace_bytes(int B, int H, int NQ, int, int d1, int d2, i
   if (!((d1 == 64 || d1 == 128) && (d2 == 64 || d2 == 128))) return 0;
   const long long BH = (long long)B * H;
   if (!bwd_fused_selected(NQ, want_teacher != 0)) return size_t(BH) * size_t(skl::bwd_stats_padded_rows(NQ)) * 16;
-  // one-visit Setting-1 kernel (mode FUSED, or AUTO with NQ <= 512): + its fp32 dQ2 accumulator, O(NQ d2)
-  return stats_bytes_aligned(BH, NQ) + size_t(BH) * size_t(NQ) * size_t(d2) * sizeof(float);
+  // one-visit kernels (mode FUSED, or AUTO with NQ <= 512): + their fp32 dQ accumulators, O(NQ d)
+  return stats_bytes_aligned(BH, NQ) + fused_acc_bytes_aligned(BH, NQ, d2) + (want_teacher ? fused_acc_bytes_aligned(BH, NQ, d1) : 0);
 }
 
 int streamkl_set_bwd_mode(int mode) {
@@ -676,6 +700,12 @@ int streamkl_last_launch_count(void) { return g_last_launches; }
 
 int streamkl_profile_enable(int on) {
   g_prof_on = on != 0;
+  // on > 1: also create that many event pairs now, so that no event is created inside the caller's timed region
+  if (on > 1) {
+    std::vector<cudaEvent_t> tmp;
+    for (int i = 0; i < 2 * on; ++i) { cudaEvent_t e = prof_event(); if (!e) break; tmp.push_back(e); }
+    for (cudaEvent_t e : tmp) prof_release(e);
+  }
   return STREAMKL_OK;
 }
 
@@ -687,8 +717,8 @@ int streamkl_profile_collect(int max_records, int* kernel_ids, float* ms) {
     float t = 0.f;
     if (cudaEventSynchronize(r.b) != cudaSuccess || cudaEventElapsedTime(&t, r.a, r.b) != cudaSuccess) { cudaGetLastError(); rc = STREAMKL_ERR_CUDA; }
     else if (n < max_records) { kernel_ids[n] = r.id; ms[n] = t; ++n; }
-    cudaEventDestroy(r.a);
-    cudaEventDestroy(r.b);
+    prof_release(r.a);
+    prof_release(r.b);
   }
   g_prof->clear();
   return rc < 0 ? rc : n;

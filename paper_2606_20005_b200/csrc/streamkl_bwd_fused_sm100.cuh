@@ -1,8 +1,11 @@
-// streamkl_bwd_fused_sm100.cuh -- one-visit ("fused") StreamKL backward for Setting 1 (teacher frozen: dQ2, dK2 only),
-// the CTA owns a 128-row K tile, visits every (query tile, key tile) pair ONCE, accumulates dK2 in
-// place and adds its dQ2 contribution with fp32 atomics.  Against the two separate kernels (streamkl_bwd_sm100.cuh) this
-// halves the logit recomputation and the exps; the price is an fp32 dQ2 workspace, a convert pass, and a dQ2 that is
-// reproducible only up to fp32 summation order (the separate kernels remain the deterministic mode).
+// streamkl_bwd_fused_sm100.cuh -- one-visit ("fused") StreamKL backward: the CTA owns a 128-row K tile,
+// visits every (query tile, key tile) pair ONCE, accumulates dK in place and adds its dQ contribution with fp32 atomics.
+// One pass per differentiated distribution: the student pass (TPASS = false: dS2 -> dK2, dQ2; all of Setting 1) and the
+// teacher pass (TPASS = true: dS1 -> dK1, dQ1; Setting 2 runs both).  Against the separate kernels (streamkl_bwd_sm100.cuh)
+// the student pass alone halves the logit recomputation and the exps of Setting 1; for Setting 2 the two passes execute the
+// same work as the two owner kernels, but both grids are K-owner grids (bsz x T_K CTAs), which is what fills the machine
+// when N_Q is small.  The price is an fp32 dQ workspace, a convert pass, and a dQ that is reproducible only up to fp32
+// summation order (the separate kernels remain the deterministic mode).  Below, "2" stands for the pass's distribution.
 //
 // Per 64-query step, with K = the owned key tile (X) and Q = the streamed query tile (Y):
 //   S1' = K1 Q1^T, S2' = K2 Q2^T          tcgen05.mma (SS) -> TMEM, lane = key                                   (B2)
@@ -21,7 +24,7 @@
 
 namespace skl {
 
-template <int D1, int D2>
+template <int D1, int D2, bool TPASS = false>
 struct BwdFusedCfg {
   static_assert(D1 % 64 == 0 && D2 % 64 == 0 && D1 <= 128 && D2 <= 128, "tcgen05 path: d in {64,128}");
   static constexpr int BX = 128, BY = 64;
@@ -39,10 +42,11 @@ struct BwdFusedCfg {
   static constexpr int SMEM_BYTES = 1024 + X_BYTES + DS_BYTES + NSTAGE * (Y_STAGE + STAT_STAGE) + AUX_BYTES;
   static constexpr int THREADS = 128 + 512;
   static constexpr uint32_t TMEM_COLS = 512;
-  static constexpr int NSS = (512 - 64 - D2 - 128) / 128 >= 2 ? 2 : 1;
+  static constexpr int DG = TPASS ? D1 : D2;                  // head dim of the distribution this pass differentiates
+  static constexpr int NSS = (512 - 64 - DG - 128) / 128 >= 2 ? 2 : 1;
   static constexpr uint32_t COL_DS = NSS * 128;               // 2 stages x 32 packed columns
   static constexpr uint32_t COL_DK = COL_DS + 64;
-  static constexpr uint32_t COL_DQ = COL_DK + D2;             // 2 stages x 64 columns (queries), lane = d
+  static constexpr uint32_t COL_DQ = COL_DK + DG;             // 2 stages x 64 columns (queries), lane = d
   static_assert(COL_DQ + 128 <= 512, "TMEM budget");
 };
 
@@ -50,11 +54,11 @@ struct BwdFusedParams {
   int NQ, NK, TX, BH;
   float c1, c2;
   const float4* stats;   // as BwdParams::stats
-  float* dq_acc;         // [BH][NQ][D2] fp32, zeroed by the caller of the kernel
-  __nv_bfloat16* dK2;
+  float* dq_acc;         // [BH][NQ][DG] fp32, zeroed by the caller of the kernel
+  __nv_bfloat16* dK;     // dK2 (student pass) or dK1 (teacher pass)
 };
 
-// dQ2 = bf16(c2 * dq_acc): the one rounding of the atomically accumulated gradient
+// dQ = bf16(scale * dq_acc): the one rounding of the atomically accumulated gradient (scale = c2, or c1 ln2 for the teacher)
 __global__ void streamkl_bwd_dq_convert_kernel(const float4* __restrict__ acc, uint2* __restrict__ out, float c2, long long n4) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n4) return;
@@ -62,12 +66,13 @@ __global__ void streamkl_bwd_dq_convert_kernel(const float4* __restrict__ acc, u
   out[i] = make_uint2(pack_bf16x2(v.x * c2, v.y * c2), pack_bf16x2(v.z * c2, v.w * c2));
 }
 
-template <int D1, int D2, bool CAUSAL>
-__global__ void __launch_bounds__(BwdFusedCfg<D1, D2>::THREADS, 1)
+template <int D1, int D2, bool CAUSAL, bool TPASS = false>
+__global__ void __launch_bounds__(BwdFusedCfg<D1, D2, TPASS>::THREADS, 1)
 streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid_constant__ CUtensorMap tmK1,
                                 const __grid_constant__ CUtensorMap tmQ2, const __grid_constant__ CUtensorMap tmK2,
                                 const BwdFusedParams p) {
-  using C = BwdFusedCfg<D1, D2>;
+  using C = BwdFusedCfg<D1, D2, TPASS>;
+  constexpr int DG = C::DG;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   uint8_t* sX1 = smem;                                    // K1 tile (owner)
@@ -184,13 +189,13 @@ streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const 
       }
     } else if (warp == 3) {
       // ===================== gradient MMA issuer =====================
-      constexpr uint32_t idesc_k = umma_idesc_bf16(C::BX, D2, 0, 1);    // dK2 += dS2 Q2   : A from TMEM, B = Q2 MN-major
+      constexpr uint32_t idesc_k = umma_idesc_bf16(C::BX, DG, 0, 1);    // dK2 += dS2 Q2   : A from TMEM, B = Q2 MN-major
       constexpr uint32_t idesc_q = umma_idesc_bf16(128, C::BY, 1, 1);   // dQ2^T = K2^T dS2: A = K2 MN-major, B = dS2 MN-major
       // MN-major operands: rows = the contraction index (128 B each, 8-row groups 1024 B apart = SBO), 64-element chunks
       // of the M/N index LBO bytes apart; a K=16 slice = 16 rows = 2048 B.  For d2 = 64 the padded half of M reads the
       // shared memory behind the K2 tile: those accumulator lanes (d >= 64) are never drained.
       const uint64_t dym = umma_smem_desc_sw128(smem_u32(sY), C::YBLK, 1024);
-      const uint64_t dka = umma_smem_desc_sw128(smem_u32(sX2), C::XBLK, 1024);
+      const uint64_t dka = umma_smem_desc_sw128(smem_u32(TPASS ? sX1 : sX2), C::XBLK, 1024);
       const uint64_t dsb = umma_smem_desc_sw128(smem_u32(sDS), C::DS_TILE, 1024);
       for (int it = 0; it < nsteps; ++it) {
         const int s = it % C::NSTAGE;
@@ -199,7 +204,7 @@ streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const 
         mbar_wait(&ds_full[par], u & 1);
         mbar_wait(&dq_empty[par], (u & 1) ^ 1);     // the dQ2^T stage of step it-2 has been copied to registers
         tc_fence_after();
-        uint64_t dys = dym + uint64_t((s * C::Y_STAGE + C::KB1 * C::YBLK) >> 4), ka = dka, db = dsb + uint64_t((par * C::DS_TILE) >> 4);
+        uint64_t dys = dym + uint64_t((s * C::Y_STAGE + (TPASS ? 0 : C::KB1 * C::YBLK)) >> 4), ka = dka, db = dsb + uint64_t((par * C::DS_TILE) >> 4);
         asm volatile("" : "+l"(dys), "+l"(ka), "+l"(db));
         const uint32_t tA = tmem_base + C::COL_DS + par * 32;
         const uint32_t acc = it > 0;
@@ -237,7 +242,7 @@ streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const 
     uint8_t* ds_srow = sDS + par * C::DS_TILE + rloc * 128;
     const int swz = rloc & 7;
     const uint32_t dq_taddr = lane_addr + C::COL_DQ + par * 64 + half * 32;
-    const bool d_valid = rloc < D2;           // this lane's d index exists (d2 = 64: lanes 64..127 are padding)
+    const bool d_valid = rloc < DG;           // this lane's d index exists (d = 64: lanes 64..127 are padding)
 
     // copy the dQ2^T stage of step `itd` (one of this group's steps) to registers, free the stage, add it to the fp32 workspace
     auto drain = [&](int itd) {
@@ -251,10 +256,10 @@ streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const 
       if (lane == 0) mbar_arrive(&dq_empty[par]);
       if (d_valid) {
         const int q0 = (j_begin + itd) * C::BY + half * 32;
-        float* dst = p.dq_acc + (size_t(bh) * p.NQ + q0) * D2 + rloc;
+        float* dst = p.dq_acc + (size_t(bh) * p.NQ + q0) * DG + rloc;
 #pragma unroll
         for (int c = 0; c < 32; ++c)
-          if (q0 + c < p.NQ) atomicAdd(dst + size_t(c) * D2, __uint_as_float(q[c]));   // result unused: red.global.add.f32
+          if (q0 + c < p.NQ) atomicAdd(dst + size_t(c) * DG, __uint_as_float(q[c]));   // result unused: red.global.add.f32
       }
     };
 
@@ -280,8 +285,10 @@ streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const 
       // be inf there, and unlike the separate K-owner kernel this kernel CONTRACTS over the owned keys: dQ2^T = K2^T dS2)
       const bool masked = (CAUSAL && (y0 + off < x0 + C::BX - 1)) || (x0 + C::BX > p.NK);
       const uint32_t stat = stat_base + s * C::STAT_STAGE;
-      if (masked) ds_row<32, false, true, CAUSAL, true>(r1, r2, o1, o2, sc1, sc2, 0.f, 0.f, 0.f, stat, xrow, y0, off, p.NK);
-      else        ds_row<32, false, true, CAUSAL, false>(r1, r2, o1, o2, sc1, sc2, 0.f, 0.f, 0.f, stat, xrow, y0, off, p.NK);
+      // (o2 = the pass's dS: the teacher pass takes ds_row's dS1 output)
+      uint32_t (&f1)[16] = *(TPASS ? &o2 : &o1), (&f2)[16] = *(TPASS ? &o1 : &o2);
+      if (masked) ds_row<32, TPASS, true, CAUSAL, true, !TPASS>(r1, r2, f1, f2, sc1, sc2, 0.f, 0.f, 0.f, stat, xrow, y0, off, p.NK);
+      else        ds_row<32, TPASS, true, CAUSAL, false, !TPASS>(r1, r2, f1, f2, sc1, sc2, 0.f, 0.f, 0.f, stat, xrow, y0, off, p.NK);
       mbar_wait(&ds_empty[par], (u & 1) ^ 1);   // the MMAs of step it-2 have consumed both copies of this dS2 stage
       tc_fence_after();
       tmem_st16(ds_taddr, o2);
@@ -302,10 +309,12 @@ streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const 
     if (nsteps > 0) {
       mbar_wait(dk_full, 0);
       tc_fence_after();
-      store_dx_cols<D2 / 4>(lane_addr + C::COL_DK + grp * (D2 / 4), p.c2, p.dK2 + orow * D2 + grp * (D2 / 4), valid);
+      // (the teacher's dS1 is kept in log2 units, Eq.12: its ln2 joins the scale here, as in the separate kernels)
+      store_dx_cols<DG / 4>(lane_addr + C::COL_DK + grp * (DG / 4), TPASS ? p.c1 * 0.6931471805599453f : p.c2,
+                            p.dK + orow * DG + grp * (DG / 4), valid);
     } else if (valid) {
       const uint4 z = make_uint4(0, 0, 0, 0);
-      for (int c = 0; c < D2 / 4; c += 8) *reinterpret_cast<uint4*>(p.dK2 + orow * D2 + grp * (D2 / 4) + c) = z;
+      for (int c = 0; c < DG / 4; c += 8) *reinterpret_cast<uint4*>(p.dK + orow * DG + grp * (DG / 4) + c) = z;
     }
   }
   tc_fence_before();

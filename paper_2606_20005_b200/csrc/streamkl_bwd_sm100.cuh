@@ -145,7 +145,7 @@ __device__ __forceinline__ float4 lds_f4(uint32_t saddr) {
 //   OWNER_K: per-column scalars come from shared memory (`stat`: shared-space address of these NC/2 column
 //            pairs, two float4 each), g is applied here.
 // MASKED: causal diagonal tiles and streamed-key tails; P (possibly inf for a zero-filled logit) is discarded by SELECT.
-template <int NC, bool TEACHER, bool OWNER_K, bool CAUSAL, bool MASKED>
+template <int NC, bool TEACHER, bool OWNER_K, bool CAUSAL, bool MASKED, bool WANT2 = true>
 __device__ __forceinline__ void ds_row(const uint32_t (&r1)[NC], const uint32_t (&r2)[NC], uint32_t (&o1)[NC / 2], uint32_t (&o2)[NC / 2],
                                          float sc1, float sc2, float nL1, float nL2, float klog, uint32_t stat, int xrow,
                                          int y0, int off, int NK) {
@@ -164,8 +164,11 @@ __device__ __forceinline__ void ds_row(const uint32_t (&r1)[NC], const uint32_t 
     const bool poly = PE > 0 && ((e >> 1) % (PE > 0 ? PE : 1)) == 0;
     const float2 p1 = poly ? ex2_poly2(x1) : make_float2(ex2_approx(x1.x), ex2_approx(x1.y));
     const float2 p2 = poly ? ex2_poly2(x2) : make_float2(ex2_approx(x2.x), ex2_approx(x2.y));
-    float2 a2 = sub2(p2, p1);                                            // dS2 / g (Alg.2 line 8): fp32 subtract, rounded once below
-    if constexpr (OWNER_K) a2 = mul2(a2, vg);
+    float2 a2 = make_float2(0.f, 0.f);
+    if constexpr (WANT2) {
+      a2 = sub2(p2, p1);                                                 // dS2 / g (Alg.2 line 8): fp32 subtract, rounded once below
+      if constexpr (OWNER_K) a2 = mul2(a2, vg);
+    }
     float2 a1 = make_float2(0.f, 0.f);
     if constexpr (TEACHER) {                                             // dS1 / (g ln2) = P1 (x1 - x2 - kl log2e)   (Alg.3 lines 9-10, Eq.12)
       const float2 d = sub2(sub2(x1, x2), vk);
@@ -179,7 +182,7 @@ __device__ __forceinline__ void ds_row(const uint32_t (&r1)[NC], const uint32_t 
       a2.x = ok0 ? a2.x : 0.f; a2.y = ok1 ? a2.y : 0.f;
       a1.x = ok0 ? a1.x : 0.f; a1.y = ok1 ? a1.y : 0.f;
     }
-    o2[e >> 1] = pack_bf16x2(a2.x, a2.y);
+    if constexpr (WANT2) o2[e >> 1] = pack_bf16x2(a2.x, a2.y);
     if constexpr (TEACHER) o1[e >> 1] = pack_bf16x2(a1.x, a1.y);
   }
 }

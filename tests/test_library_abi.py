@@ -104,11 +104,22 @@ def test_workspace_is_never_quadratic(L):
     assert big <= 16 * max(small, 1) + 4 * 32 * 65536 * 256 * 4  # O((NQ+NK) d), not O(NQ NK)
 
 
-def test_bwd_workspace_is_16_bytes_per_padded_query(L):
+def test_bwd_workspace_follows_the_selected_strategy(L):
+    """16 B of packed per-query scalars (rows padded to 64 per head) always; the fp32 dQ accumulators of the one-visit kernels
+    only when that strategy will run (mode FUSED, or AUTO with NQ <= 512 / <= 256 with teacher gradients) -- cfg 3 (Setting 1, NQ = 16384) needs 8 MB, not 143."""
+    a256 = lambda n: (n + 255) // 256 * 256
+    assert L.streamkl_set_bwd_mode(0) == 0   # AUTO
     assert L.streamkl_bwd_workspace_bytes(1, 32, 65536, 65536, 128, 128, 1) == 32 * 65536 * 16
-    assert L.streamkl_bwd_workspace_bytes(2, 3, 100, 777, 128, 64, 1) == 6 * 128 * 16      # rows padded to 64 per head
-    # Setting 1: + the fp32 dQ2 accumulator of the fused strategy (scalars padded to 256 B)
-    assert L.streamkl_bwd_workspace_bytes(2, 3, 100, 777, 128, 64, 0) == 6 * 128 * 16 + 6 * 100 * 64 * 4
+    assert L.streamkl_bwd_workspace_bytes(1, 32, 16384, 16384, 128, 64, 0) == 32 * 16384 * 16              # cfg 3: 8 MB
+    # NQ <= 512 under AUTO: one-visit kernels, + fp32 dQ2 (+ dQ1 with teacher gradients), each region 256-byte aligned
+    assert L.streamkl_bwd_workspace_bytes(2, 3, 100, 777, 128, 64, 0) == a256(6 * 128 * 16) + a256(6 * 100 * 64 * 4)
+    assert L.streamkl_bwd_workspace_bytes(2, 3, 100, 777, 128, 64, 1) == a256(6 * 128 * 16) + a256(6 * 100 * 64 * 4) + a256(6 * 100 * 128 * 4)
+    assert L.streamkl_set_bwd_mode(1) == 0   # SEPARATE: never the accumulators
+    assert L.streamkl_bwd_workspace_bytes(2, 3, 100, 777, 128, 64, 0) == 6 * 128 * 16
+    assert L.streamkl_bwd_workspace_bytes(2, 3, 100, 777, 128, 64, 1) == 6 * 128 * 16
+    assert L.streamkl_set_bwd_mode(2) == 0   # FUSED: always
+    assert L.streamkl_bwd_workspace_bytes(1, 32, 16384, 16384, 128, 64, 0) == a256(32 * 16384 * 16) + a256(32 * 16384 * 64 * 4)
+    assert L.streamkl_set_bwd_mode(0) == 0
     assert L.streamkl_bwd_workspace_bytes(1, 1, 256, 256, 48, 80, 0) == 0                  # SIMT path: no workspace
 
 

@@ -37,6 +37,19 @@ def run_case(cfg: W.Config, teacher=None, check_bwd=True):
         check_grad_heads(to_f64(dK1), ref["dK1"], cfg.name + " dK1")
     else:
         assert dQ1 is None and dK1 is None
+    if cfg.dtype == "bf16" and cfg.d1 in (64, 128) and cfg.d2 in (64, 128):
+        # the default (AUTO) picks the one-visit kernels for NQ <= 512 and the owner kernels beyond: run the OTHER strategy too
+        other = skl.STREAMKL_BWD_SEPARATE if cfg.NQ <= (256 if teacher else 512) else skl.STREAMKL_BWD_FUSED
+        skl.streamkl_set_bwd_mode(other)
+        try:
+            g1, k1, g2, k2 = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, cfg.causal, kl, l1, l2, g, teacher=teacher)
+        finally:
+            skl.streamkl_set_bwd_mode(skl.STREAMKL_BWD_AUTO)
+        check_grad_heads(to_f64(g2), ref["dQ2"], f"{cfg.name} mode {other} dQ2")
+        check_grad_heads(to_f64(k2), ref["dK2"], f"{cfg.name} mode {other} dK2")
+        if teacher:
+            check_grad_heads(to_f64(g1), ref["dQ1"], f"{cfg.name} mode {other} dQ1")
+            check_grad_heads(to_f64(k1), ref["dK1"], f"{cfg.name} mode {other} dK1")
     return stats
 
 
@@ -248,6 +261,36 @@ def test_setting1_fused_and_separate_strategies_agree_with_the_oracle(d1, d2, ca
     finally:
         skl.streamkl_set_bwd_mode(skl.STREAMKL_BWD_AUTO)
     assert res[skl.STREAMKL_BWD_FUSED][2] == 3 and res[skl.STREAMKL_BWD_SEPARATE][2] == 3   # {stats, fused, convert} / {stats, dQ, dK}
+
+
+@pytest.mark.parametrize("d1,d2", [(128, 128), (128, 64), (64, 128), (64, 64)])
+@pytest.mark.parametrize("causal", [False, True])
+def test_setting2_fused_and_separate_strategies_agree_with_the_oracle(d1, d2, causal):
+    """Setting 2 (teacher trainable) through both strategies: two one-visit passes (student: dS2 -> dK2, dQ2; teacher: dS1 -> dK1,
+    dQ1, each dQ by fp32 atomics) and the two deterministic owner kernels; ragged sizes; mixed-sign upstream gradient."""
+    import torch
+
+    import paper_2606_20005_b200 as skl
+
+    cfg = W.Config(70 + d1 // 64 * 2 + d2 // 64, "setting2", 1, 3, 457, 901, d1, d2, "bf16", causal)
+    inp = W.all_inputs(cfg)
+    gnp = (inp["g"] - 0.9).astype(np.float32)
+    Q1, K1, Q2, K2 = (to_torch(inp[k]) for k in ("Q1", "K1", "Q2", "K2"))
+    g = torch.from_numpy(gnp).cuda()
+    ref = attention_kl(*(bits_to_f64(inp[k]) for k in ("Q1", "K1", "Q2", "K2")), cfg.c1, cfg.c2, cfg.causal,
+                       g=gnp.astype(np.float64), teacher=True)
+    kl, l1, l2 = skl.streamkl_fwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, cfg.causal)
+    counts = {}
+    try:
+        for mode in (skl.STREAMKL_BWD_FUSED, skl.STREAMKL_BWD_SEPARATE):
+            skl.streamkl_set_bwd_mode(mode)
+            grads = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, cfg.causal, kl, l1, l2, g, teacher=True)
+            counts[mode] = skl.streamkl_last_launch_count()
+            for name, t in zip(("dQ1", "dK1", "dQ2", "dK2"), grads):
+                check_grad_heads(to_f64(t), ref[name], f"mode {mode} {name}")
+    finally:
+        skl.streamkl_set_bwd_mode(skl.STREAMKL_BWD_AUTO)
+    assert counts[skl.STREAMKL_BWD_FUSED] == 5 and counts[skl.STREAMKL_BWD_SEPARATE] == 3   # {stats, 2 x (fused, convert)} / {stats, dQ, dK}
 
 
 def test_setting1_fused_mixed_sign_upstream_gradient_and_tiny_sizes():
