@@ -14,11 +14,13 @@
  * with g = dkl_rows[i] the upstream gradient (dL in Alg.2/3).  No N_Q x N_K intermediate is ever written to HBM.
  *
  * Conventions (all entry points):
- *  - Tensors are contiguous row-major [B][H][N][d] ("bsz" = B*H flattened); per-row vectors are
- *    [B][H][NQ] float32.  Outputs are in natural-log units.  Same H for all four tensors (no GQA).
- *  - `*_bf16` / `*_f32` name the element type of Q1,K1,Q2,K2 and of the gradient outputs (one rounding from
- *    fp32 accumulators).  All accumulation is fp32.  bf16 with d1,d2 in {64,128} runs the tcgen05/TMA kernels;
- *    every other case (fp32 inputs, other head dims <= 256) runs the SIMT fp32 kernels.
+ *  - Tensors are contiguous row-major [B][H][N][d] ("bsz" = B*H flattened) unless a streamkl_layout says
+ *    otherwise (strided tensors, K heads shared by groups of query heads: the `*_ex` entry points); per-row vectors are
+ *    always contiguous [B][H][NQ] float32.  Outputs are in natural-log units.
+ *  - The plain entry points take bf16, `*_f32` fp32, `*_ex` the element type named in the layout (bf16 / fp16 / fp32); gradients
+ *    come back in the input type (one rounding from fp32 accumulators).  All accumulation is fp32.  16-bit inputs with d1, d2
+ *    multiples of 8 up to 128 run the tcgen05/TMA kernels (head dims other than 64 / 128 zero-padded to the next of the two);
+ *    every other case (fp32 inputs, head dims up to 256 that are not multiples of 8 or exceed 128) runs the SIMT fp32 kernels.
  *  - Device entry points take DEVICE pointers owned by the caller; the library never allocates, frees or
  *    retains them, and only enqueues work on `stream` (asynchronous; device faults surface at the caller's next
  *    synchronisation).  `*_host` entry points take HOST pointers, allocate their own device scratch, copy in,
@@ -56,7 +58,7 @@ enum {
   STREAMKL_ERR_DTYPE = -7      /* unknown dtype code */
 };
 
-enum { STREAMKL_BF16 = 0, STREAMKL_F32 = 1 };
+enum { STREAMKL_BF16 = 0, STREAMKL_F32 = 1, STREAMKL_F16 = 2 };
 
 /*
  * Forward (Algorithm 1).  Device pointers.
@@ -70,6 +72,35 @@ int streamkl_fwd(const void* Q1, const void* K1, const void* Q2, const void* K2,
 int streamkl_fwd_f32(const void* Q1, const void* K1, const void* Q2, const void* K2,
                      int B, int H, int NQ, int NK, int d1, int d2, float c1, float c2, int causal,
                      float* kl_rows, float* lse1, float* lse2, streamkl_stream_t stream);      /* fp32 inputs */
+
+/*
+ * Layouts beyond contiguous [B][H][N][d] (the paper itself only has [bsz, N, d]).
+ *   dtype      : STREAMKL_BF16 | STREAMKL_F16 (| STREAMKL_F32: default layout only) -- element type of Q1,K1,Q2,K2 and of the gradients.
+ *   kv_heads   : HK, the number of K heads; 0 = H.  H must be a multiple of HK; query head h reads K head h / (H/HK) ("grouped-query"
+ *                sharing; K tensors are then [B][HK][NK][d] and dK sums over the H/HK query heads of each group).
+ *   *_stride   : ELEMENT strides {batch, head, row} of each input; the head dimension is contiguous (stride 1).  All zero = the
+ *                contiguous default for that tensor ([B][H][N][d], or [B][HK][NK][d] for K).  E.g. a [B][N][H][d] tensor is
+ *                {N*H*d, d, H*d}.  Strides must be multiples of 8 elements (16 bytes, TMA) and the row stride >= d.
+ *                dQ_t is written with Q_t's strides, dK_t with K_t's; kl_rows / lse / dkl_rows stay contiguous [B][H][NQ].
+ * Non-default strides and kv_heads need the tensor-core path: 16-bit dtype and d1, d2 multiples of 8 up to 128 (STREAMKL_ERR_SHAPE
+ * otherwise).  Head dims other than 64 / 128 run zero-padded to the next of the two inside the kernels (TMA zero fill): the
+ * results are exact, the padded columns cost tensor work.
+ */
+typedef struct streamkl_layout {
+  int dtype;
+  int kv_heads;
+  long long q1_stride[3], k1_stride[3], q2_stride[3], k2_stride[3];
+} streamkl_layout;
+
+/* streamkl_fwd / streamkl_bwd with an explicit layout (NULL = bf16, contiguous, HK = H: identical to the plain entry points). */
+int streamkl_fwd_ex(const streamkl_layout* layout, const void* Q1, const void* K1, const void* Q2, const void* K2,
+                    int B, int H, int NQ, int NK, int d1, int d2, float c1, float c2, int causal,
+                    float* kl_rows, float* lse1, float* lse2, streamkl_stream_t stream);
+int streamkl_bwd_ex(const streamkl_layout* layout, const void* Q1, const void* K1, const void* Q2, const void* K2,
+                    int B, int H, int NQ, int NK, int d1, int d2, float c1, float c2, int causal,
+                    const float* kl_rows, const float* lse1, const float* lse2, const float* dkl_rows,
+                    void* dQ1, void* dK1, void* dQ2, void* dK2,
+                    void* workspace, size_t workspace_bytes, streamkl_stream_t stream);
 
 /*
  * Split-K forward for small NQ (Eq.11; bf16, d1,d2 in {64,128}).  The key range is cut into W

@@ -19,6 +19,10 @@ from .binding import (  # noqa: F401
     STREAMKL_BWD_AUTO,
     STREAMKL_BWD_SEPARATE,
     STREAMKL_BWD_FUSED,
+    STREAMKL_BF16,
+    STREAMKL_F16,
+    STREAMKL_F32,
+    StreamKLLayout,
     streamkl_fwd_splitk_splits,
     streamkl_fwd_splitk_workspace_bytes,
     streamkl_kernel_name,

@@ -16,12 +16,19 @@ __all__ = [
     "StreamKLError", "lib", "lib_path", "streamkl_fwd", "streamkl_bwd", "streamkl_bwd_workspace_bytes",
     "streamkl_fwd_splitk", "streamkl_fwd_splitk_splits", "streamkl_fwd_splitk_workspace_bytes",
     "streamkl_fwd_host", "streamkl_fwd_bwd_host", "streamkl_host_trim", "streamkl_set_bwd_mode",
-    "STREAMKL_BWD_AUTO", "STREAMKL_BWD_SEPARATE", "STREAMKL_BWD_FUSED", "streamkl_last_launch_count", "streamkl_strerror",
+    "STREAMKL_BWD_AUTO", "STREAMKL_BWD_SEPARATE", "STREAMKL_BWD_FUSED", "STREAMKL_BF16", "STREAMKL_F16", "STREAMKL_F32", "StreamKLLayout", "streamkl_last_launch_count", "streamkl_strerror",
     "streamkl_profile_enable", "streamkl_profile_collect", "streamkl_kernel_name",
     "streamkl_version",
 ]
 
-STREAMKL_BF16, STREAMKL_F32 = 0, 1
+STREAMKL_BF16, STREAMKL_F32, STREAMKL_F16 = 0, 1, 2
+
+
+class StreamKLLayout(ctypes.Structure):
+    """struct streamkl_layout of include/streamkl.h."""
+
+    _fields_ = [("dtype", ctypes.c_int), ("kv_heads", ctypes.c_int), ("q1_stride", ctypes.c_longlong * 3),
+                ("k1_stride", ctypes.c_longlong * 3), ("q2_stride", ctypes.c_longlong * 3), ("k2_stride", ctypes.c_longlong * 3)]
 STREAMKL_BWD_AUTO, STREAMKL_BWD_SEPARATE, STREAMKL_BWD_FUSED = 0, 1, 2
 
 
@@ -58,6 +65,10 @@ def lib() -> ctypes.CDLL:
         f = getattr(L, name)
         f.argtypes = [vp] * 4 + shape + [vp] * 4 + [vp] * 4 + [vp, sz, vp]
         f.restype = ci
+    L.streamkl_fwd_ex.argtypes = [vp] + [vp] * 4 + shape + [vp] * 3 + [vp]
+    L.streamkl_fwd_ex.restype = ci
+    L.streamkl_bwd_ex.argtypes = [vp] + [vp] * 4 + shape + [vp] * 4 + [vp] * 4 + [vp, sz, vp]
+    L.streamkl_bwd_ex.restype = ci
     L.streamkl_fwd_splitk.argtypes = [vp] * 4 + shape + [ci] + [vp] * 3 + [vp, sz, vp]
     L.streamkl_fwd_splitk.restype = ci
     L.streamkl_fwd_splitk_splits.argtypes = [ci] * 5
@@ -146,23 +157,56 @@ def _keep_alive_on(t, stream):
         t.record_stream(stream)
 
 
-def _check_dev(name, t, dtype=None):
+def _check_dev(name, t, dtype=None, strided=False):
     import torch
 
-    if not isinstance(t, torch.Tensor) or not t.is_cuda or not t.is_contiguous():
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{name}: expected a CUDA torch tensor")
+    if strided:
+        if t.dim() != 4 or (t.shape[-1] > 1 and t.stride(-1) != 1):
+            raise TypeError(f"{name}: expected a [B,H,N,d] CUDA tensor whose last dimension is contiguous")
+    elif not t.is_contiguous():
         raise TypeError(f"{name}: expected a contiguous CUDA torch tensor")
     if dtype is not None and t.dtype != dtype:
         raise TypeError(f"{name}: expected dtype {dtype}, got {t.dtype}")
 
 
 def _shape_of(Q1, K1, Q2, K2):
+    """-> (B, H, NQ, NK, d1, d2, HK): K tensors may carry HK <= H heads (H % HK == 0; query head h reads K head h // (H // HK))."""
     if Q1.dim() != 4 or K1.dim() != 4 or Q2.dim() != 4 or K2.dim() != 4:
         raise ValueError("Q1,K1,Q2,K2 must be [B,H,N,d]")
     B, H, NQ, d1 = Q1.shape
-    NK, d2 = K1.shape[2], Q2.shape[3]
-    if tuple(K1.shape) != (B, H, NK, d1) or tuple(Q2.shape) != (B, H, NQ, d2) or tuple(K2.shape) != (B, H, NK, d2):
+    HK, NK, d2 = K1.shape[1], K1.shape[2], Q2.shape[3]
+    if tuple(K1.shape) != (B, HK, NK, d1) or tuple(Q2.shape) != (B, H, NQ, d2) or tuple(K2.shape) != (B, HK, NK, d2):
         raise ValueError("inconsistent Q1,K1,Q2,K2 shapes")
-    return B, H, NQ, NK, d1, d2
+    if HK < 1 or H % HK != 0:
+        raise ValueError("the number of query heads must be a multiple of the number of K heads")
+    return B, H, NQ, NK, d1, d2, HK
+
+
+def _layout_of(Q1, K1, Q2, K2, HK):
+    """A StreamKLLayout for 16-bit tensors given as (possibly strided) [B,H,N,d] views, or None when everything is the
+    contiguous bf16 / fp32 default that the plain entry points take."""
+    import torch
+
+    plain = all(t.is_contiguous() for t in (Q1, K1, Q2, K2)) and HK == Q1.shape[1]
+    if plain and Q1.dtype in (torch.bfloat16, torch.float32):
+        return None
+    if Q1.dtype not in (torch.bfloat16, torch.float16):
+        raise TypeError("strided tensors / shared K heads need bfloat16 or float16 inputs")
+    L = StreamKLLayout()
+    L.dtype = STREAMKL_BF16 if Q1.dtype == torch.bfloat16 else STREAMKL_F16
+    L.kv_heads = int(HK)
+    for name, t in (("q1_stride", Q1), ("k1_stride", K1), ("q2_stride", Q2), ("k2_stride", K2)):
+        arr = getattr(L, name)
+        _, heads, n, d = t.shape
+        sb, sh, sn, _ = t.stride()
+        # torch leaves the stride of a size-1 axis arbitrary: substitute the packed value (it is never used to move)
+        sn = sn if n > 1 else d
+        sh = sh if heads > 1 else n * sn
+        sb = sb if t.shape[0] > 1 else heads * sh
+        arr[0], arr[1], arr[2] = int(sb), int(sh), int(sn)
+    return L
 
 
 def _stream_handle(stream):
@@ -178,27 +222,29 @@ def _ptr(t):
 
 
 def streamkl_fwd(Q1, K1, Q2, K2, c1, c2, causal, kl_rows=None, lse1=None, lse2=None, stream=None):
-    """Forward (Algorithm 1).  Returns (kl_rows, lse1, lse2), each [B,H,NQ] float32.  bf16 or fp32 inputs."""
+    """Forward (Algorithm 1).  Returns (kl_rows, lse1, lse2), each [B,H,NQ] float32.  bf16 / fp16 / fp32 inputs; 16-bit inputs
+    may be strided [B,H,N,d] views (last dimension contiguous) and K may have fewer heads than Q (shared K heads)."""
     import torch
 
     for n, t in (("Q1", Q1), ("K1", K1), ("Q2", Q2), ("K2", K2)):
-        _check_dev(n, t, Q1.dtype)
-    B, H, NQ, NK, d1, d2 = _shape_of(Q1, K1, Q2, K2)
+        _check_dev(n, t, Q1.dtype, strided=True)
+    B, H, NQ, NK, d1, d2, HK = _shape_of(Q1, K1, Q2, K2)
+    layout = _layout_of(Q1, K1, Q2, K2, HK)
     outs = []
     for n, t in (("kl_rows", kl_rows), ("lse1", lse1), ("lse2", lse2)):
         if t is None:
             t = torch.empty((B, H, NQ), dtype=torch.float32, device=Q1.device)
         _check_dev(n, t, torch.float32)
         outs.append(t)
-    if Q1.dtype == torch.bfloat16:
-        fn = lib().streamkl_fwd
-    elif Q1.dtype == torch.float32:
-        fn = lib().streamkl_fwd_f32
-    else:
-        raise TypeError("inputs must be bfloat16 or float32")
+    args = (_ptr(Q1), _ptr(K1), _ptr(Q2), _ptr(K2), B, H, NQ, NK, d1, d2, float(c1), float(c2), int(bool(causal)),
+            _ptr(outs[0]), _ptr(outs[1]), _ptr(outs[2]), _stream_handle(stream))
     with torch.cuda.device(Q1.device):
-        rc = fn(_ptr(Q1), _ptr(K1), _ptr(Q2), _ptr(K2), B, H, NQ, NK, d1, d2, float(c1), float(c2), int(bool(causal)),
-                _ptr(outs[0]), _ptr(outs[1]), _ptr(outs[2]), _stream_handle(stream))
+        if layout is not None:
+            rc = lib().streamkl_fwd_ex(ctypes.cast(ctypes.pointer(layout), ctypes.c_void_p), *args)
+        elif Q1.dtype == torch.bfloat16:
+            rc = lib().streamkl_fwd(*args)
+        else:
+            rc = lib().streamkl_fwd_f32(*args)
     if rc != 0:
         raise StreamKLError(rc, "streamkl_fwd")
     return tuple(outs)
@@ -218,7 +264,9 @@ def streamkl_fwd_splitk(Q1, K1, Q2, K2, c1, c2, causal, splits=0, kl_rows=None, 
 
     for n, t in (("Q1", Q1), ("K1", K1), ("Q2", Q2), ("K2", K2)):
         _check_dev(n, t, torch.bfloat16)
-    B, H, NQ, NK, d1, d2 = _shape_of(Q1, K1, Q2, K2)
+    B, H, NQ, NK, d1, d2, HK = _shape_of(Q1, K1, Q2, K2)
+    if HK != H:
+        raise ValueError("streamkl_fwd_splitk: shared K heads are not supported")
     outs = []
     for n, t in (("kl_rows", kl_rows), ("lse1", lse1), ("lse2", lse2)):
         if t is None:
@@ -246,39 +294,44 @@ def streamkl_bwd(Q1, K1, Q2, K2, c1, c2, causal, kl_rows, lse1, lse2, dkl_rows, 
     import torch
 
     for n, t in (("Q1", Q1), ("K1", K1), ("Q2", Q2), ("K2", K2)):
-        _check_dev(n, t, Q1.dtype)
+        _check_dev(n, t, Q1.dtype, strided=True)
     for n, t in (("kl_rows", kl_rows), ("lse1", lse1), ("lse2", lse2), ("dkl_rows", dkl_rows)):
         _check_dev(n, t, torch.float32)
-    B, H, NQ, NK, d1, d2 = _shape_of(Q1, K1, Q2, K2)
+    B, H, NQ, NK, d1, d2, HK = _shape_of(Q1, K1, Q2, K2)
+    layout = _layout_of(Q1, K1, Q2, K2, HK)
+    # every gradient has the shape AND the strides of its input (dQ_t like Q_t, dK_t like K_t)
+    like = lambda t: torch.empty_strided(t.shape, t.stride(), dtype=t.dtype, device=t.device)
     if dQ2 is None:
-        dQ2 = torch.empty_like(Q2)
+        dQ2 = like(Q2)
     if dK2 is None:
-        dK2 = torch.empty_like(K2)
+        dK2 = like(K2)
     if teacher:
         if dQ1 is None:
-            dQ1 = torch.empty_like(Q1)
+            dQ1 = like(Q1)
         if dK1 is None:
-            dK1 = torch.empty_like(K1)
+            dK1 = like(K1)
     else:
         dQ1 = dK1 = None
-    for n, t in (("dQ1", dQ1), ("dK1", dK1), ("dQ2", dQ2), ("dK2", dK2)):
+    for n, t, src in (("dQ1", dQ1, Q1), ("dK1", dK1, K1), ("dQ2", dQ2, Q2), ("dK2", dK2, K2)):
         if t is not None:
-            _check_dev(n, t, Q1.dtype)
+            _check_dev(n, t, Q1.dtype, strided=True)
+            if tuple(t.shape) != tuple(src.shape) or tuple(t.stride()) != tuple(src.stride()):
+                raise ValueError(f"{n}: must have the shape and strides of its input")
     need = streamkl_bwd_workspace_bytes(B, H, NQ, NK, d1, d2, teacher)
     if need > 0 and (workspace is None or workspace.numel() * workspace.element_size() < need):
         workspace = torch.empty(need, dtype=torch.uint8, device=Q1.device)
         _keep_alive_on(workspace, stream)
     ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
-    if Q1.dtype == torch.bfloat16:
-        fn = lib().streamkl_bwd
-    elif Q1.dtype == torch.float32:
-        fn = lib().streamkl_bwd_f32
-    else:
-        raise TypeError("inputs must be bfloat16 or float32")
+    args = (_ptr(Q1), _ptr(K1), _ptr(Q2), _ptr(K2), B, H, NQ, NK, d1, d2, float(c1), float(c2), int(bool(causal)),
+            _ptr(kl_rows), _ptr(lse1), _ptr(lse2), _ptr(dkl_rows), _ptr(dQ1), _ptr(dK1), _ptr(dQ2), _ptr(dK2),
+            _ptr(workspace), ctypes.c_size_t(ws_bytes), _stream_handle(stream))
     with torch.cuda.device(Q1.device):
-        rc = fn(_ptr(Q1), _ptr(K1), _ptr(Q2), _ptr(K2), B, H, NQ, NK, d1, d2, float(c1), float(c2), int(bool(causal)),
-                _ptr(kl_rows), _ptr(lse1), _ptr(lse2), _ptr(dkl_rows), _ptr(dQ1), _ptr(dK1), _ptr(dQ2), _ptr(dK2),
-                _ptr(workspace), ctypes.c_size_t(ws_bytes), _stream_handle(stream))
+        if layout is not None:
+            rc = lib().streamkl_bwd_ex(ctypes.cast(ctypes.pointer(layout), ctypes.c_void_p), *args)
+        elif Q1.dtype == torch.bfloat16:
+            rc = lib().streamkl_bwd(*args)
+        else:
+            rc = lib().streamkl_bwd_f32(*args)
     if rc != 0:
         raise StreamKLError(rc, "streamkl_bwd")
     return dQ1, dK1, dQ2, dK2

@@ -89,6 +89,15 @@ __device__ __forceinline__ void tma_load_3d_hint(void* smem_dst, const CUtensorM
       ::"r"(smem_u32(smem_dst)), "l"(reinterpret_cast<uint64_t>(m)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "l"(policy)
       : "memory");
 }
+// 4-D tiled load {d, row, head, batch}: every tensor is addressed through a 4-D map so that arbitrary (batch, head, row)
+// strides -- [B][H][N][d], [B][N][H][d], views of packed QKV buffers -- need no second code path.
+__device__ __forceinline__ void tma_load_4d_hint(void* smem_dst, const CUtensorMap* m, uint64_t* bar, int c0, int c1, int c2, int c3,
+                                                 uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%3, %4, %5, %6}], [%2], %7;"
+      ::"r"(smem_u32(smem_dst)), "l"(reinterpret_cast<uint64_t>(m)), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "l"(policy)
+      : "memory");
+}
 // 1-D bulk copy global -> shared (size multiple of 16 B, both addresses 16-byte aligned), completion on an mbarrier.
 __device__ __forceinline__ void bulk_load_1d(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -153,6 +162,12 @@ __host__ __device__ constexpr uint32_t umma_idesc_bf16(int M, int N, int a_mn, i
          | (1u << 7) | (1u << 10)                // A, B format bf16
          | (uint32_t(a_mn) << 15) | (uint32_t(b_mn) << 16)
          | (uint32_t(N >> 3) << 17) | (uint32_t(M >> 4) << 24);
+}
+
+// The same with the 16-bit operand format chosen at run time: fmt16 = 1 bf16, 0 fp16 (kind::f16 covers both).
+__host__ __device__ constexpr uint32_t umma_idesc_16(int M, int N, int a_mn, int b_mn, uint32_t fmt16) {
+  return (1u << 4) | (fmt16 << 7) | (fmt16 << 10) | (uint32_t(a_mn) << 15) | (uint32_t(b_mn) << 16) | (uint32_t(N >> 3) << 17) |
+         (uint32_t(M >> 4) << 24);
 }
 
 // Shared-memory matrix descriptor, 128-byte swizzle, descriptor version 1 (sm_100).

@@ -85,23 +85,66 @@ bool device_is_sm100() {
   return major == 10;
 }
 
-// [BH][N][d] bf16 row-major tensor, box = {64 elements (128 B), box_rows, 1}, 128-byte swizzle, zero OOB fill.
-bool make_tmap_bf16(CUtensorMap* m, const void* base, int BH, int N, int d, int box_rows) {
+// Element strides {batch, head, row} of one tensor (the head dimension is contiguous).
+struct Strides { long long b, h, n; };
+
+// 4-D map {d, N, heads, B} of a 16-bit tensor with arbitrary (batch, head, row) strides; box = {64 elements (128 B), box_rows, 1, 1},
+// 128-byte swizzle, zero OOB fill: rows beyond N and columns beyond d (head dims that are not 64 / 128) arrive as zeros.
+bool make_tmap_16(CUtensorMap* m, const void* base, int B, int heads, int N, int d, const Strides& st, int box_rows, bool f16) {
   EncodeTiledFn enc = get_encode_fn();
   if (!enc) return false;
-  cuuint64_t dims[3] = {cuuint64_t(d), cuuint64_t(N), cuuint64_t(BH)};
-  cuuint64_t strides[2] = {cuuint64_t(d) * 2, cuuint64_t(N) * cuuint64_t(d) * 2};
-  cuuint32_t box[3] = {64, cuuint32_t(box_rows), 1};
-  cuuint32_t estr[3] = {1, 1, 1};
-  return enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
-             CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+  cuuint64_t dims[4] = {cuuint64_t(d), cuuint64_t(N), cuuint64_t(heads), cuuint64_t(B)};
+  cuuint64_t strides[3] = {cuuint64_t(st.n) * 2, cuuint64_t(st.h) * 2, cuuint64_t(st.b) * 2};
+  cuuint32_t box[4] = {64, cuuint32_t(box_rows), 1, 1};
+  cuuint32_t estr[4] = {1, 1, 1, 1};
+  return enc(m, f16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(base), dims, strides, box,
+             estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 struct Shape {
   int B, H, NQ, NK, d1, d2, causal;
   float c1, c2;
   long long BH;
+  // layout (streamkl_layout): K heads, element strides of Q1, K1, Q2, K2 (gradients share their input's strides)
+  int HK = 0;
+  Strides q1{}, k1{}, q2{}, k2{};
+  bool default_layout = true;
+  int G() const { return HK > 0 ? H / HK : 1; }
 };
+
+Strides contiguous(int heads, int N, int d) { return Strides{(long long)heads * N * d, (long long)N * d, (long long)d}; }
+
+// fills the layout part of `s` from `L` (NULL = contiguous [B][H][N][d], HK = H) and validates it
+int apply_layout(Shape& s, const streamkl_layout* L) {
+  s.HK = s.H;
+  s.q1 = contiguous(s.H, s.NQ, s.d1); s.k1 = contiguous(s.H, s.NK, s.d1);
+  s.q2 = contiguous(s.H, s.NQ, s.d2); s.k2 = contiguous(s.H, s.NK, s.d2);
+  s.default_layout = true;
+  if (!L) return STREAMKL_OK;
+  if (L->kv_heads < 0) return STREAMKL_ERR_SHAPE;
+  if (L->kv_heads > 0) {
+    if (s.H > 0 && (L->kv_heads > s.H || s.H % L->kv_heads != 0)) return STREAMKL_ERR_SHAPE;
+    s.HK = L->kv_heads;
+    s.k1 = contiguous(s.HK, s.NK, s.d1); s.k2 = contiguous(s.HK, s.NK, s.d2);
+  }
+  auto take = [&](const long long (&v)[3], Strides& dst, int d, int N) -> int {
+    if (v[0] == 0 && v[1] == 0 && v[2] == 0) return STREAMKL_OK;          // default for this tensor
+    if (v[0] < 0 || v[1] < 0 || v[2] < d) return STREAMKL_ERR_SHAPE;       // rows must not overlap; broadcast batch / head (0) is allowed
+    if ((v[0] | v[1] | v[2]) & 7) return STREAMKL_ERR_ALIGN;               // 16-byte multiples (TMA global strides)
+    (void)N;
+    dst = Strides{v[0], v[1], v[2]};
+    return STREAMKL_OK;
+  };
+  int rc;
+  if ((rc = take(L->q1_stride, s.q1, s.d1, s.NQ)) != STREAMKL_OK || (rc = take(L->k1_stride, s.k1, s.d1, s.NK)) != STREAMKL_OK ||
+      (rc = take(L->q2_stride, s.q2, s.d2, s.NQ)) != STREAMKL_OK || (rc = take(L->k2_stride, s.k2, s.d2, s.NK)) != STREAMKL_OK)
+    return rc;
+  auto same = [](const Strides& a, const Strides& b) { return a.b == b.b && a.h == b.h && a.n == b.n; };
+  s.default_layout = s.HK == s.H && same(s.q1, contiguous(s.H, s.NQ, s.d1)) && same(s.k1, contiguous(s.H, s.NK, s.d1)) &&
+                     same(s.q2, contiguous(s.H, s.NQ, s.d2)) && same(s.k2, contiguous(s.H, s.NK, s.d2));
+  return STREAMKL_OK;
+}
 
 int validate_common(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s) {
   if (s.B < 0 || s.H < 0 || s.NQ < 0 || s.NK < 1 || s.d1 < 1 || s.d2 < 1 || s.d1 > 256 || s.d2 > 256) return STREAMKL_ERR_SHAPE;
@@ -116,21 +159,29 @@ int validate_common(const void* Q1, const void* K1, const void* Q2, const void* 
   return STREAMKL_OK;
 }
 
+// tensor-core path: 16-bit inputs, head dims that are multiples of 8 (TMA: 16-byte rows) up to 128.  The kernels are
+// instantiated for head dims 64 and 128; anything else runs zero-padded to the next of the two (pad_dim).
 bool tc_shape(int dtype, const Shape& s) {
-  return dtype == STREAMKL_BF16 && (s.d1 == 64 || s.d1 == 128) && (s.d2 == 64 || s.d2 == 128);
+  return (dtype == STREAMKL_BF16 || dtype == STREAMKL_F16) && s.d1 % 8 == 0 && s.d2 % 8 == 0 && s.d1 <= 128 && s.d2 <= 128;
+}
+int pad_dim(int d) { return d <= 64 ? 64 : 128; }
+
+bool make_maps(CUtensorMap (&t)[4], const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, int rows_q, int rows_k,
+               bool f16) {
+  return make_tmap_16(&t[0], Q1, s.B, s.H, s.NQ, s.d1, s.q1, rows_q, f16) && make_tmap_16(&t[1], K1, s.B, s.HK, s.NK, s.d1, s.k1, rows_k, f16) &&
+         make_tmap_16(&t[2], Q2, s.B, s.H, s.NQ, s.d2, s.q2, rows_q, f16) && make_tmap_16(&t[3], K2, s.B, s.HK, s.NK, s.d2, s.k2, rows_k, f16);
 }
 
 // ----------------------------------------------------------------------------------------- forward launchers
 // splits == 1: the default kernel (grid (bsz, T_Q)).  splits > 1: split-K (grid (bsz, T_Q, W), partial
 // statistics to `part`, then the reduce kernel).
 template <int D1, int D2, bool CAUSAL, bool SPLIT = false>
-int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, float* kl, float* lse1, float* lse2,
-                  cudaStream_t stream, int splits = 1, float* part = nullptr) {
+int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, float* kl, float* lse1,
+                  float* lse2, cudaStream_t stream, int splits = 1, float* part = nullptr) {
   using C = skl::FwdCfg<D1, D2>;
-  CUtensorMap tQ1, tK1, tQ2, tK2;
-  if (!make_tmap_bf16(&tQ1, Q1, int(s.BH), s.NQ, D1, C::BM) || !make_tmap_bf16(&tK1, K1, int(s.BH), s.NK, D1, C::BK) ||
-      !make_tmap_bf16(&tQ2, Q2, int(s.BH), s.NQ, D2, C::BM) || !make_tmap_bf16(&tK2, K2, int(s.BH), s.NK, D2, C::BK))
-    return STREAMKL_ERR_CUDA;
+  CUtensorMap tm[4];
+  if (!make_maps(tm, Q1, K1, Q2, K2, s, C::BM, C::BK, f16)) return STREAMKL_ERR_CUDA;
+  const CUtensorMap &tQ1 = tm[0], &tK1 = tm[1], &tQ2 = tm[2], &tK2 = tm[3];
   auto kern = skl::streamkl_fwd_sm100_kernel<D1, D2, CAUSAL, SPLIT>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
     cudaGetLastError();
@@ -138,6 +189,7 @@ int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2
   }
   skl::FwdParams p;
   p.NQ = s.NQ; p.NK = s.NK; p.BH = int(s.BH);
+  p.H = s.H; p.G = s.G(); p.fmt16 = f16 ? 0u : 1u;
   p.TQ = (s.NQ + C::BQ - 1) / C::BQ;
   p.sc1 = s.c1 * 1.4426950408889634f;
   p.sc2 = s.c2 * 1.4426950408889634f;
@@ -197,25 +249,29 @@ int launch_fwd_simt(const void* Q1, const void* K1, const void* Q2, const void* 
   return STREAMKL_OK;
 }
 
-int fwd_dispatch(int dtype, const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1,
-                 int d2, float c1, float c2, int causal, float* kl, float* lse1, float* lse2, cudaStream_t stream, int splits = 1,
-                 float* part = nullptr) {
+int fwd_dispatch(int dtype, const streamkl_layout* L, const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ,
+                 int NK, int d1, int d2, float c1, float c2, int causal, float* kl, float* lse1, float* lse2, cudaStream_t stream,
+                 int splits = 1, float* part = nullptr) {
+  if (dtype != STREAMKL_BF16 && dtype != STREAMKL_F16 && dtype != STREAMKL_F32) return STREAMKL_ERR_DTYPE;
   Shape s{B, H, NQ, NK, d1, d2, causal ? 1 : 0, c1, c2, (long long)B * (long long)H};
   int rc = validate_common(Q1, K1, Q2, K2, s);
   if (rc != STREAMKL_OK) return rc;
+  if ((rc = apply_layout(s, L)) != STREAMKL_OK) return rc;
   g_last_launches = 0;
   if (s.BH == 0 || s.NQ == 0) return STREAMKL_OK;
   if (!kl || !lse1 || !lse2) return STREAMKL_ERR_NULLPTR;
+  if (!tc_shape(dtype, s) && !s.default_layout) return STREAMKL_ERR_SHAPE;   // strides / shared K heads: tensor-core path only
   if (!device_is_sm100()) return STREAMKL_ERR_CUDA;
-  if (s.BH > 65535) return STREAMKL_ERR_SHAPE;
   if (tc_shape(dtype, s)) {
-#define SKL_FWD_CASE(A, Bd)                                                                                                  \
-  if (d1 == A && d2 == Bd) {                                                                                                 \
-    if (splits > 1)                                                                                                          \
-      return s.causal ? launch_fwd_tc<A, Bd, true, true>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream, splits, part)            \
-                      : launch_fwd_tc<A, Bd, false, true>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream, splits, part);          \
-    return s.causal ? launch_fwd_tc<A, Bd, true>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream)                                  \
-                    : launch_fwd_tc<A, Bd, false>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream);                                \
+    const bool f16 = dtype == STREAMKL_F16;
+    const int p1 = pad_dim(d1), p2 = pad_dim(d2);
+#define SKL_FWD_CASE(A, Bd)                                                                                                       \
+  if (p1 == A && p2 == Bd) {                                                                                                      \
+    if (splits > 1)                                                                                                               \
+      return s.causal ? launch_fwd_tc<A, Bd, true, true>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream, splits, part)            \
+                      : launch_fwd_tc<A, Bd, false, true>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream, splits, part);          \
+    return s.causal ? launch_fwd_tc<A, Bd, true>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream)                                  \
+                    : launch_fwd_tc<A, Bd, false>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream);                                \
   }
     SKL_FWD_CASE(128, 128)
     SKL_FWD_CASE(128, 64)
@@ -223,9 +279,10 @@ int fwd_dispatch(int dtype, const void* Q1, const void* K1, const void* Q2, cons
     SKL_FWD_CASE(64, 64)
 #undef SKL_FWD_CASE
   }
+  if (s.BH > 65535) return STREAMKL_ERR_SHAPE;   // SIMT grids put the head index in gridDim.y
   if (dtype == STREAMKL_BF16) return launch_fwd_simt<__nv_bfloat16>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream);
-  if (dtype == STREAMKL_F32) return launch_fwd_simt<float>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream);
-  return STREAMKL_ERR_DTYPE;
+  if (dtype == STREAMKL_F16) return launch_fwd_simt<__half>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream);
+  return launch_fwd_simt<float>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream);
 }
 
 // ----------------------------------------------------------------------------------------- backward launchers
@@ -253,16 +310,16 @@ int launch_bwd_simt(const void* Q1, const void* K1, const void* Q2, const void* 
   return STREAMKL_OK;
 }
 
+skl::OutGeom out_geom(const Strides& st, int d) { return skl::OutGeom{st.b, st.h, st.n, d}; }
+
 template <int D1, int D2, bool CAUSAL, bool TEACHER, bool OWNER_K>
-int launch_bwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, const float4* stats, void* dX1,
+int launch_bwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, const float4* stats, void* dX1,
                   void* dX2, cudaStream_t stream) {
   using C = skl::BwdCfg<D1, D2, TEACHER>;
-  CUtensorMap tQ1, tK1, tQ2, tK2;
+  CUtensorMap tm[4];
   // the owner side is loaded in 128-row boxes, the streamed side in BY-row boxes
   const int rq = OWNER_K ? C::BY : C::BX, rk = OWNER_K ? C::BX : C::BY;
-  if (!make_tmap_bf16(&tQ1, Q1, int(s.BH), s.NQ, D1, rq) || !make_tmap_bf16(&tK1, K1, int(s.BH), s.NK, D1, rk) ||
-      !make_tmap_bf16(&tQ2, Q2, int(s.BH), s.NQ, D2, rq) || !make_tmap_bf16(&tK2, K2, int(s.BH), s.NK, D2, rk))
-    return STREAMKL_ERR_CUDA;
+  if (!make_maps(tm, Q1, K1, Q2, K2, s, rq, rk, f16)) return STREAMKL_ERR_CUDA;
   auto kern = skl::streamkl_bwd_sm100_kernel<D1, D2, CAUSAL, TEACHER, OWNER_K>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
     cudaGetLastError();
@@ -270,16 +327,19 @@ int launch_bwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2
   }
   skl::BwdParams p;
   p.NQ = s.NQ; p.NK = s.NK; p.BH = int(s.BH);
+  p.H = s.H; p.HK = s.HK; p.G = s.G(); p.fmt16 = f16 ? 0u : 1u;
   p.TX = ((OWNER_K ? s.NK : s.NQ) + C::BX - 1) / C::BX;
   p.c1 = s.c1; p.c2 = s.c2;
   p.stats = stats;
-  p.dX1 = static_cast<__nv_bfloat16*>(dX1);
-  p.dX2 = static_cast<__nv_bfloat16*>(dX2);
-  const long long grid = (long long)p.TX * s.BH;
+  p.dX1 = static_cast<uint16_t*>(dX1);
+  p.dX2 = static_cast<uint16_t*>(dX2);
+  p.g1 = out_geom(OWNER_K ? s.k1 : s.q1, s.d1);   // dK_t has K_t's strides, dQ_t has Q_t's
+  p.g2 = out_geom(OWNER_K ? s.k2 : s.q2, s.d2);
+  const long long grid = (long long)p.TX * s.B * (OWNER_K ? s.HK : s.H);
   if (grid > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
   {
     ProfScope ps(OWNER_K ? KID_BWD_DK_TC : KID_BWD_DQ_TC, stream);
-    kern<<<dim3((unsigned)grid), C::THREADS, C::SMEM_BYTES, stream>>>(tQ1, tK1, tQ2, tK2, p);
+    kern<<<dim3((unsigned)grid), C::THREADS, C::SMEM_BYTES, stream>>>(tm[0], tm[1], tm[2], tm[3], p);
   }
   if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
   g_last_launches += 1;
@@ -301,13 +361,11 @@ size_t stats_bytes_aligned(long long BH, int NQ) { return (size_t(BH) * size_t(s
 // One one-visit pass: zero the fp32 dQ accumulator, run the fused K-owner kernel, convert dQ.
 // TPASS = false: student (dS2 -> dQ2, dK2); true: teacher (dS1 -> dQ1, dK1).
 template <int D1, int D2, bool CAUSAL, bool TPASS>
-int launch_bwd_fused(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, const float4* stats, float* dq_acc,
-                     void* dQ, void* dK, cudaStream_t stream) {
+int launch_bwd_fused(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, const float4* stats,
+                     float* dq_acc, void* dQ, void* dK, cudaStream_t stream) {
   using C = skl::BwdFusedCfg<D1, D2, TPASS>;
-  CUtensorMap tQ1, tK1, tQ2, tK2;
-  if (!make_tmap_bf16(&tQ1, Q1, int(s.BH), s.NQ, D1, C::BY) || !make_tmap_bf16(&tK1, K1, int(s.BH), s.NK, D1, C::BX) ||
-      !make_tmap_bf16(&tQ2, Q2, int(s.BH), s.NQ, D2, C::BY) || !make_tmap_bf16(&tK2, K2, int(s.BH), s.NK, D2, C::BX))
-    return STREAMKL_ERR_CUDA;
+  CUtensorMap tm[4];
+  if (!make_maps(tm, Q1, K1, Q2, K2, s, C::BY, C::BX, f16)) return STREAMKL_ERR_CUDA;
   auto kern = skl::streamkl_bwd_fused_sm100_kernel<D1, D2, CAUSAL, TPASS>;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
     cudaGetLastError();
@@ -317,22 +375,25 @@ int launch_bwd_fused(const void* Q1, const void* K1, const void* Q2, const void*
   if (cudaMemsetAsync(dq_acc, 0, n * sizeof(float), stream) != cudaSuccess) { cudaGetLastError(); return STREAMKL_ERR_CUDA; }
   skl::BwdFusedParams p;
   p.NQ = s.NQ; p.NK = s.NK; p.BH = int(s.BH);
+  p.H = s.H; p.HK = s.HK; p.G = s.G(); p.fmt16 = f16 ? 0u : 1u;
   p.TX = (s.NK + C::BX - 1) / C::BX;
   p.c1 = s.c1; p.c2 = s.c2;
   p.stats = stats; p.dq_acc = dq_acc;
-  p.dK = static_cast<__nv_bfloat16*>(dK);
-  const long long grid = (long long)p.TX * s.BH;
+  p.dK = static_cast<uint16_t*>(dK);
+  p.gk = out_geom(TPASS ? s.k1 : s.k2, TPASS ? s.d1 : s.d2);
+  const long long grid = (long long)p.TX * s.B * s.HK;
   if (grid > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
   {
     ProfScope ps(KID_BWD_FUSED_TC, stream);
-    kern<<<dim3((unsigned)grid), C::THREADS, C::SMEM_BYTES, stream>>>(tQ1, tK1, tQ2, tK2, p);
+    kern<<<dim3((unsigned)grid), C::THREADS, C::SMEM_BYTES, stream>>>(tm[0], tm[1], tm[2], tm[3], p);
   }
   if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
   const long long n4 = (long long)(n / 4);
   {
     ProfScope ps(KID_BWD_DQ_CONVERT, stream);
     skl::streamkl_bwd_dq_convert_kernel<<<dim3((unsigned)((n4 + 255) / 256)), 256, 0, stream>>>(
-        reinterpret_cast<const float4*>(dq_acc), static_cast<uint2*>(dQ), TPASS ? s.c1 * 0.6931471805599453f : s.c2, n4);
+        reinterpret_cast<const float4*>(dq_acc), static_cast<uint16_t*>(dQ), TPASS ? s.c1 * 0.6931471805599453f : s.c2, n4, s.NQ, s.H,
+        C::DG, out_geom(TPASS ? s.q1 : s.q2, TPASS ? s.d1 : s.d2), f16 ? 1 : 0);
   }
   if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
   g_last_launches += 2;
@@ -340,7 +401,7 @@ int launch_bwd_fused(const void* Q1, const void* K1, const void* Q2, const void*
 }
 
 template <int D1, int D2>
-int bwd_tc_both(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, const float* kl, const float* lse1,
+int bwd_tc_both(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, const float* kl, const float* lse1,
                 const float* lse2, const float* dkl, void* dQ1, void* dK1, void* dQ2, void* dK2, void* workspace, cudaStream_t st) {
   const bool t = dQ1 != nullptr;
   int rc;
@@ -367,27 +428,29 @@ int bwd_tc_both(const void* Q1, const void* K1, const void* Q2, const void* K2, 
     uint8_t* w = static_cast<uint8_t*>(workspace) + stats_bytes_aligned(s.BH, s.NQ);
     float* acc2 = reinterpret_cast<float*>(w);
     float* acc1 = reinterpret_cast<float*>(w + fused_acc_bytes_aligned(s.BH, s.NQ, D2));
-    rc = s.causal ? launch_bwd_fused<D1, D2, true, false>(Q1, K1, Q2, K2, s, stats, acc2, dQ2, dK2, st)
-                  : launch_bwd_fused<D1, D2, false, false>(Q1, K1, Q2, K2, s, stats, acc2, dQ2, dK2, st);
+    rc = s.causal ? launch_bwd_fused<D1, D2, true, false>(Q1, K1, Q2, K2, s, f16, stats, acc2, dQ2, dK2, st)
+                  : launch_bwd_fused<D1, D2, false, false>(Q1, K1, Q2, K2, s, f16, stats, acc2, dQ2, dK2, st);
     if (rc != STREAMKL_OK || !t) return rc;
-    return s.causal ? launch_bwd_fused<D1, D2, true, true>(Q1, K1, Q2, K2, s, stats, acc1, dQ1, dK1, st)
-                    : launch_bwd_fused<D1, D2, false, true>(Q1, K1, Q2, K2, s, stats, acc1, dQ1, dK1, st);
+    return s.causal ? launch_bwd_fused<D1, D2, true, true>(Q1, K1, Q2, K2, s, f16, stats, acc1, dQ1, dK1, st)
+                    : launch_bwd_fused<D1, D2, false, true>(Q1, K1, Q2, K2, s, f16, stats, acc1, dQ1, dK1, st);
   }
 #define SKL_BWD(CA, TE)                                                                                                   \
-  rc = launch_bwd_tc<D1, D2, CA, TE, false>(Q1, K1, Q2, K2, s, stats, dQ1, dQ2, st);                                      \
+  rc = launch_bwd_tc<D1, D2, CA, TE, false>(Q1, K1, Q2, K2, s, f16, stats, dQ1, dQ2, st);                                 \
   if (rc != STREAMKL_OK) return rc;                                                                                       \
-  return launch_bwd_tc<D1, D2, CA, TE, true>(Q1, K1, Q2, K2, s, stats, dK1, dK2, st);
+  return launch_bwd_tc<D1, D2, CA, TE, true>(Q1, K1, Q2, K2, s, f16, stats, dK1, dK2, st);
   if (s.causal) { if (t) { SKL_BWD(true, true) } else { SKL_BWD(true, false) } }
   else          { if (t) { SKL_BWD(false, true) } else { SKL_BWD(false, false) } }
 #undef SKL_BWD
 }
 
-int bwd_dispatch(int dtype, const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1,
-                 int d2, float c1, float c2, int causal, const float* kl, const float* lse1, const float* lse2, const float* dkl,
-                 void* dQ1, void* dK1, void* dQ2, void* dK2, void* workspace, size_t workspace_bytes, cudaStream_t stream) {
+int bwd_dispatch(int dtype, const streamkl_layout* L, const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ,
+                 int NK, int d1, int d2, float c1, float c2, int causal, const float* kl, const float* lse1, const float* lse2,
+                 const float* dkl, void* dQ1, void* dK1, void* dQ2, void* dK2, void* workspace, size_t workspace_bytes, cudaStream_t stream) {
+  if (dtype != STREAMKL_BF16 && dtype != STREAMKL_F16 && dtype != STREAMKL_F32) return STREAMKL_ERR_DTYPE;
   Shape s{B, H, NQ, NK, d1, d2, causal ? 1 : 0, c1, c2, (long long)B * (long long)H};
   int rc = validate_common(Q1, K1, Q2, K2, s);
   if (rc != STREAMKL_OK) return rc;
+  if ((rc = apply_layout(s, L)) != STREAMKL_OK) return rc;
   g_last_launches = 0;
   if ((dQ1 == nullptr) != (dK1 == nullptr)) return STREAMKL_ERR_NULLPTR;
   if (s.BH == 0) return STREAMKL_OK;
@@ -399,31 +462,37 @@ int bwd_dispatch(int dtype, const void* Q1, const void* K1, const void* Q2, cons
   const size_t need = streamkl_bwd_workspace_bytes(B, H, NQ, NK, d1, d2, dQ1 != nullptr);
   if (need > 0 && (!workspace || workspace_bytes < need)) return STREAMKL_ERR_WORKSPACE;
   if (reinterpret_cast<uintptr_t>(workspace) & 15) return STREAMKL_ERR_ALIGN;
+  if (!tc_shape(dtype, s) && !s.default_layout) return STREAMKL_ERR_SHAPE;   // strides / shared K heads: tensor-core path only
   if (!device_is_sm100()) return STREAMKL_ERR_CUDA;
-  if (s.BH > 65535) return STREAMKL_ERR_SHAPE;
-  const size_t es = dtype == STREAMKL_BF16 ? 2 : 4;
+  const size_t es = dtype == STREAMKL_F32 ? 4 : 2;
   if (s.NQ == 0) {  // no query rows: dK = 0, nothing else to write
+    if (!s.default_layout) return STREAMKL_ERR_SHAPE;
     if (cudaMemsetAsync(dK2, 0, size_t(s.BH) * NK * d2 * es, stream) != cudaSuccess) return STREAMKL_ERR_CUDA;
     if (dK1 && cudaMemsetAsync(dK1, 0, size_t(s.BH) * NK * d1 * es, stream) != cudaSuccess) return STREAMKL_ERR_CUDA;
     return STREAMKL_OK;
   }
   if (tc_shape(dtype, s)) {
-    if (d1 == 128 && d2 == 128) return bwd_tc_both<128, 128>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, workspace, stream);
-    if (d1 == 128 && d2 == 64) return bwd_tc_both<128, 64>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, workspace, stream);
-    if (d1 == 64 && d2 == 128) return bwd_tc_both<64, 128>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, workspace, stream);
-    if (d1 == 64 && d2 == 64) return bwd_tc_both<64, 64>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, workspace, stream);
+    const bool f16 = dtype == STREAMKL_F16;
+    const int p1 = pad_dim(d1), p2 = pad_dim(d2);
+    if (p1 == 128 && p2 == 128) return bwd_tc_both<128, 128>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, workspace, stream);
+    if (p1 == 128 && p2 == 64) return bwd_tc_both<128, 64>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, workspace, stream);
+    if (p1 == 64 && p2 == 128) return bwd_tc_both<64, 128>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, workspace, stream);
+    return bwd_tc_both<64, 64>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, workspace, stream);
   }
+  if (s.BH > 65535) return STREAMKL_ERR_SHAPE;   // SIMT grids put the head index in gridDim.y
   if (dtype == STREAMKL_BF16) {
     rc = launch_bwd_simt<__nv_bfloat16, false>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dQ2, stream);
     if (rc != STREAMKL_OK) return rc;
     return launch_bwd_simt<__nv_bfloat16, true>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dK1, dK2, stream);
   }
-  if (dtype == STREAMKL_F32) {
-    rc = launch_bwd_simt<float, false>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dQ2, stream);
+  if (dtype == STREAMKL_F16) {
+    rc = launch_bwd_simt<__half, false>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dQ2, stream);
     if (rc != STREAMKL_OK) return rc;
-    return launch_bwd_simt<float, true>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dK1, dK2, stream);
+    return launch_bwd_simt<__half, true>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dK1, dK2, stream);
   }
-  return STREAMKL_ERR_DTYPE;
+  rc = launch_bwd_simt<float, false>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dQ2, stream);
+  if (rc != STREAMKL_OK) return rc;
+  return launch_bwd_simt<float, true>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dK1, dK2, stream);
 }
 
 // Device scratch of the *_host entry points, taken from the device's stream-ordered pool.  The pool keeps freed blocks
@@ -477,26 +546,39 @@ extern "C" {
 
 int streamkl_fwd(const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1, int d2, float c1,
                  float c2, int causal, float* kl_rows, float* lse1, float* lse2, streamkl_stream_t stream) {
-  return fwd_dispatch(STREAMKL_BF16, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
+  return fwd_dispatch(STREAMKL_BF16, nullptr, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
                       static_cast<cudaStream_t>(stream));
 }
 int streamkl_fwd_f32(const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1, int d2,
                      float c1, float c2, int causal, float* kl_rows, float* lse1, float* lse2, streamkl_stream_t stream) {
-  return fwd_dispatch(STREAMKL_F32, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
+  return fwd_dispatch(STREAMKL_F32, nullptr, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
                       static_cast<cudaStream_t>(stream));
 }
 int streamkl_bwd(const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1, int d2, float c1,
                  float c2, int causal, const float* kl_rows, const float* lse1, const float* lse2, const float* dkl_rows, void* dQ1,
                  void* dK1, void* dQ2, void* dK2, void* workspace, size_t workspace_bytes, streamkl_stream_t stream) {
-  return bwd_dispatch(STREAMKL_BF16, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2, dkl_rows, dQ1, dK1,
+  return bwd_dispatch(STREAMKL_BF16, nullptr, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2, dkl_rows, dQ1, dK1,
                       dQ2, dK2, workspace, workspace_bytes, static_cast<cudaStream_t>(stream));
 }
 int streamkl_bwd_f32(const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1, int d2,
                      float c1, float c2, int causal, const float* kl_rows, const float* lse1, const float* lse2,
                      const float* dkl_rows, void* dQ1, void* dK1, void* dQ2, void* dK2, void* workspace, size_t workspace_bytes,
                      streamkl_stream_t stream) {
-  return bwd_dispatch(STREAMKL_F32, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2, dkl_rows, dQ1, dK1,
+  return bwd_dispatch(STREAMKL_F32, nullptr, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2, dkl_rows, dQ1, dK1,
                       dQ2, dK2, workspace, workspace_bytes, static_cast<cudaStream_t>(stream));
+}
+
+int streamkl_fwd_ex(const streamkl_layout* layout, const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK,
+                    int d1, int d2, float c1, float c2, int causal, float* kl_rows, float* lse1, float* lse2, streamkl_stream_t stream) {
+  return fwd_dispatch(layout ? layout->dtype : STREAMKL_BF16, layout, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
+                      static_cast<cudaStream_t>(stream));
+}
+int streamkl_bwd_ex(const streamkl_layout* layout, const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK,
+                    int d1, int d2, float c1, float c2, int causal, const float* kl_rows, const float* lse1, const float* lse2,
+                    const float* dkl_rows, void* dQ1, void* dK1, void* dQ2, void* dK2, void* workspace, size_t workspace_bytes,
+                    streamkl_stream_t stream) {
+  return bwd_dispatch(layout ? layout->dtype : STREAMKL_BF16, layout, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
+                      dkl_rows, dQ1, dK1, dQ2, dK2, workspace, workspace_bytes, static_cast<cudaStream_t>(stream));
 }
 
 int streamkl_fwd_splitk_splits(int B, int H, int NQ, int NK, int p_target) {
@@ -522,14 +604,14 @@ int streamkl_fwd_splitk(const void* Q1, const void* K1, const void* Q2, const vo
   if (splits <= 0) splits = streamkl_fwd_splitk_splits(B, H, NQ, NK, 0);
   const int tk = NK > 0 ? (NK + skl::FwdCfg<128, 128>::BK - 1) / skl::FwdCfg<128, 128>::BK : 1;
   if (splits > tk) splits = tk;
-  const bool tc = (d1 == 64 || d1 == 128) && (d2 == 64 || d2 == 128);
+  const bool tc = d1 % 8 == 0 && d2 % 8 == 0 && d1 >= 8 && d2 >= 8 && d1 <= 128 && d2 <= 128;
   if (!tc || splits <= 1)   // other head dims run the (unsplit) SIMT kernel; W = 1 is the default kernel
-    return fwd_dispatch(STREAMKL_BF16, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
+    return fwd_dispatch(STREAMKL_BF16, nullptr, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
                         static_cast<cudaStream_t>(stream));
   const size_t need = streamkl_fwd_splitk_workspace_bytes(B, H, NQ, splits);
   if (need > 0 && (!workspace || workspace_bytes < need)) return STREAMKL_ERR_WORKSPACE;
   if (reinterpret_cast<uintptr_t>(workspace) & 15) return STREAMKL_ERR_ALIGN;
-  return fwd_dispatch(STREAMKL_BF16, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
+  return fwd_dispatch(STREAMKL_BF16, nullptr, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
                       static_cast<cudaStream_t>(stream), splits, static_cast<float*>(workspace));
 }
 
@@ -537,11 +619,11 @@ size_t streamkl_bwd_workspace_bytes(int B, int H, int NQ, int, int d1, int d2, i
   // both gradients are produced by tile ownership: no fp32 accumulation workspace.  The tcgen05 kernels read the
   // per-query scalars (lse1, lse2, dkl, kl) from a packed copy: 16 B per query, rows padded to 64 per head -- O(NQ).
   if (B <= 0 || H <= 0 || NQ <= 0) return 0;
-  if (!((d1 == 64 || d1 == 128) && (d2 == 64 || d2 == 128))) return 0;
+  if (!(d1 % 8 == 0 && d2 % 8 == 0 && d1 >= 8 && d2 >= 8 && d1 <= 128 && d2 <= 128)) return 0;   // SIMT path: no workspace
   const long long BH = (long long)B * H;
   if (!bwd_fused_selected(NQ, want_teacher != 0)) return size_t(BH) * size_t(skl::bwd_stats_padded_rows(NQ)) * 16;
   // one-visit kernels (mode FUSED, or AUTO with NQ <= 512): + their fp32 dQ accumulators, O(NQ d)
-  return stats_bytes_aligned(BH, NQ) + fused_acc_bytes_aligned(BH, NQ, d2) + (want_teacher ? fused_acc_bytes_aligned(BH, NQ, d1) : 0);
+  return stats_bytes_aligned(BH, NQ) + fused_acc_bytes_aligned(BH, NQ, pad_dim(d2)) + (want_teacher ? fused_acc_bytes_aligned(BH, NQ, pad_dim(d1)) : 0);
 }
 
 int streamkl_set_bwd_mode(int mode) {
@@ -645,14 +727,14 @@ int streamkl_fwd_bwd_host(int dtype, const void* Q1, const void* K1, const void*
     if (!ok) break;
     // ---- kernels (stream `cmp`): the group is a batch of hn heads
     if (s.NQ > 0) {
-      rc = fwd_dispatch(dtype, bQ1 + h0 * hq1, bK1 + h0 * hk1, bQ2 + h0 * hq2, bK2 + h0 * hk2, 1, hn, NQ, NK, d1, d2, c1, c2, causal,
+      rc = fwd_dispatch(dtype, nullptr, bQ1 + h0 * hq1, bK1 + h0 * hk1, bQ2 + h0 * hq2, bK2 + h0 * hk2, 1, hn, NQ, NK, d1, d2, c1, c2, causal,
                         reinterpret_cast<float*>(bkl + h0 * hrow), reinterpret_cast<float*>(bl1 + h0 * hrow),
                         reinterpret_cast<float*>(bl2 + h0 * hrow), hs.cmp);
       if (rc != STREAMKL_OK) break;
       launches += g_last_launches;
     }
     if (want_bwd) {
-      rc = bwd_dispatch(dtype, bQ1 + h0 * hq1, bK1 + h0 * hk1, bQ2 + h0 * hq2, bK2 + h0 * hk2, 1, hn, NQ, NK, d1, d2, c1, c2, causal,
+      rc = bwd_dispatch(dtype, nullptr, bQ1 + h0 * hq1, bK1 + h0 * hk1, bQ2 + h0 * hq2, bK2 + h0 * hk2, 1, hn, NQ, NK, d1, d2, c1, c2, causal,
                         reinterpret_cast<float*>(bkl + h0 * hrow), reinterpret_cast<float*>(bl1 + h0 * hrow),
                         reinterpret_cast<float*>(bl2 + h0 * hrow), reinterpret_cast<float*>(bg + h0 * hrow),
                         teacher ? gQ1 + h0 * hq1 : nullptr, teacher ? gK1 + h0 * hk1 : nullptr, gQ2 + h0 * hq2, gK2 + h0 * hk2,
@@ -742,6 +824,6 @@ const char* streamkl_strerror(int code) {
   }
 }
 
-const char* streamkl_version(void) { return "streamkl-b200 0.1 (sm_100a; tcgen05+TMA bf16, SIMT fp32)"; }
+const char* streamkl_version(void) { return "streamkl-b200 0.2 (sm_100a; tcgen05+TMA bf16/fp16, strided + shared-K-head layouts; SIMT fp32)"; }
 
 }  // extern "C"

@@ -51,19 +51,32 @@ struct BwdFusedCfg {
 };
 
 struct BwdFusedParams {
-  int NQ, NK, TX, BH;
+  int NQ, NK, TX, BH;    // BH = B * H query heads
+  int H, HK, G;          // query heads, K heads, query heads per K head (GQA)
+  uint32_t fmt16;        // 1 bf16, 0 fp16
   float c1, c2;
   const float4* stats;   // as BwdParams::stats
   float* dq_acc;         // [BH][NQ][DG] fp32, zeroed by the caller of the kernel
-  __nv_bfloat16* dK;     // dK2 (student pass) or dK1 (teacher pass)
+  uint16_t* dK;          // dK2 (student pass) or dK1 (teacher pass), 16-bit elements
+  OutGeom gk;            // its strides and true head dim
 };
 
-// dQ = bf16(scale * dq_acc): the one rounding of the atomically accumulated gradient (scale = c2, or c1 ln2 for the teacher)
-__global__ void streamkl_bwd_dq_convert_kernel(const float4* __restrict__ acc, uint2* __restrict__ out, float c2, long long n4) {
+// dQ = 16-bit(scale * dq_acc): the one rounding of the atomically accumulated gradient (scale = c2, or c1 ln2 for the teacher).
+// dq_acc is dense [B*H][NQ][DG] (DG = padded head dim); dQ has the caller's strides and true head dim.  One thread per 4 columns.
+__global__ void streamkl_bwd_dq_convert_kernel(const float4* __restrict__ acc, uint16_t* __restrict__ out, float scale, long long n4,
+                                               int NQ, int H, int DG, OutGeom g, int f16) {
   const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n4) return;
+  const int c4 = DG / 4;
+  const int col = int(i % c4) * 4;
+  if (col >= g.d) return;
+  const long long r = i / c4;
+  const int row = int(r % NQ);
+  const long long bh = r / NQ;
   const float4 v = acc[i];
-  out[i] = make_uint2(pack_bf16x2(v.x * c2, v.y * c2), pack_bf16x2(v.z * c2, v.w * c2));
+  uint16_t* o = out + (bh / H) * g.sb + (bh % H) * g.sh + (long long)row * g.sn + col;
+  *reinterpret_cast<uint2*>(o) = f16 ? make_uint2(pack_f16x2(v.x * scale, v.y * scale), pack_f16x2(v.z * scale, v.w * scale))
+                                     : make_uint2(pack_bf16x2(v.x * scale, v.y * scale), pack_bf16x2(v.z * scale, v.w * scale));
 }
 
 template <int D1, int D2, bool CAUSAL, bool TPASS = false>
@@ -94,7 +107,8 @@ streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const 
   uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(dk_full + 1);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int bh = blockIdx.x / p.TX;
+  const int unit = blockIdx.x / p.TX;            // (batch, K head); the query tiles of its G query heads are streamed in turn
+  const int bx = unit / p.HK, hx = unit % p.HK;
   const int xt = blockIdx.x % p.TX;              // early K tiles are seen by more queries: heavy first
   const int x0 = xt * C::BX;
   const int off = p.NK - p.NQ;
@@ -102,7 +116,10 @@ streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const 
   int j_begin = 0;
   const int j_end = (p.NQ + C::BY - 1) / C::BY;
   if (CAUSAL) j_begin = max(0, x0 - off) / C::BY;    // first query that sees key x0
-  const int nsteps = max(0, j_end - j_begin);
+  const int nsteps1 = max(0, j_end - j_begin);   // steps per streamed query head
+  const int nsteps = nsteps1 * p.G;
+  auto step_g = [&](int it) { return it / max(nsteps1, 1); };
+  auto step_j = [&](int it) { return j_begin + it % max(nsteps1, 1); };
 
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tmQ1); tma_prefetch_desc(&tmK1); tma_prefetch_desc(&tmQ2); tma_prefetch_desc(&tmK2);
@@ -132,26 +149,27 @@ streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const 
         const uint64_t pol_x = l2_policy_evict_first(), pol_y = l2_policy_evict_last();
         mbar_arrive_expect_tx(x_full, C::X_BYTES);
 #pragma unroll
-        for (int kb = 0; kb < C::KB1; ++kb) tma_load_3d_hint(sX1 + kb * C::XBLK, &tmK1, x_full, kb * 64, x0, bh, pol_x);
+        for (int kb = 0; kb < C::KB1; ++kb) tma_load_4d_hint(sX1 + kb * C::XBLK, &tmK1, x_full, kb * 64, x0, hx, bx, pol_x);
 #pragma unroll
-        for (int kb = 0; kb < C::KB2; ++kb) tma_load_3d_hint(sX2 + kb * C::XBLK, &tmK2, x_full, kb * 64, x0, bh, pol_x);
+        for (int kb = 0; kb < C::KB2; ++kb) tma_load_4d_hint(sX2 + kb * C::XBLK, &tmK2, x_full, kb * 64, x0, hx, bx, pol_x);
         for (int it = 0; it < nsteps; ++it) {
-          const int j = j_begin + it;
+          const int j = step_j(it);
+          const int hy = hx * p.G + step_g(it);        // streamed query head
           const int s = it % C::NSTAGE;
           mbar_wait(&y_empty[s], ((it / C::NSTAGE) & 1) ^ 1);
           mbar_arrive_expect_tx(&y_full[s], C::Y_STAGE + C::STAT_STAGE);
           uint8_t* st = sY + s * C::Y_STAGE;
 #pragma unroll
-          for (int kb = 0; kb < C::KB1; ++kb) tma_load_3d_hint(st + kb * C::YBLK, &tmQ1, &y_full[s], kb * 64, j * C::BY, bh, pol_y);
+          for (int kb = 0; kb < C::KB1; ++kb) tma_load_4d_hint(st + kb * C::YBLK, &tmQ1, &y_full[s], kb * 64, j * C::BY, hy, bx, pol_y);
 #pragma unroll
           for (int kb = 0; kb < C::KB2; ++kb)
-            tma_load_3d_hint(st + (C::KB1 + kb) * C::YBLK, &tmQ2, &y_full[s], kb * 64, j * C::BY, bh, pol_y);
-          bulk_load_1d(sStat + s * C::BY, p.stats + (size_t(bh) * NQP + size_t(j) * C::BY), C::STAT_STAGE, &y_full[s]);
+            tma_load_4d_hint(st + (C::KB1 + kb) * C::YBLK, &tmQ2, &y_full[s], kb * 64, j * C::BY, hy, bx, pol_y);
+          bulk_load_1d(sStat + s * C::BY, p.stats + (size_t(bx * p.H + hy) * NQP + size_t(j) * C::BY), C::STAT_STAGE, &y_full[s]);
         }
       }
     } else if (warp == 1) {
       // ===================== S' MMA issuer =====================
-      constexpr uint32_t idesc_s = umma_idesc_bf16(C::BX, C::BY, 0, 0);
+      const uint32_t idesc_s = umma_idesc_16(C::BX, C::BY, 0, 0, p.fmt16);
       const uint64_t dx1 = umma_smem_desc_sw128(smem_u32(sX1), 16, 1024);
       const uint64_t dx2 = umma_smem_desc_sw128(smem_u32(sX2), 16, 1024);
       const uint64_t dyk = umma_smem_desc_sw128(smem_u32(sY), 16, 1024);
@@ -189,8 +207,8 @@ streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const 
       }
     } else if (warp == 3) {
       // ===================== gradient MMA issuer =====================
-      constexpr uint32_t idesc_k = umma_idesc_bf16(C::BX, DG, 0, 1);    // dK2 += dS2 Q2   : A from TMEM, B = Q2 MN-major
-      constexpr uint32_t idesc_q = umma_idesc_bf16(128, C::BY, 1, 1);   // dQ2^T = K2^T dS2: A = K2 MN-major, B = dS2 MN-major
+      const uint32_t idesc_k = umma_idesc_16(C::BX, DG, 0, 1, p.fmt16);    // dK2 += dS2 Q2   : A from TMEM, B = Q2 MN-major
+      const uint32_t idesc_q = umma_idesc_16(128, C::BY, 1, 1, p.fmt16);   // dQ2^T = K2^T dS2: A = K2 MN-major, B = dS2 MN-major
       // MN-major operands: rows = the contraction index (128 B each, 8-row groups 1024 B apart = SBO), 64-element chunks
       // of the M/N index LBO bytes apart; a K=16 slice = 16 rows = 2048 B.  For d2 = 64 the padded half of M reads the
       // shared memory behind the K2 tile: those accumulator lanes (d >= 64) are never drained.
@@ -255,8 +273,8 @@ streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const 
       __syncwarp();
       if (lane == 0) mbar_arrive(&dq_empty[par]);
       if (d_valid) {
-        const int q0 = (j_begin + itd) * C::BY + half * 32;
-        float* dst = p.dq_acc + (size_t(bh) * p.NQ + q0) * DG + rloc;
+        const int q0 = step_j(itd) * C::BY + half * 32;
+        float* dst = p.dq_acc + (size_t(bx * p.H + hx * p.G + step_g(itd)) * p.NQ + q0) * DG + rloc;
 #pragma unroll
         for (int c = 0; c < 32; ++c)
           if (q0 + c < p.NQ) atomicAdd(dst + size_t(c) * DG, __uint_as_float(q[c]));   // result unused: red.global.add.f32
@@ -264,8 +282,9 @@ streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const 
     };
 
     int last = -1;
+    const bool f16 = p.fmt16 == 0;
     for (int it = par; it < nsteps; it += 2) {
-      const int j = j_begin + it;
+      const int j = step_j(it);
       const int s = it % C::NSTAGE;
       const int ss = it % C::NSS;
       const uint32_t u = uint32_t(it >> 1);
@@ -287,8 +306,13 @@ streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const 
       const uint32_t stat = stat_base + s * C::STAT_STAGE;
       // (o2 = the pass's dS: the teacher pass takes ds_row's dS1 output)
       uint32_t (&f1)[16] = *(TPASS ? &o2 : &o1), (&f2)[16] = *(TPASS ? &o1 : &o2);
-      if (masked) ds_row<32, TPASS, true, CAUSAL, true, !TPASS>(r1, r2, f1, f2, sc1, sc2, 0.f, 0.f, 0.f, stat, xrow, y0, off, p.NK);
-      else        ds_row<32, TPASS, true, CAUSAL, false, !TPASS>(r1, r2, f1, f2, sc1, sc2, 0.f, 0.f, 0.f, stat, xrow, y0, off, p.NK);
+      if (!f16) {
+        if (masked) ds_row<32, TPASS, true, CAUSAL, true, !TPASS>(r1, r2, f1, f2, sc1, sc2, 0.f, 0.f, 0.f, stat, xrow, y0, off, p.NK);
+        else        ds_row<32, TPASS, true, CAUSAL, false, !TPASS>(r1, r2, f1, f2, sc1, sc2, 0.f, 0.f, 0.f, stat, xrow, y0, off, p.NK);
+      } else {
+        if (masked) ds_row<32, TPASS, true, CAUSAL, true, !TPASS, true>(r1, r2, f1, f2, sc1, sc2, 0.f, 0.f, 0.f, stat, xrow, y0, off, p.NK);
+        else        ds_row<32, TPASS, true, CAUSAL, false, !TPASS, true>(r1, r2, f1, f2, sc1, sc2, 0.f, 0.f, 0.f, stat, xrow, y0, off, p.NK);
+      }
       mbar_wait(&ds_empty[par], (u & 1) ^ 1);   // the MMAs of step it-2 have consumed both copies of this dS2 stage
       tc_fence_after();
       tmem_st16(ds_taddr, o2);
@@ -303,18 +327,18 @@ streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const 
       last = it;
     }
     if (last >= 0) drain(last);
-    // ---- epilogue: dK2 (TMEM fp32) * c2 -> bf16 -> HBM; each warp group takes a quarter of the columns
+    // ---- epilogue: dK (TMEM fp32) * scale -> 16-bit -> HBM; each warp group takes a quarter of the (padded) columns
     const bool valid = xrow < p.NK;
-    const size_t orow = size_t(bh) * p.NK + (valid ? xrow : 0);
+    uint16_t* ok = p.dK + (bx * p.gk.sb + hx * p.gk.sh + (long long)(valid ? xrow : 0) * p.gk.sn) + grp * (DG / 4);
     if (nsteps > 0) {
       mbar_wait(dk_full, 0);
       tc_fence_after();
       // (the teacher's dS1 is kept in log2 units, Eq.12: its ln2 joins the scale here, as in the separate kernels)
-      store_dx_cols<DG / 4>(lane_addr + C::COL_DK + grp * (DG / 4), TPASS ? p.c1 * 0.6931471805599453f : p.c2,
-                            p.dK + orow * DG + grp * (DG / 4), valid);
+      store_dx_cols<DG / 4>(lane_addr + C::COL_DK + grp * (DG / 4), TPASS ? p.c1 * 0.6931471805599453f : p.c2, ok, valid, f16,
+                            grp * (DG / 4), p.gk.d);
     } else if (valid) {
       const uint4 z = make_uint4(0, 0, 0, 0);
-      for (int c = 0; c < DG / 4; c += 8) *reinterpret_cast<uint4*>(p.dK + orow * DG + grp * (DG / 4) + c) = z;
+      for (int c = 0; c < DG / 4 && grp * (DG / 4) + c < p.gk.d; c += 8) *reinterpret_cast<uint4*>(ok + c) = z;
     }
   }
   tc_fence_before();

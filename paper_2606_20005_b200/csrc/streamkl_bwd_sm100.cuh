@@ -76,12 +76,21 @@ struct BwdCfg {
 // queries per head in the padded per-query scalar array
 __host__ __device__ constexpr long long bwd_stats_padded_rows(long long NQ) { return (NQ + 63) / 64 * 64; }
 
+// Element strides {batch, head, row} of a gradient tensor (the head dimension is contiguous) and its true head dim: the kernels
+// run on head dims padded to 64 / 128 (TMA zero-fills the extra columns of the inputs); columns >= d are not stored.
+struct OutGeom {
+  long long sb, sh, sn;
+  int d;
+};
 struct BwdParams {
-  int NQ, NK, TX, BH;
+  int NQ, NK, TX, BH;   // BH = B * H query heads
+  int H, HK, G;         // query heads, K heads (H = HK * G), query heads per K head (GQA)
+  uint32_t fmt16;       // 16-bit element format of inputs and gradients: 1 bf16, 0 fp16
   float c1, c2;
-  const float4* stats;  // [BH][NQP/2][2] float4, NQP = bwd_stats_padded_rows(NQ)
-  __nv_bfloat16* dX1;   // dQ1 or dK1 (nullptr when !TEACHER)
-  __nv_bfloat16* dX2;   // dQ2 or dK2
+  const float4* stats;  // [B*H][NQP/2][2] float4, NQP = bwd_stats_padded_rows(NQ)
+  uint16_t* dX1;        // dQ1 or dK1 (nullptr when !TEACHER), 16-bit elements
+  uint16_t* dX2;        // dQ2 or dK2
+  OutGeom g1, g2;
 };
 
 // B1: per-query scalars in the layout the dS warps consume (see the header comment)
@@ -113,10 +122,17 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
   return r;
 }
+__device__ __forceinline__ uint32_t pack_f16x2(float lo, float hi) {
+  uint32_t r;
+  asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
+  return r;
+}
+template <bool F16> __device__ __forceinline__ uint32_t pack_16x2(float lo, float hi) { return F16 ? pack_f16x2(lo, hi) : pack_bf16x2(lo, hi); }
 
-// dX accumulator (this warp's 32 lanes x NC fp32 columns) -> * scale -> bf16 -> global row
+// dX accumulator (this warp's 32 lanes x NC fp32 columns starting at column `col0`) -> * scale -> 16-bit -> global row;
+// 8-column chunks at or beyond the true head dim `d` (a multiple of 8) are padding and are not stored
 template <int NC>
-__device__ __forceinline__ void store_dx_cols(uint32_t taddr, float scale, __nv_bfloat16* out, bool valid) {
+__device__ __forceinline__ void store_dx_cols(uint32_t taddr, float scale, uint16_t* out, bool valid, bool f16, int col0, int d) {
   static_assert(NC == 16 || NC == 32, "column slice per dS warp group");
   uint32_t v[NC];
   if constexpr (NC == 32) tmem_ld32(taddr, v); else tmem_ld16(taddr, v);
@@ -124,11 +140,19 @@ __device__ __forceinline__ void store_dx_cols(uint32_t taddr, float scale, __nv_
   if (valid) {
 #pragma unroll
     for (int q = 0; q < NC / 8; ++q) {
+      if (col0 + q * 8 >= d) break;
       uint4 o;
-      o.x = pack_bf16x2(__uint_as_float(v[q * 8 + 0]) * scale, __uint_as_float(v[q * 8 + 1]) * scale);
-      o.y = pack_bf16x2(__uint_as_float(v[q * 8 + 2]) * scale, __uint_as_float(v[q * 8 + 3]) * scale);
-      o.z = pack_bf16x2(__uint_as_float(v[q * 8 + 4]) * scale, __uint_as_float(v[q * 8 + 5]) * scale);
-      o.w = pack_bf16x2(__uint_as_float(v[q * 8 + 6]) * scale, __uint_as_float(v[q * 8 + 7]) * scale);
+      if (f16) {
+        o.x = pack_f16x2(__uint_as_float(v[q * 8 + 0]) * scale, __uint_as_float(v[q * 8 + 1]) * scale);
+        o.y = pack_f16x2(__uint_as_float(v[q * 8 + 2]) * scale, __uint_as_float(v[q * 8 + 3]) * scale);
+        o.z = pack_f16x2(__uint_as_float(v[q * 8 + 4]) * scale, __uint_as_float(v[q * 8 + 5]) * scale);
+        o.w = pack_f16x2(__uint_as_float(v[q * 8 + 6]) * scale, __uint_as_float(v[q * 8 + 7]) * scale);
+      } else {
+        o.x = pack_bf16x2(__uint_as_float(v[q * 8 + 0]) * scale, __uint_as_float(v[q * 8 + 1]) * scale);
+        o.y = pack_bf16x2(__uint_as_float(v[q * 8 + 2]) * scale, __uint_as_float(v[q * 8 + 3]) * scale);
+        o.z = pack_bf16x2(__uint_as_float(v[q * 8 + 4]) * scale, __uint_as_float(v[q * 8 + 5]) * scale);
+        o.w = pack_bf16x2(__uint_as_float(v[q * 8 + 6]) * scale, __uint_as_float(v[q * 8 + 7]) * scale);
+      }
       *reinterpret_cast<uint4*>(out + q * 8) = o;
     }
   }
@@ -145,7 +169,7 @@ __device__ __forceinline__ float4 lds_f4(uint32_t saddr) {
 //   OWNER_K: per-column scalars come from shared memory (`stat`: shared-space address of these NC/2 column
 //            pairs, two float4 each), g is applied here.
 // MASKED: causal diagonal tiles and streamed-key tails; P (possibly inf for a zero-filled logit) is discarded by SELECT.
-template <int NC, bool TEACHER, bool OWNER_K, bool CAUSAL, bool MASKED, bool WANT2 = true>
+template <int NC, bool TEACHER, bool OWNER_K, bool CAUSAL, bool MASKED, bool WANT2 = true, bool F16 = false>
 __device__ __forceinline__ void ds_row(const uint32_t (&r1)[NC], const uint32_t (&r2)[NC], uint32_t (&o1)[NC / 2], uint32_t (&o2)[NC / 2],
                                          float sc1, float sc2, float nL1, float nL2, float klog, uint32_t stat, int xrow,
                                          int y0, int off, int NK) {
@@ -182,8 +206,8 @@ __device__ __forceinline__ void ds_row(const uint32_t (&r1)[NC], const uint32_t 
       a2.x = ok0 ? a2.x : 0.f; a2.y = ok1 ? a2.y : 0.f;
       a1.x = ok0 ? a1.x : 0.f; a1.y = ok1 ? a1.y : 0.f;
     }
-    if constexpr (WANT2) o2[e >> 1] = pack_bf16x2(a2.x, a2.y);
-    if constexpr (TEACHER) o1[e >> 1] = pack_bf16x2(a1.x, a1.y);
+    if constexpr (WANT2) o2[e >> 1] = pack_16x2<F16>(a2.x, a2.y);
+    if constexpr (TEACHER) o1[e >> 1] = pack_16x2<F16>(a1.x, a1.y);
   }
 }
 
@@ -216,7 +240,11 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
   const CUtensorMap* tmY2 = OWNER_K ? &tmQ2 : &tmK2;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int bh = blockIdx.x / p.TX;
+  // the CTA's unit = (batch, owner head): a query head for the Q owner; a K head for the K owner, which then streams the
+  // query tiles of all G query heads that share it (GQA; G = 1 otherwise).  TMA coordinates are {d, row, head, batch}.
+  const int unit = blockIdx.x / p.TX;
+  const int HX = OWNER_K ? p.HK : p.H;
+  const int bx = unit / HX, hx = unit % HX;
   // heavy tiles first: late Q tiles see more keys, early K tiles are seen by more queries
   const int xt = (CAUSAL && !OWNER_K) ? (p.TX - 1 - (blockIdx.x % p.TX)) : (blockIdx.x % p.TX);
   const int x0 = xt * C::BX;
@@ -229,7 +257,11 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
     if (OWNER_K) j_begin = max(0, x0 - off) / C::BY;                       // first query that sees key x0
     else         j_end = min(p.NK - 1, x0 + C::BX - 1 + off) / C::BY + 1;   // last key the tile's last row sees
   }
-  const int nsteps = max(0, j_end - j_begin);
+  const int nsteps1 = max(0, j_end - j_begin);             // steps per streamed head
+  const int nsteps = nsteps1 * (OWNER_K ? p.G : 1);
+  // step `it` -> (streamed head index g within the group, streamed tile j)
+  auto step_g = [&](int it) { return OWNER_K ? it / max(nsteps1, 1) : 0; };
+  auto step_j = [&](int it) { return j_begin + (OWNER_K ? it % max(nsteps1, 1) : it); };
 
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tmQ1); tma_prefetch_desc(&tmK1); tma_prefetch_desc(&tmQ2); tma_prefetch_desc(&tmK2);
@@ -258,29 +290,30 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
         const uint64_t pol_x = l2_policy_evict_first(), pol_y = l2_policy_evict_last();
         mbar_arrive_expect_tx(x_full, C::X_BYTES);
 #pragma unroll
-        for (int kb = 0; kb < C::KB1; ++kb) tma_load_3d_hint(sX1 + kb * C::XBLK, tmX1, x_full, kb * 64, x0, bh, pol_x);
+        for (int kb = 0; kb < C::KB1; ++kb) tma_load_4d_hint(sX1 + kb * C::XBLK, tmX1, x_full, kb * 64, x0, hx, bx, pol_x);
 #pragma unroll
-        for (int kb = 0; kb < C::KB2; ++kb) tma_load_3d_hint(sX2 + kb * C::XBLK, tmX2, x_full, kb * 64, x0, bh, pol_x);
+        for (int kb = 0; kb < C::KB2; ++kb) tma_load_4d_hint(sX2 + kb * C::XBLK, tmX2, x_full, kb * 64, x0, hx, bx, pol_x);
         for (int it = 0; it < nsteps; ++it) {
-          const int j = j_begin + it;
+          const int j = step_j(it);
+          const int hy = OWNER_K ? hx * p.G + step_g(it) : hx / p.G;   // streamed head: a query head of the group / the K head
           const int s = it % C::NSTAGE;
           const uint32_t ph = (it / C::NSTAGE) & 1;
           mbar_wait(&y_empty[s], ph ^ 1);
           mbar_arrive_expect_tx(&y_full[s], C::Y_STAGE + (OWNER_K ? C::STAT_STAGE : 0));
           uint8_t* st = sY + s * C::Y_STAGE;
 #pragma unroll
-          for (int kb = 0; kb < C::KB1; ++kb) tma_load_3d_hint(st + kb * C::YBLK, tmY1, &y_full[s], kb * 64, j * C::BY, bh, pol_y);
+          for (int kb = 0; kb < C::KB1; ++kb) tma_load_4d_hint(st + kb * C::YBLK, tmY1, &y_full[s], kb * 64, j * C::BY, hy, bx, pol_y);
 #pragma unroll
           for (int kb = 0; kb < C::KB2; ++kb)
-            tma_load_3d_hint(st + (C::KB1 + kb) * C::YBLK, tmY2, &y_full[s], kb * 64, j * C::BY, bh, pol_y);
+            tma_load_4d_hint(st + (C::KB1 + kb) * C::YBLK, tmY2, &y_full[s], kb * 64, j * C::BY, hy, bx, pol_y);
           if (OWNER_K)   // the streamed queries' scalars (B1): 64 queries = 32 pairs x 32 B, contiguous and 1 KB aligned
-            bulk_load_1d(sStat + s * C::BY, p.stats + (size_t(bh) * NQP + size_t(j) * C::BY), C::STAT_STAGE, &y_full[s]);
+            bulk_load_1d(sStat + s * C::BY, p.stats + (size_t(bx * p.H + hy) * NQP + size_t(j) * C::BY), C::STAT_STAGE, &y_full[s]);
         }
       }
     } else if (warp == 1) {
       // ===================== S' MMA issuer =====================
       // The whole warp runs the loop (warp-uniform control flow); only the tcgen05 instructions are issued by one lane.
-      constexpr uint32_t idesc_s = umma_idesc_bf16(C::BX, C::BY, 0, 0);      // S' = X Y^T   : A,B K-major from smem
+      const uint32_t idesc_s = umma_idesc_16(C::BX, C::BY, 0, 0, p.fmt16);     // S' = X Y^T   : A,B K-major from smem
       const uint64_t dx1 = umma_smem_desc_sw128(smem_u32(sX1), 16, 1024);
       const uint64_t dx2 = umma_smem_desc_sw128(smem_u32(sX2), 16, 1024);
       const uint64_t dyk = umma_smem_desc_sw128(smem_u32(sY), 16, 1024);
@@ -322,8 +355,8 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
       }
     } else if (warp == 3) {
       // ===================== dX MMA issuer =====================
-      constexpr uint32_t idesc_g1 = umma_idesc_bf16(C::BX, D1, 0, 1);        // dX1 += dS1 Y1: A from TMEM, B MN-major
-      constexpr uint32_t idesc_g2 = umma_idesc_bf16(C::BX, D2, 0, 1);
+      const uint32_t idesc_g1 = umma_idesc_16(C::BX, D1, 0, 1, p.fmt16);       // dX1 += dS1 Y1: A from TMEM, B MN-major
+      const uint32_t idesc_g2 = umma_idesc_16(C::BX, D2, 0, 1, p.fmt16);
       // Y as the MN-major B operand: 64-column chunks YBLK apart (LBO), 8-row groups 1024 B apart (SBO);
       // a K=16 slice = 16 streamed rows = 2048 B
       const uint64_t dym = umma_smem_desc_sw128(smem_u32(sY), C::YBLK, 1024);
@@ -368,15 +401,16 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
     const float sc1 = p.c1 * L2E, sc2 = p.c2 * L2E;
     float nL1 = -1e30f, nL2 = -1e30f, klog = 0.f, my_g = 0.f;
     if (!OWNER_K && xrow < p.NQ) {
-      const float* sp = reinterpret_cast<const float*>(p.stats + (size_t(bh) * NQP + size_t(xrow & ~1)));  // pair (xrow>>1): 2 float4
+      const float* sp = reinterpret_cast<const float*>(p.stats + (size_t(unit) * NQP + size_t(xrow & ~1)));  // pair (xrow>>1): 2 float4
       const int u = xrow & 1;
       nL1 = sp[u]; nL2 = sp[2 + u]; my_g = sp[4 + u]; klog = sp[6 + u];
     }
     const uint32_t lane_addr = tmem_base + (uint32_t(quarter * 32) << 16);
     const uint32_t stat_base = smem_u32(sStat) + half * 32 * 16;
     const uint32_t ds_addr = lane_addr + C::COL_DS + par * 64 + half * 16;   // dS1 here, dS2 32 columns further
+    const bool f16 = p.fmt16 == 0;
     for (int it = par; it < nsteps; it += 2) {
-      const int j = j_begin + it;
+      const int j = step_j(it);
       const int s = it % C::NSTAGE;
       const int ss = it % C::NSS;
       mbar_wait(&s_full[par], (it >> 1) & 1);
@@ -395,8 +429,13 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
       const bool masked = OWNER_K ? (CAUSAL && (y0 + off < x0 + C::BX - 1))
                                   : ((CAUSAL && (y0 + 31 > x0 + off)) || (y0 + 32 > p.NK));
       const uint32_t stat = stat_base + s * C::STAT_STAGE;
-      if (masked) ds_row<32, TEACHER, OWNER_K, CAUSAL, true>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
-      else        ds_row<32, TEACHER, OWNER_K, CAUSAL, false>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
+      if (!f16) {
+        if (masked) ds_row<32, TEACHER, OWNER_K, CAUSAL, true>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
+        else        ds_row<32, TEACHER, OWNER_K, CAUSAL, false>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
+      } else {
+        if (masked) ds_row<32, TEACHER, OWNER_K, CAUSAL, true, true, true>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
+        else        ds_row<32, TEACHER, OWNER_K, CAUSAL, false, true, true>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
+      }
       mbar_wait(&ds_empty[par], ((it >> 1) & 1) ^ 1);   // the dX MMAs of step it-2 have consumed this dS stage
       tc_fence_after();
       tmem_st16(ds_addr + 32, o2);
@@ -406,20 +445,21 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
       __syncwarp();
       if (lane == 0) mbar_arrive(&ds_full[par]);
     }
-    // ---- epilogue: dX (TMEM fp32) * c_t -> bf16 -> HBM; each warp group takes a quarter of the columns
+    // ---- epilogue: dX (TMEM fp32) * c_t -> 16-bit -> HBM; each warp group takes a quarter of the (padded) columns
     const bool valid = xrow < NX;
-    const size_t orow = size_t(bh) * NX + (valid ? xrow : 0);
+    const long long xr = valid ? xrow : 0;
+    uint16_t* o2 = p.dX2 + (bx * p.g2.sb + hx * p.g2.sh + xr * p.g2.sn) + grp * (D2 / 4);
+    uint16_t* o1 = TEACHER ? p.dX1 + (bx * p.g1.sb + hx * p.g1.sh + xr * p.g1.sn) + grp * (D1 / 4) : nullptr;
     const float g_row = OWNER_K ? 1.f : my_g;   // Q owner: g is a per-row factor of dS, applied here
     if (nsteps > 0) {
       mbar_wait(dx_full, 0);
       tc_fence_after();
-      store_dx_cols<D2 / 4>(lane_addr + C::COL_DX2 + grp * (D2 / 4), p.c2 * g_row, p.dX2 + orow * D2 + grp * (D2 / 4), valid);
-      if (TEACHER)
-        store_dx_cols<D1 / 4>(lane_addr + C::COL_DX1 + grp * (D1 / 4), p.c1 * LN2 * g_row, p.dX1 + orow * D1 + grp * (D1 / 4), valid);
+      store_dx_cols<D2 / 4>(lane_addr + C::COL_DX2 + grp * (D2 / 4), p.c2 * g_row, o2, valid, f16, grp * (D2 / 4), p.g2.d);
+      if (TEACHER) store_dx_cols<D1 / 4>(lane_addr + C::COL_DX1 + grp * (D1 / 4), p.c1 * LN2 * g_row, o1, valid, f16, grp * (D1 / 4), p.g1.d);
     } else if (valid) {
       const uint4 z = make_uint4(0, 0, 0, 0);
-      for (int c = 0; c < D2 / 4; c += 8) *reinterpret_cast<uint4*>(p.dX2 + orow * D2 + grp * (D2 / 4) + c) = z;
-      if (TEACHER) for (int c = 0; c < D1 / 4; c += 8) *reinterpret_cast<uint4*>(p.dX1 + orow * D1 + grp * (D1 / 4) + c) = z;
+      for (int c = 0; c < D2 / 4 && grp * (D2 / 4) + c < p.g2.d; c += 8) *reinterpret_cast<uint4*>(o2 + c) = z;
+      if (TEACHER) for (int c = 0; c < D1 / 4 && grp * (D1 / 4) + c < p.g1.d; c += 8) *reinterpret_cast<uint4*>(o1 + c) = z;
     }
   }
   tc_fence_before();

@@ -71,7 +71,9 @@ struct FwdCfg {
 
 struct FwdParams {
   int NQ, NK, TQ;       // TQ = number of 128-row Q tiles per head
-  int BH;
+  int BH;               // B * H query heads
+  int H, G;             // query heads per batch; query heads per K head (GQA: query head h reads K head h / G)
+  uint32_t fmt16;       // operand format of the logit MMAs: 1 bf16, 0 fp16
   float sc1, sc2;       // c_t * log2(e)
   float* kl;
   float* lse1;
@@ -226,6 +228,7 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
   const int tile = SPLIT ? int(blockIdx.x) / p.W : int(blockIdx.x);
   const int wk = SPLIT ? int(blockIdx.x) % p.W : 0;          // key chunk of this CTA (split-K grid (b, i, w))
   const int bh = tile / p.TQ;
+  const int hq = bh % p.H, bq = bh / p.H, hk = hq / p.G;      // TMA coordinates {d, row, head, batch}
   const int qt = p.TQ - 1 - (tile % p.TQ);
   const int q0 = qt * C::BQ;
   const int off = p.NK - p.NQ;
@@ -258,9 +261,9 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
       const uint64_t pol_q = l2_policy_evict_first(), pol_k = l2_policy_evict_last();
       mbar_arrive_expect_tx(q_full, C::Q_BYTES);
 #pragma unroll
-      for (int kb = 0; kb < C::KB1; ++kb) tma_load_3d_hint(sQ1 + kb * C::QBLK, &tmQ1, q_full, kb * 64, q0, bh, pol_q);
+      for (int kb = 0; kb < C::KB1; ++kb) tma_load_4d_hint(sQ1 + kb * C::QBLK, &tmQ1, q_full, kb * 64, q0, hq, bq, pol_q);
 #pragma unroll
-      for (int kb = 0; kb < C::KB2; ++kb) tma_load_3d_hint(sQ2 + kb * C::QBLK, &tmQ2, q_full, kb * 64, q0, bh, pol_q);
+      for (int kb = 0; kb < C::KB2; ++kb) tma_load_4d_hint(sQ2 + kb * C::QBLK, &tmQ2, q_full, kb * 64, q0, hq, bq, pol_q);
       for (int j = 0; j < nsteps; ++j) {
         const int s = j % C::NSTAGE;
         const uint32_t ph = (j / C::NSTAGE) & 1;
@@ -269,17 +272,17 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
         uint8_t* st = sK + s * C::STAGE_BYTES;
 #pragma unroll
         for (int kb = 0; kb < C::KB1; ++kb)
-          tma_load_3d_hint(st + kb * C::KBLK, &tmK1, &k_full[s], kb * 64, (j_begin + j) * C::BK, bh, pol_k);
+          tma_load_4d_hint(st + kb * C::KBLK, &tmK1, &k_full[s], kb * 64, (j_begin + j) * C::BK, hk, bq, pol_k);
 #pragma unroll
         for (int kb = 0; kb < C::KB2; ++kb)
-          tma_load_3d_hint(st + (C::KB1 + kb) * C::KBLK, &tmK2, &k_full[s], kb * 64, (j_begin + j) * C::BK, bh, pol_k);
+          tma_load_4d_hint(st + (C::KB1 + kb) * C::KBLK, &tmK2, &k_full[s], kb * 64, (j_begin + j) * C::BK, hk, bq, pol_k);
       }
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
     // The whole warp runs the loop (warp-uniform control flow and descriptors stay in uniform registers); only the
     // tcgen05.mma / tcgen05.commit instructions themselves are issued by one elected lane.
-    constexpr uint32_t idesc = umma_idesc_bf16(C::BM, C::BK, 0, 0);
+    const uint32_t idesc = umma_idesc_16(C::BM, C::BK, 0, 0, p.fmt16);
     const uint64_t dq1 = umma_smem_desc_sw128(smem_u32(sQ1), 16, 1024);
     const uint64_t dq2 = umma_smem_desc_sw128(smem_u32(sQ2), 16, 1024);
     const uint64_t dk = umma_smem_desc_sw128(smem_u32(sK), 16, 1024);

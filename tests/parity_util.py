@@ -17,7 +17,7 @@ GRAD_ZERO_ATOL = 1e-4
 
 
 def to_torch(a: np.ndarray, device="cuda"):
-    """numpy (uint16 bf16 bits | float32) -> torch tensor on `device` (bfloat16 | float32)."""
+    """numpy (uint16 bf16 bits | float16 | float32) -> torch tensor on `device` (bfloat16 | float16 | float32)."""
     import torch
 
     if a.dtype == np.uint16:

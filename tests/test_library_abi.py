@@ -46,8 +46,8 @@ def test_binding_exposes_the_same_names():
     import paper_2606_20005_b200 as skl
 
     for name in declared_functions():
-        if name.endswith("_f32"):
-            continue  # the binding dispatches on the tensor dtype
+        if name.endswith("_f32") or name.endswith("_ex"):
+            continue  # the binding dispatches on the tensor's dtype, strides and head counts (streamkl_fwd / streamkl_bwd)
         assert hasattr(skl, name)
 
 
@@ -120,7 +120,8 @@ def test_bwd_workspace_follows_the_selected_strategy(L):
     assert L.streamkl_set_bwd_mode(2) == 0   # FUSED: always
     assert L.streamkl_bwd_workspace_bytes(1, 32, 16384, 16384, 128, 64, 0) == a256(32 * 16384 * 16) + a256(32 * 16384 * 64 * 4)
     assert L.streamkl_set_bwd_mode(0) == 0
-    assert L.streamkl_bwd_workspace_bytes(1, 1, 256, 256, 48, 80, 0) == 0                  # SIMT path: no workspace
+    assert L.streamkl_bwd_workspace_bytes(1, 1, 256, 256, 44, 80, 0) == 0                  # head dim not a multiple of 8: SIMT path, no workspace
+    assert L.streamkl_bwd_workspace_bytes(1, 1, 256, 256, 192, 64, 0) == 0                 # head dim > 128: SIMT path
 
 
 def test_splitk_adaptive_split_selection_follows_the_paper_rule(L):

@@ -33,7 +33,7 @@ class Config:
     NK: int
     d1: int
     d2: int
-    dtype: str  # "bf16" | "f32"
+    dtype: str  # "bf16" | "f16" | "f32"
     causal: bool
     near: bool = False
     q1_scale: float = 1.0
@@ -106,7 +106,7 @@ def bf16_to_f32(bits: np.ndarray) -> np.ndarray:
 
 
 def widen_f64(a: np.ndarray) -> np.ndarray:
-    """Exact widening of a stored tensor (uint16 bf16 bits or float32) to float64."""
+    """Exact widening of a stored tensor (uint16 bf16 bits, float16 or float32) to float64."""
     if a.dtype == np.uint16:
         return bf16_to_f32(a).astype(np.float64)
     return a.astype(np.float64)
@@ -117,6 +117,8 @@ def _store(x: np.ndarray, dtype: str) -> np.ndarray:
         return f32_to_bf16_bits(x)
     if dtype == "f32":
         return np.ascontiguousarray(x, dtype=np.float32)
+    if dtype == "f16":
+        return np.ascontiguousarray(x, dtype=np.float32).astype(np.float16)   # IEEE round-to-nearest-even
     raise ValueError(dtype)
 
 
@@ -159,7 +161,7 @@ def all_inputs(cfg: Config, heads=None):
         shape = (cfg.B, cfg.H)
     else:
         shape = (len(heads),)
-    st = np.uint16 if cfg.dtype == "bf16" else np.float32
+    st = {"bf16": np.uint16, "f16": np.float16, "f32": np.float32}[cfg.dtype]
     out = {
         "Q1": np.empty(shape + (cfg.NQ, cfg.d1), st),
         "K1": np.empty(shape + (cfg.NK, cfg.d1), st),
