@@ -41,6 +41,7 @@ UNIT = "TFLOP/s"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 SPEC_BF16_TFLOPS = 2250.0
 WORKLOADS = {"cfg2": 2, "cfg3": 3, "cfg4": 4, "cfg5": 5}
+SIDE_LEGS = ("splitk", "bwd-strategies")   # --workload <leg>: run only that secondary measurement (profiling runs)
 
 
 def peaks():
@@ -402,13 +403,13 @@ def kernel_flops_one_visit(cfg: W.Config, name: str, launches_of_bwd_kernels: fl
 BWD_MODES = {"auto": 0, "separate": 1, "fused": 2}
 
 
-def time_bwd_strategies(skl, iters: int = 20):
+def time_bwd_strategies(skl, iters: int = 20, nqs=(16, 128, 256, 512, 1024, 4096)):
     """Backward strategy table (Fig.13): separate owner kernels vs the one-visit kernels,
     both settings, small-to-medium N_Q, bsz 16, N_K = 16384, d = 128/128, no mask.  ms per streamkl_bwd call."""
     import torch
 
     out = {}
-    for NQ in (16, 128, 256, 512, 1024, 4096):
+    for NQ in nqs:
         cfg = W.Config(71, "bwd-strategy", 1, 16, NQ, 16384, 128, 128, "bf16", False)
         inp = W.all_inputs(cfg)
         Q1, K1, Q2, K2 = (to_dev(inp[k]) for k in ("Q1", "K1", "Q2", "K2"))
@@ -450,7 +451,9 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="streamkl", choices=["streamkl", "reference"])
-    ap.add_argument("--workload", default="cfg4", choices=sorted(WORKLOADS))
+    ap.add_argument("--workload", default="cfg4", choices=sorted(WORKLOADS) + list(SIDE_LEGS))
+    ap.add_argument("--nq", type=int, default=0, help="--workload bwd-strategies: only this N_Q")
+    ap.add_argument("--iters", type=int, default=20, help="--workload splitk / bwd-strategies: timed calls per point")
     ap.add_argument("--no-also", action="store_true", help="skip the secondary measurements (cfg3, cfg2, cfg5, split-K, strategy table)")
     ap.add_argument("--bwd-mode", default="auto", choices=sorted(BWD_MODES), help="backward strategy of the timed step (streamkl_set_bwd_mode)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
@@ -460,6 +463,19 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.workload in SIDE_LEGS:   # one secondary leg alone: a short, committed command for ncu captures
+        import torch
+
+        import paper_2606_20005_b200 as skl
+
+        torch.cuda.set_device(local)
+        if args.workload == "splitk":
+            out = time_splitk(skl, iters=args.iters)
+        else:
+            out = time_bwd_strategies(skl, iters=args.iters, nqs=(args.nq,) if args.nq > 0 else (16, 128, 256, 512, 1024, 4096))
+        if rank == 0:
+            print(json.dumps({"leg": args.workload, "result": out, "library": skl.streamkl_version()}), flush=True)
+        return
     cfg = W.CONFIGS[WORKLOADS[args.workload]]
 
     if args.impl == "reference":
