@@ -21,6 +21,12 @@ Per (b,h) and query row i  (readings R1,R2,R4,R5 of DESIGN.md
   dQ_t    = c_t * dS_t @ K_t ;  dK_t = c_t * dS_t^T @ Q_t                        (:64, :69; chain rule on c_t)
 Masked entries contribute 0 everywhere.  Outputs stay float64; nothing is rounded on this side.
 
+Student activation ("Generalizability beyond Softmax": "the ReLU variant used in the indexer training of
+DeepSeek-V3.2"; the paper gives no formula -- reading R23 of DESIGN.md).  With `act2="relu"` the student's logit passes through
+ReLU BEFORE its softmax, s2[j] = relu(c2 <Q2[i], K2[j]>), exactly as that indexer scores a key (one indexer head, unit weight) and
+is then trained with KL(P1 || softmax(s2)).  Everything above is unchanged with this s2; the chain rule adds relu'(.) = 1[c2 <q,k> > 0]
+to the student's logit gradient:  dS2 = g_i (P2 - P1) * 1[raw s2 > 0]  (0 at the kink).  The teacher's gradient is Eq.3 verbatim.
+
 Pins (tests/test_oracle_pins.py, `-m "not gpu"`): hand-derived worked example (tests/golden/),
 closed forms (identical logits, P2 uniform, P1 uniform, NK=1, NK=2 Bernoulli), scipy
 logsumexp/rel_entr, torch float64 autograd through log_softmax, central finite differences,
@@ -44,7 +50,7 @@ def visible_mask(rows: np.ndarray, NQ: int, NK: int, causal: bool) -> np.ndarray
     return j <= (np.asarray(rows)[:, None] + (NK - NQ))
 
 
-def attention_kl_rows(Q1, K1, Q2, K2, c1, c2, causal, rows, g=None, teacher=True):
+def attention_kl_rows(Q1, K1, Q2, K2, c1, c2, causal, rows, g=None, teacher=True, act2=None):
     """Definition for a group of query rows of one head.
 
     Q_t [NQ,d_t], K_t [NK,d_t] float64.  rows: int array of query indices.
@@ -56,6 +62,11 @@ def attention_kl_rows(Q1, K1, Q2, K2, c1, c2, causal, rows, g=None, teacher=True
     vis = visible_mask(rows, NQ, NK, causal)
     S1 = c1 * (Q1[rows] @ K1.T)  # [R,NK]  logits of distribution 1
     S2 = c2 * (Q2[rows] @ K2.T)
+    if act2 not in (None, "relu"):
+        raise ValueError("act2 must be None or 'relu'")
+    if act2 == "relu":  # R23: the student's logit is relu(c2 q.k); its derivative gates dS2 below
+        relu_grad = (S2 > 0.0).astype(np.float64)
+        S2 = np.maximum(S2, 0.0)
     neg = -np.inf
     S1m = np.where(vis, S1, neg)
     S2m = np.where(vis, S2, neg)
@@ -74,6 +85,8 @@ def attention_kl_rows(Q1, K1, Q2, K2, c1, c2, causal, rows, g=None, teacher=True
         return out
     gi = np.asarray(g, dtype=np.float64)[rows][:, None]
     dS2 = gi * (P2 - P1)  # Eq.2
+    if act2 == "relu":
+        dS2 = dS2 * relu_grad
     out["dQ2"] = c2 * (dS2 @ K2)
     out["dK2_part"] = c2 * (dS2.T @ Q2[rows])
     if teacher:
@@ -83,7 +96,7 @@ def attention_kl_rows(Q1, K1, Q2, K2, c1, c2, causal, rows, g=None, teacher=True
     return out
 
 
-def attention_kl_head(Q1, K1, Q2, K2, c1, c2, causal, g=None, teacher=True, row_block=None):
+def attention_kl_head(Q1, K1, Q2, K2, c1, c2, causal, g=None, teacher=True, row_block=None, act2=None):
     """Whole head: every query row, dK summed over all rows.  Inputs any float dtype; computed in float64."""
     Q1 = np.asarray(Q1, dtype=np.float64)
     K1 = np.asarray(K1, dtype=np.float64)
@@ -102,7 +115,7 @@ def attention_kl_head(Q1, K1, Q2, K2, c1, c2, causal, g=None, teacher=True, row_
             res["dK1"] = np.zeros((NK, K1.shape[1]))
     for r0 in range(0, NQ, row_block):
         rows = np.arange(r0, min(NQ, r0 + row_block))
-        part = attention_kl_rows(Q1, K1, Q2, K2, c1, c2, causal, rows, g, teacher)
+        part = attention_kl_rows(Q1, K1, Q2, K2, c1, c2, causal, rows, g, teacher, act2)
         for k in ("kl", "lse1", "lse2"):
             res[k][rows] = part[k]
         if g is not None:
@@ -114,7 +127,7 @@ def attention_kl_head(Q1, K1, Q2, K2, c1, c2, causal, g=None, teacher=True, row_
     return res
 
 
-def attention_kl(Q1, K1, Q2, K2, c1, c2, causal, g=None, teacher=True):
+def attention_kl(Q1, K1, Q2, K2, c1, c2, causal, g=None, teacher=True, act2=None):
     """Batched [..., N, d] wrapper: loops over the leading (batch, head) axes, heads are independent."""
     Q1 = np.asarray(Q1)
     lead = Q1.shape[:-2]
@@ -125,7 +138,7 @@ def attention_kl(Q1, K1, Q2, K2, c1, c2, causal, g=None, teacher=True):
     K2r = np.asarray(K2).reshape((n,) + np.asarray(K2).shape[-2:])
     gr = None if g is None else np.asarray(g).reshape(n, -1)
     outs = [
-        attention_kl_head(Q1r[i], K1r[i], Q2r[i], K2r[i], c1, c2, causal, None if gr is None else gr[i], teacher)
+        attention_kl_head(Q1r[i], K1r[i], Q2r[i], K2r[i], c1, c2, causal, None if gr is None else gr[i], teacher, act2=act2)
         for i in range(n)
     ]
     return {k: np.stack([o[k] for o in outs]).reshape(lead + outs[0][k].shape) for k in outs[0]}

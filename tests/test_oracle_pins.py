@@ -295,3 +295,66 @@ def test_batched_wrapper_matches_per_head():
     o12 = orc.attention_kl_head(Q1[1, 2], K1[1, 2], Q2[1, 2], K2[1, 2], 0.5, 0.7, True, g=g[1, 2])
     for k in o12:
         np.testing.assert_array_equal(o[k][1, 2], o12[k])
+
+
+# ------------------------------------------------------------------ student ReLU activation (R23)
+@pytest.mark.parametrize("causal", [False, True])
+def test_relu_student_against_torch_autograd(causal):
+    """softmax(relu(c2 Q2 K2^T)) built from torch float64 primitives + autograd pins the forward values and all four gradients."""
+    import torch
+
+    NQ, NK, d1, d2 = 7, 11, 5, 4
+    Q1, K1, Q2, K2, g = _rand(NQ, NK, d1, d2, seed=21)
+    c1, c2 = 0.6, 0.8
+    o = orc.attention_kl_head(Q1, K1, Q2, K2, c1, c2, causal, g=g, act2="relu")
+    t = [torch.tensor(a, dtype=torch.float64, requires_grad=True) for a in (Q1, K1, Q2, K2)]
+    S1 = c1 * t[0] @ t[1].T
+    S2 = torch.relu(c2 * t[2] @ t[3].T)
+    if causal:
+        m = torch.arange(NK)[None, :] <= (torch.arange(NQ)[:, None] + NK - NQ)
+        S1 = S1.masked_fill(~m, -math.inf); S2 = S2.masked_fill(~m, -math.inf)
+    lp1 = torch.log_softmax(S1, -1); lp2 = torch.log_softmax(S2, -1)
+    kl = torch.where(lp1 > -math.inf, lp1.exp() * (lp1 - lp2), torch.zeros_like(lp1)).sum(-1)
+    (kl * torch.tensor(g)).sum().backward()
+    np.testing.assert_allclose(o["kl"], kl.detach().numpy(), atol=1e-12)
+    np.testing.assert_allclose(o["lse2"], torch.logsumexp(S2, -1).detach().numpy(), atol=1e-12)
+    for k, x in zip(("dQ1", "dK1", "dQ2", "dK2"), t):
+        np.testing.assert_allclose(o[k], x.grad.numpy(), atol=1e-11, err_msg=k)
+
+
+def test_relu_student_closed_forms():
+    """(a) every raw student logit <= 0  =>  relu makes P2 uniform: lse2 = log nV, KL = log nV - H(P1), student gradients vanish
+    identically (the gate is 0 everywhere);  (b) every raw student logit > 0  =>  identical to the plain softmax student."""
+    Q1, K1, _, _, g = _rand(6, 9, 4, 3, seed=22)
+    r = np.random.default_rng(23)
+    Q2 = np.abs(r.standard_normal((6, 3))); K2 = -np.abs(r.standard_normal((9, 3)))        # <q2,k2> < 0 always
+    o = orc.attention_kl_head(Q1, K1, Q2, K2, 0.5, 0.9, False, g=g, act2="relu")
+    np.testing.assert_allclose(o["lse2"], math.log(9.0), atol=1e-13)
+    S1 = 0.5 * Q1 @ K1.T
+    P1 = np.exp(S1 - S1.max(1, keepdims=True)); P1 /= P1.sum(1, keepdims=True)
+    np.testing.assert_allclose(o["kl"], math.log(9.0) + (P1 * np.log(P1)).sum(1), atol=1e-12)
+    assert np.abs(o["dQ2"]).max() == 0.0 and np.abs(o["dK2"]).max() == 0.0
+    K2p = np.abs(K2)                                                                          # <q2,k2> > 0 always
+    a = orc.attention_kl_head(Q1, K1, Q2, K2p, 0.5, 0.9, True, g=g, act2="relu")
+    b = orc.attention_kl_head(Q1, K1, Q2, K2p, 0.5, 0.9, True, g=g)
+    for k in a:
+        np.testing.assert_allclose(a[k], b[k], atol=1e-14, err_msg=k)
+
+
+def test_relu_student_finite_differences():
+    """Central differences on sum_i g_i KL_i (kinks have measure zero for random inputs; h is far below the smallest |raw s2|)."""
+    NQ, NK, d1, d2 = 5, 7, 4, 3
+    Q1, K1, Q2, K2, g = _rand(NQ, NK, d1, d2, seed=24)
+    c1, c2 = 0.7, 1.1
+    assert np.abs(c2 * Q2 @ K2.T).min() > 1e-4
+    o = orc.attention_kl_head(Q1, K1, Q2, K2, c1, c2, True, g=g, act2="relu")
+    f = lambda a, b, c, d: float((g * orc.attention_kl_head(a, b, c, d, c1, c2, True, act2="relu")["kl"]).sum())
+    h = 1e-6
+    args = [Q1, K1, Q2, K2]
+    for idx, name in enumerate(("dQ1", "dK1", "dQ2", "dK2")):
+        num = np.zeros_like(args[idx])
+        for i in np.ndindex(*args[idx].shape):
+            ap = [x.copy() for x in args]; am = [x.copy() for x in args]
+            ap[idx][i] += h; am[idx][i] -= h
+            num[i] = (f(*ap) - f(*am)) / (2 * h)
+        np.testing.assert_allclose(o[name], num, atol=2e-8, err_msg=name)
