@@ -314,10 +314,13 @@ def test_relu_student_against_torch_autograd(causal):
         m = torch.arange(NK)[None, :] <= (torch.arange(NQ)[:, None] + NK - NQ)
         S1 = S1.masked_fill(~m, -math.inf); S2 = S2.masked_fill(~m, -math.inf)
     lp1 = torch.log_softmax(S1, -1); lp2 = torch.log_softmax(S2, -1)
-    kl = torch.where(lp1 > -math.inf, lp1.exp() * (lp1 - lp2), torch.zeros_like(lp1)).sum(-1)
+    lse2 = torch.logsumexp(S2, -1).detach().numpy()
+    if causal:  # -inf log-probs at masked entries would make 0*(-inf - -inf) = nan in kl_div
+        lp1 = lp1.masked_fill(~m, -1e3); lp2 = lp2.masked_fill(~m, -1e3)  # exp(-1e3) == 0 exactly in float64
+    kl = torch.nn.functional.kl_div(lp2, lp1, reduction="none", log_target=True).sum(-1)
     (kl * torch.tensor(g)).sum().backward()
     np.testing.assert_allclose(o["kl"], kl.detach().numpy(), atol=1e-12)
-    np.testing.assert_allclose(o["lse2"], torch.logsumexp(S2, -1).detach().numpy(), atol=1e-12)
+    np.testing.assert_allclose(o["lse2"], lse2, atol=1e-12)
     for k, x in zip(("dQ1", "dK1", "dQ2", "dK2"), t):
         np.testing.assert_allclose(o[k], x.grad.numpy(), atol=1e-11, err_msg=k)
 
