@@ -82,14 +82,21 @@ int streamkl_fwd_f32(const void* Q1, const void* K1, const void* Q2, const void*
  *                contiguous default for that tensor ([B][H][N][d], or [B][HK][NK][d] for K).  E.g. a [B][N][H][d] tensor is
  *                {N*H*d, d, H*d}.  Strides must be multiples of 8 elements (16 bytes, TMA) and the row stride >= d.
  *                dQ_t is written with Q_t's strides, dK_t with K_t's; kl_rows / lse / dkl_rows stay contiguous [B][H][NQ].
- * Non-default strides and kv_heads need the tensor-core path: 16-bit dtype and d1, d2 multiples of 8 up to 128 (STREAMKL_ERR_SHAPE
+ *   student_activation : SURVEY 8(f) NEXT-4, "Generalizability beyond Softmax" ("the ReLU variant used in the indexer
+ *                training of DeepSeek-V3.2"; the paper prints no formula, so this is the library's reading, R23).
+ *                STREAMKL_ACT_RELU: the student's logit is s2[j] = relu(c2 <Q2[i], K2[j]>) -- that indexer's score with one head and
+ *                unit weight -- and P2 = softmax_j(s2) as before; kl / lse2 are those of this P2, and the student's logit gradient
+ *                is gated by relu': dS2 = g (P2 - P1) 1[<Q2[i],K2[j]> > 0].  The teacher side (P1, dS1 of Eq.3) is unchanged.
+ * Non-default strides, kv_heads and activations need the tensor-core path: 16-bit dtype and d1, d2 multiples of 8 up to 128 (STREAMKL_ERR_SHAPE
  * otherwise).  Head dims other than 64 / 128 run zero-padded to the next of the two inside the kernels (TMA zero fill): the
  * results are exact, the padded columns cost tensor work.
  */
+enum { STREAMKL_ACT_NONE = 0, STREAMKL_ACT_RELU = 1 };
 typedef struct streamkl_layout {
   int dtype;
   int kv_heads;
   long long q1_stride[3], k1_stride[3], q2_stride[3], k2_stride[3];
+  int student_activation;   /* STREAMKL_ACT_NONE | STREAMKL_ACT_RELU, see below */
 } streamkl_layout;
 
 /* streamkl_fwd / streamkl_bwd with an explicit layout (NULL = bf16, contiguous, HK = H: identical to the plain entry points). */

@@ -28,7 +28,8 @@ class StreamKLLayout(ctypes.Structure):
     """struct streamkl_layout of include/streamkl.h."""
 
     _fields_ = [("dtype", ctypes.c_int), ("kv_heads", ctypes.c_int), ("q1_stride", ctypes.c_longlong * 3),
-                ("k1_stride", ctypes.c_longlong * 3), ("q2_stride", ctypes.c_longlong * 3), ("k2_stride", ctypes.c_longlong * 3)]
+                ("k1_stride", ctypes.c_longlong * 3), ("q2_stride", ctypes.c_longlong * 3), ("k2_stride", ctypes.c_longlong * 3),
+                ("student_activation", ctypes.c_int)]
 STREAMKL_BWD_AUTO, STREAMKL_BWD_SEPARATE, STREAMKL_BWD_FUSED = 0, 1, 2
 
 
@@ -184,17 +185,23 @@ def _shape_of(Q1, K1, Q2, K2):
     return B, H, NQ, NK, d1, d2, HK
 
 
-def _layout_of(Q1, K1, Q2, K2, HK):
+STREAMKL_ACT_NONE, STREAMKL_ACT_RELU = 0, 1
+_ACTS = {None: STREAMKL_ACT_NONE, "none": STREAMKL_ACT_NONE, "relu": STREAMKL_ACT_RELU}
+
+
+def _layout_of(Q1, K1, Q2, K2, HK, student_activation=None):
     """A StreamKLLayout for 16-bit tensors given as (possibly strided) [B,H,N,d] views, or None when everything is the
     contiguous bf16 / fp32 default that the plain entry points take."""
     import torch
 
-    plain = all(t.is_contiguous() for t in (Q1, K1, Q2, K2)) and HK == Q1.shape[1]
+    act = _ACTS[student_activation]
+    plain = all(t.is_contiguous() for t in (Q1, K1, Q2, K2)) and HK == Q1.shape[1] and act == STREAMKL_ACT_NONE
     if plain and Q1.dtype in (torch.bfloat16, torch.float32):
         return None
     if Q1.dtype not in (torch.bfloat16, torch.float16):
-        raise TypeError("strided tensors / shared K heads need bfloat16 or float16 inputs")
+        raise TypeError("strided tensors / shared K heads / student activations need bfloat16 or float16 inputs")
     L = StreamKLLayout()
+    L.student_activation = act
     L.dtype = STREAMKL_BF16 if Q1.dtype == torch.bfloat16 else STREAMKL_F16
     L.kv_heads = int(HK)
     for name, t in (("q1_stride", Q1), ("k1_stride", K1), ("q2_stride", Q2), ("k2_stride", K2)):
@@ -221,7 +228,7 @@ def _ptr(t):
     return ctypes.c_void_p(t.data_ptr()) if t is not None else ctypes.c_void_p(0)
 
 
-def streamkl_fwd(Q1, K1, Q2, K2, c1, c2, causal, kl_rows=None, lse1=None, lse2=None, stream=None):
+def streamkl_fwd(Q1, K1, Q2, K2, c1, c2, causal, kl_rows=None, lse1=None, lse2=None, stream=None, student_activation=None):
     """Forward (Algorithm 1).  Returns (kl_rows, lse1, lse2), each [B,H,NQ] float32.  bf16 / fp16 / fp32 inputs; 16-bit inputs
     may be strided [B,H,N,d] views (last dimension contiguous) and K may have fewer heads than Q (shared K heads)."""
     import torch
@@ -229,7 +236,7 @@ def streamkl_fwd(Q1, K1, Q2, K2, c1, c2, causal, kl_rows=None, lse1=None, lse2=N
     for n, t in (("Q1", Q1), ("K1", K1), ("Q2", Q2), ("K2", K2)):
         _check_dev(n, t, Q1.dtype, strided=True)
     B, H, NQ, NK, d1, d2, HK = _shape_of(Q1, K1, Q2, K2)
-    layout = _layout_of(Q1, K1, Q2, K2, HK)
+    layout = _layout_of(Q1, K1, Q2, K2, HK, student_activation)
     outs = []
     for n, t in (("kl_rows", kl_rows), ("lse1", lse1), ("lse2", lse2)):
         if t is None:
@@ -289,7 +296,7 @@ def streamkl_fwd_splitk(Q1, K1, Q2, K2, c1, c2, causal, splits=0, kl_rows=None, 
 
 
 def streamkl_bwd(Q1, K1, Q2, K2, c1, c2, causal, kl_rows, lse1, lse2, dkl_rows, teacher=False,
-                 dQ1=None, dK1=None, dQ2=None, dK2=None, workspace=None, stream=None):
+                 dQ1=None, dK1=None, dQ2=None, dK2=None, workspace=None, stream=None, student_activation=None):
     """Backward by recomputation (Alg.2/3 + K-owner transposes).  Returns (dQ1, dK1, dQ2, dK2); dQ1,dK1 None unless teacher."""
     import torch
 
@@ -298,7 +305,7 @@ def streamkl_bwd(Q1, K1, Q2, K2, c1, c2, causal, kl_rows, lse1, lse2, dkl_rows, 
     for n, t in (("kl_rows", kl_rows), ("lse1", lse1), ("lse2", lse2), ("dkl_rows", dkl_rows)):
         _check_dev(n, t, torch.float32)
     B, H, NQ, NK, d1, d2, HK = _shape_of(Q1, K1, Q2, K2)
-    layout = _layout_of(Q1, K1, Q2, K2, HK)
+    layout = _layout_of(Q1, K1, Q2, K2, HK, student_activation)
     # every gradient has the shape AND the strides of its input (dQ_t like Q_t, dK_t like K_t)
     like = lambda t: torch.empty_strided(t.shape, t.stride(), dtype=t.dtype, device=t.device)
     if dQ2 is None:

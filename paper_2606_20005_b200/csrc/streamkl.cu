@@ -1,8 +1,11 @@
-// streamkl.cu -- the C-ABI boundary (include/streamkl.h): argument validation, TMA tensor maps, kernel dispatch.
-// No torch types, no allocation on the device entry points, no CPU fallback.
+// streamkl.cu -- the C-ABI boundary (include/streamkl.h): argument validation, layouts, strategy selection, the SIMT fallback
+// launchers, the host-buffer entry points and profiling.  The tensor-core kernel families are launched through the dispatchers
+// of streamkl_host.cuh, each compiled in its own translation unit (streamkl_fwd.cu, streamkl_bwd_q.cu, streamkl_bwd_k.cu,
+// streamkl_bwd_fused.cu).  No torch types, no allocation on the device entry points, no CPU fallback.
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
 
 #include <algorithm>
 #include <cmath>
@@ -10,25 +13,14 @@
 #include <cstring>
 #include <vector>
 
-#include "../../include/streamkl.h"
-#include "streamkl_fwd_sm100.cuh"
-#include "streamkl_bwd_sm100.cuh"
-#include "streamkl_bwd_fused_sm100.cuh"
+#include "streamkl_host.cuh"
 #include "streamkl_simt.cuh"
 
-namespace {
+namespace sklh {
 
 thread_local int g_last_launches = 0;
-thread_local int g_bwd_mode = STREAMKL_BWD_AUTO;
 
-// ---- optional per-kernel timing (streamkl_profile_*): CUDA events recorded on the launch stream around every kernel
-enum KernelId { KID_FWD_TC = 0, KID_BWD_DQ_TC, KID_BWD_DK_TC, KID_FWD_SIMT, KID_BWD_DQ_SIMT, KID_BWD_DK_SIMT, KID_BWD_STATS, KID_FWD_SPLITK_TC, KID_FWD_SPLITK_REDUCE, KID_BWD_FUSED_TC, KID_BWD_DQ_CONVERT, KID_COUNT };
-const char* const kKernelNames[KID_COUNT] = {"streamkl_fwd_sm100_kernel", "streamkl_bwd_sm100_kernel<OWNER_Q>",
-                                             "streamkl_bwd_sm100_kernel<OWNER_K>", "streamkl_fwd_simt_kernel",
-                                             "streamkl_bwd_simt_kernel<OWNER_Q>", "streamkl_bwd_simt_kernel<OWNER_K>",
-                                             "streamkl_bwd_stats_kernel", "streamkl_fwd_sm100_kernel<SPLIT>",
-                                             "streamkl_fwd_splitk_reduce_kernel", "streamkl_bwd_fused_sm100_kernel",
-                                             "streamkl_bwd_dq_convert_kernel"};
+namespace {
 struct ProfRecord { int id; cudaEvent_t a, b; };
 thread_local bool g_prof_on = false;
 thread_local std::vector<ProfRecord>* g_prof = nullptr;
@@ -45,21 +37,21 @@ void prof_release(cudaEvent_t e) {
   if (!g_prof_pool) g_prof_pool = new std::vector<cudaEvent_t>();
   g_prof_pool->push_back(e);
 }
+}  // namespace
 
-struct ProfScope {  // brackets ONE kernel launch; a no-op unless profiling is enabled on this thread
-  cudaStream_t st; cudaEvent_t b = nullptr;
-  ProfScope(int id, cudaStream_t s) : st(s) {
-    if (!g_prof_on) return;
-    if (!g_prof) g_prof = new std::vector<ProfRecord>();
-    cudaEvent_t a = prof_event();
-    if (!a) return;
-    b = prof_event();
-    if (!b) { prof_release(a); return; }
-    cudaEventRecord(a, st);
-    g_prof->push_back({id, a, b});
-  }
-  ~ProfScope() { if (b) cudaEventRecord(b, st); }
-};
+ProfScope::ProfScope(int id, cudaStream_t s) : st(s) {
+  if (!g_prof_on) return;
+  if (!g_prof) g_prof = new std::vector<ProfRecord>();
+  cudaEvent_t a = prof_event();
+  if (!a) return;
+  b = prof_event();
+  if (!b) { prof_release(a); return; }
+  cudaEventRecord(a, st);
+  g_prof->push_back({id, a, b});
+}
+ProfScope::~ProfScope() { if (b) cudaEventRecord(b, st); }
+
+namespace {
 
 using EncodeTiledFn = CUresult (*)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
                                    const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -85,9 +77,6 @@ bool device_is_sm100() {
   return major == 10;
 }
 
-// Element strides {batch, head, row} of one tensor (the head dimension is contiguous).
-struct Strides { long long b, h, n; };
-
 // 4-D map {d, N, heads, B} of a 16-bit tensor with arbitrary (batch, head, row) strides; box = {64 elements (128 B), box_rows, 1, 1},
 // 128-byte swizzle, zero OOB fill: rows beyond N and columns beyond d (head dims that are not 64 / 128) arrive as zeros.
 bool make_tmap_16(CUtensorMap* m, const void* base, int B, int heads, int N, int d, const Strides& st, int box_rows, bool f16) {
@@ -102,17 +91,6 @@ bool make_tmap_16(CUtensorMap* m, const void* base, int B, int heads, int N, int
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-struct Shape {
-  int B, H, NQ, NK, d1, d2, causal;
-  float c1, c2;
-  long long BH;
-  // layout (streamkl_layout): K heads, element strides of Q1, K1, Q2, K2 (gradients share their input's strides)
-  int HK = 0;
-  Strides q1{}, k1{}, q2{}, k2{};
-  bool default_layout = true;
-  int G() const { return HK > 0 ? H / HK : 1; }
-};
-
 Strides contiguous(int heads, int N, int d) { return Strides{(long long)heads * N * d, (long long)N * d, (long long)d}; }
 
 // fills the layout part of `s` from `L` (NULL = contiguous [B][H][N][d], HK = H) and validates it
@@ -121,8 +99,11 @@ int apply_layout(Shape& s, const streamkl_layout* L) {
   s.q1 = contiguous(s.H, s.NQ, s.d1); s.k1 = contiguous(s.H, s.NK, s.d1);
   s.q2 = contiguous(s.H, s.NQ, s.d2); s.k2 = contiguous(s.H, s.NK, s.d2);
   s.default_layout = true;
+  s.act2 = 0;
   if (!L) return STREAMKL_OK;
   if (L->kv_heads < 0) return STREAMKL_ERR_SHAPE;
+  if (L->student_activation != STREAMKL_ACT_NONE && L->student_activation != STREAMKL_ACT_RELU) return STREAMKL_ERR_SHAPE;
+  s.act2 = L->student_activation;
   if (L->kv_heads > 0) {
     if (s.H > 0 && (L->kv_heads > s.H || s.H % L->kv_heads != 0)) return STREAMKL_ERR_SHAPE;
     s.HK = L->kv_heads;
@@ -141,7 +122,7 @@ int apply_layout(Shape& s, const streamkl_layout* L) {
       (rc = take(L->q2_stride, s.q2, s.d2, s.NQ)) != STREAMKL_OK || (rc = take(L->k2_stride, s.k2, s.d2, s.NK)) != STREAMKL_OK)
     return rc;
   auto same = [](const Strides& a, const Strides& b) { return a.b == b.b && a.h == b.h && a.n == b.n; };
-  s.default_layout = s.HK == s.H && same(s.q1, contiguous(s.H, s.NQ, s.d1)) && same(s.k1, contiguous(s.H, s.NK, s.d1)) &&
+  s.default_layout = s.act2 == 0 && s.HK == s.H && same(s.q1, contiguous(s.H, s.NQ, s.d1)) && same(s.k1, contiguous(s.H, s.NK, s.d1)) &&
                      same(s.q2, contiguous(s.H, s.NQ, s.d2)) && same(s.k2, contiguous(s.H, s.NK, s.d2));
   return STREAMKL_OK;
 }
@@ -164,7 +145,8 @@ int validate_common(const void* Q1, const void* K1, const void* Q2, const void* 
 bool tc_shape(int dtype, const Shape& s) {
   return (dtype == STREAMKL_BF16 || dtype == STREAMKL_F16) && s.d1 % 8 == 0 && s.d2 % 8 == 0 && s.d1 <= 128 && s.d2 <= 128;
 }
-int pad_dim(int d) { return d <= 64 ? 64 : 128; }
+
+}  // namespace
 
 bool make_maps(CUtensorMap (&t)[4], const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, int rows_q, int rows_k,
                bool f16) {
@@ -172,52 +154,21 @@ bool make_maps(CUtensorMap (&t)[4], const void* Q1, const void* K1, const void* 
          make_tmap_16(&t[2], Q2, s.B, s.H, s.NQ, s.d2, s.q2, rows_q, f16) && make_tmap_16(&t[3], K2, s.B, s.HK, s.NK, s.d2, s.k2, rows_k, f16);
 }
 
-// ----------------------------------------------------------------------------------------- forward launchers
-// splits == 1: the default kernel (grid (bsz, T_Q)).  splits > 1: split-K (grid (bsz, T_Q, W), partial
-// statistics to `part`, then the reduce kernel).
-template <int D1, int D2, bool CAUSAL, bool SPLIT = false>
-int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, float* kl, float* lse1,
-                  float* lse2, cudaStream_t stream, int splits = 1, float* part = nullptr) {
-  using C = skl::FwdCfg<D1, D2>;
-  CUtensorMap tm[4];
-  if (!make_maps(tm, Q1, K1, Q2, K2, s, C::BM, C::BK, f16)) return STREAMKL_ERR_CUDA;
-  const CUtensorMap &tQ1 = tm[0], &tK1 = tm[1], &tQ2 = tm[2], &tK2 = tm[3];
-  auto kern = skl::streamkl_fwd_sm100_kernel<D1, D2, CAUSAL, SPLIT>;
-  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
-    cudaGetLastError();
-    return STREAMKL_ERR_CUDA;
-  }
-  skl::FwdParams p;
-  p.NQ = s.NQ; p.NK = s.NK; p.BH = int(s.BH);
-  p.H = s.H; p.G = s.G(); p.fmt16 = f16 ? 0u : 1u;
-  p.TQ = (s.NQ + C::BQ - 1) / C::BQ;
-  p.sc1 = s.c1 * 1.4426950408889634f;
-  p.sc2 = s.c2 * 1.4426950408889634f;
-  p.kl = kl; p.lse1 = lse1; p.lse2 = lse2;
-  const int TK = (s.NK + C::BK - 1) / C::BK;
-  p.chunk_steps = SPLIT ? (TK + splits - 1) / splits : TK;       // C_K = ceil(N_K / W), in whole BK-key steps
-  p.W = SPLIT ? (TK + p.chunk_steps - 1) / p.chunk_steps : 1;    // no empty trailing chunk
-  p.part = part;
-  const long long grid = (long long)p.TQ * s.BH * p.W;
-  if (grid > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
-  {
-    ProfScope ps(SPLIT ? KID_FWD_SPLITK_TC : KID_FWD_TC, stream);
-    kern<<<dim3((unsigned)grid), C::THREADS, C::SMEM_BYTES, stream>>>(tQ1, tK1, tQ2, tK2, p);
-  }
-  if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
-  g_last_launches += 1;
-  if (SPLIT) {
-    const long long rows = s.BH * (long long)s.NQ;
-    {
-      ProfScope ps(KID_FWD_SPLITK_REDUCE, stream);
-      skl::streamkl_fwd_splitk_reduce_kernel<<<dim3((unsigned)((rows + 127) / 128)), 128, 0, stream>>>(part, s.NQ, p.W, rows, kl, lse1, lse2);
-    }
-    if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
-    g_last_launches += 1;
-  }
-  return STREAMKL_OK;
-}
+}  // namespace sklh
 
+namespace {
+using namespace sklh;
+
+thread_local int g_bwd_mode = STREAMKL_BWD_AUTO;
+
+// ---- optional per-kernel timing (streamkl_profile_*): CUDA events recorded on the launch stream around every kernel
+const char* const kKernelNames[KID_COUNT] = {"streamkl_fwd_sm100_kernel", "streamkl_bwd_sm100_kernel<OWNER_Q>",
+                                             "streamkl_bwd_sm100_kernel<OWNER_K>", "streamkl_fwd_simt_kernel",
+                                             "streamkl_bwd_simt_kernel<OWNER_Q>", "streamkl_bwd_simt_kernel<OWNER_K>",
+                                             "streamkl_bwd_stats_kernel", "streamkl_fwd_sm100_kernel<SPLIT>",
+                                             "streamkl_fwd_splitk_reduce_kernel", "streamkl_bwd_fused_sm100_kernel",
+                                             "streamkl_bwd_dq_convert_kernel"};
+// ----------------------------------------------------------------------------------------- forward (SIMT fallback, dispatch)
 int simt_block_rows(size_t floats_per_row, size_t fixed_floats, size_t* smem_bytes) {
   for (int br : {128, 64, 32}) {
     size_t b = (floats_per_row * br + fixed_floats) * sizeof(float);
@@ -262,30 +213,14 @@ int fwd_dispatch(int dtype, const streamkl_layout* L, const void* Q1, const void
   if (!kl || !lse1 || !lse2) return STREAMKL_ERR_NULLPTR;
   if (!tc_shape(dtype, s) && !s.default_layout) return STREAMKL_ERR_SHAPE;   // strides / shared K heads: tensor-core path only
   if (!device_is_sm100()) return STREAMKL_ERR_CUDA;
-  if (tc_shape(dtype, s)) {
-    const bool f16 = dtype == STREAMKL_F16;
-    const int p1 = pad_dim(d1), p2 = pad_dim(d2);
-#define SKL_FWD_CASE(A, Bd)                                                                                                       \
-  if (p1 == A && p2 == Bd) {                                                                                                      \
-    if (splits > 1)                                                                                                               \
-      return s.causal ? launch_fwd_tc<A, Bd, true, true>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream, splits, part)            \
-                      : launch_fwd_tc<A, Bd, false, true>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream, splits, part);          \
-    return s.causal ? launch_fwd_tc<A, Bd, true>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream)                                  \
-                    : launch_fwd_tc<A, Bd, false>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream);                                \
-  }
-    SKL_FWD_CASE(128, 128)
-    SKL_FWD_CASE(128, 64)
-    SKL_FWD_CASE(64, 128)
-    SKL_FWD_CASE(64, 64)
-#undef SKL_FWD_CASE
-  }
+  if (tc_shape(dtype, s)) return fwd_tc_launch(Q1, K1, Q2, K2, s, dtype == STREAMKL_F16, kl, lse1, lse2, stream, splits, part);
   if (s.BH > 65535) return STREAMKL_ERR_SHAPE;   // SIMT grids put the head index in gridDim.y
   if (dtype == STREAMKL_BF16) return launch_fwd_simt<__nv_bfloat16>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream);
   if (dtype == STREAMKL_F16) return launch_fwd_simt<__half>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream);
   return launch_fwd_simt<float>(Q1, K1, Q2, K2, s, kl, lse1, lse2, stream);
 }
 
-// ----------------------------------------------------------------------------------------- backward launchers
+// ----------------------------------------------------------------------------------------- backward (SIMT fallback, strategy, dispatch)
 template <typename T, bool OWNER_K>
 int launch_bwd_simt(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, const float* kl,
                     const float* lse1, const float* lse2, const float* dkl, void* dX1, void* dX2, cudaStream_t stream) {
@@ -310,42 +245,6 @@ int launch_bwd_simt(const void* Q1, const void* K1, const void* Q2, const void* 
   return STREAMKL_OK;
 }
 
-skl::OutGeom out_geom(const Strides& st, int d) { return skl::OutGeom{st.b, st.h, st.n, d}; }
-
-template <int D1, int D2, bool CAUSAL, bool TEACHER, bool OWNER_K>
-int launch_bwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, const float4* stats, void* dX1,
-                  void* dX2, cudaStream_t stream) {
-  using C = skl::BwdCfg<D1, D2, TEACHER>;
-  CUtensorMap tm[4];
-  // the owner side is loaded in 128-row boxes, the streamed side in BY-row boxes
-  const int rq = OWNER_K ? C::BY : C::BX, rk = OWNER_K ? C::BX : C::BY;
-  if (!make_maps(tm, Q1, K1, Q2, K2, s, rq, rk, f16)) return STREAMKL_ERR_CUDA;
-  auto kern = skl::streamkl_bwd_sm100_kernel<D1, D2, CAUSAL, TEACHER, OWNER_K>;
-  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
-    cudaGetLastError();
-    return STREAMKL_ERR_CUDA;
-  }
-  skl::BwdParams p;
-  p.NQ = s.NQ; p.NK = s.NK; p.BH = int(s.BH);
-  p.H = s.H; p.HK = s.HK; p.G = s.G(); p.fmt16 = f16 ? 0u : 1u;
-  p.TX = ((OWNER_K ? s.NK : s.NQ) + C::BX - 1) / C::BX;
-  p.c1 = s.c1; p.c2 = s.c2;
-  p.stats = stats;
-  p.dX1 = static_cast<uint16_t*>(dX1);
-  p.dX2 = static_cast<uint16_t*>(dX2);
-  p.g1 = out_geom(OWNER_K ? s.k1 : s.q1, s.d1);   // dK_t has K_t's strides, dQ_t has Q_t's
-  p.g2 = out_geom(OWNER_K ? s.k2 : s.q2, s.d2);
-  const long long grid = (long long)p.TX * s.B * (OWNER_K ? s.HK : s.H);
-  if (grid > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
-  {
-    ProfScope ps(OWNER_K ? KID_BWD_DK_TC : KID_BWD_DQ_TC, stream);
-    kern<<<dim3((unsigned)grid), C::THREADS, C::SMEM_BYTES, stream>>>(tm[0], tm[1], tm[2], tm[3], p);
-  }
-  if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
-  g_last_launches += 1;
-  return STREAMKL_OK;
-}
-
 // Strategy selection of the backward (see bwd_tc_both): the one-visit kernels iff the mode is FUSED, or AUTO below the measured
 // crossover (bench.py "backward strategies", profiles/r02_bwd_strategies.md): at most four 128-query tiles per head for
 // Setting 1 (one pass: half the recomputation), at most two for Setting 2 (two passes: same work as the owner kernels, the
@@ -356,91 +255,30 @@ bool bwd_fused_selected(int NQ, bool teacher) {
 }
 size_t fused_acc_bytes_aligned(long long BH, int NQ, int d) { return (size_t(BH) * size_t(NQ) * size_t(d) * sizeof(float) + 255) & ~size_t(255); }
 
-size_t stats_bytes_aligned(long long BH, int NQ) { return (size_t(BH) * size_t(skl::bwd_stats_padded_rows(NQ)) * 16 + 255) & ~size_t(255); }
+size_t stats_bytes_aligned(long long BH, int NQ) { return (size_t(BH) * size_t(stats_padded_rows(NQ)) * 16 + 255) & ~size_t(255); }
 
-// One one-visit pass: zero the fp32 dQ accumulator, run the fused K-owner kernel, convert dQ.
-// TPASS = false: student (dS2 -> dQ2, dK2); true: teacher (dS1 -> dQ1, dK1).
-template <int D1, int D2, bool CAUSAL, bool TPASS>
-int launch_bwd_fused(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, const float4* stats,
-                     float* dq_acc, void* dQ, void* dK, cudaStream_t stream) {
-  using C = skl::BwdFusedCfg<D1, D2, TPASS>;
-  CUtensorMap tm[4];
-  if (!make_maps(tm, Q1, K1, Q2, K2, s, C::BY, C::BX, f16)) return STREAMKL_ERR_CUDA;
-  auto kern = skl::streamkl_bwd_fused_sm100_kernel<D1, D2, CAUSAL, TPASS>;
-  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
-    cudaGetLastError();
-    return STREAMKL_ERR_CUDA;
-  }
-  const size_t n = size_t(s.BH) * s.NQ * C::DG;
-  if (cudaMemsetAsync(dq_acc, 0, n * sizeof(float), stream) != cudaSuccess) { cudaGetLastError(); return STREAMKL_ERR_CUDA; }
-  skl::BwdFusedParams p;
-  p.NQ = s.NQ; p.NK = s.NK; p.BH = int(s.BH);
-  p.H = s.H; p.HK = s.HK; p.G = s.G(); p.fmt16 = f16 ? 0u : 1u;
-  p.TX = (s.NK + C::BX - 1) / C::BX;
-  p.c1 = s.c1; p.c2 = s.c2;
-  p.stats = stats; p.dq_acc = dq_acc;
-  p.dK = static_cast<uint16_t*>(dK);
-  p.gk = out_geom(TPASS ? s.k1 : s.k2, TPASS ? s.d1 : s.d2);
-  const long long grid = (long long)p.TX * s.B * s.HK;
-  if (grid > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
-  {
-    ProfScope ps(KID_BWD_FUSED_TC, stream);
-    kern<<<dim3((unsigned)grid), C::THREADS, C::SMEM_BYTES, stream>>>(tm[0], tm[1], tm[2], tm[3], p);
-  }
-  if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
-  const long long n4 = (long long)(n / 4);
-  {
-    ProfScope ps(KID_BWD_DQ_CONVERT, stream);
-    skl::streamkl_bwd_dq_convert_kernel<<<dim3((unsigned)((n4 + 255) / 256)), 256, 0, stream>>>(
-        reinterpret_cast<const float4*>(dq_acc), static_cast<uint16_t*>(dQ), TPASS ? s.c1 * 0.6931471805599453f : s.c2, n4, s.NQ, s.H,
-        C::DG, out_geom(TPASS ? s.q1 : s.q2, TPASS ? s.d1 : s.d2), f16 ? 1 : 0);
-  }
-  if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
-  g_last_launches += 2;
-  return STREAMKL_OK;
-}
-
-template <int D1, int D2>
+// B1 pre-pass, then the selected strategy.
 int bwd_tc_both(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, const float* kl, const float* lse1,
                 const float* lse2, const float* dkl, void* dQ1, void* dK1, void* dQ2, void* dK2, void* workspace, cudaStream_t st) {
   const bool t = dQ1 != nullptr;
-  int rc;
-  // B1: per-query scalars, packed for the dS warps, into the caller's workspace
-  float4* stats = static_cast<float4*>(workspace);
-  {
-    const long long pph = skl::bwd_stats_padded_rows(s.NQ) / 2, total = pph * s.BH;
-    const long long blocks = (total + 255) / 256;
-    if (blocks > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
-    {
-      ProfScope ps(KID_BWD_STATS, st);
-      skl::streamkl_bwd_stats_kernel<<<dim3((unsigned)blocks), 256, 0, st>>>(kl, lse1, lse2, dkl, stats, s.NQ, pph, total);
-    }
-    if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
-    g_last_launches += 1;
-  }
+  int rc = bwd_stats_launch(s, kl, lse1, lse2, dkl, workspace, st);
+  if (rc != STREAMKL_OK) return rc;
   // Strategy (PAPER.md:321 picks fused iff T_Q*C <= T_K with an empirically tuned C).  Measured on B200
   // (profiles/r01f_fused_bwd.md, r02_bwd_strategies.md): the one-visit kernels win while the Q-owner grid is small (Setting 1:
   // 1.3-3.0x up to T_Q = 4 tiles of 128 queries, level at 8; Setting 2: 1.3-1.5x up to T_Q = 2, 0.8x at 4) and lose beyond,
   // where their fp32 atomics (64 KB per 128x128 tile pair and pass) run into the L2's atomic throughput; the crossover did
   // not move with T_K (128 vs 1024), so the rule is on T_Q alone.
-  const bool fused = bwd_fused_selected(s.NQ, t);
-  if (fused) {   // one visit per differentiated distribution, dQ through fp32 atomics
+  if (bwd_fused_selected(s.NQ, t)) {   // one visit per differentiated distribution, dQ through fp32 atomics
     uint8_t* w = static_cast<uint8_t*>(workspace) + stats_bytes_aligned(s.BH, s.NQ);
     float* acc2 = reinterpret_cast<float*>(w);
-    float* acc1 = reinterpret_cast<float*>(w + fused_acc_bytes_aligned(s.BH, s.NQ, D2));
-    rc = s.causal ? launch_bwd_fused<D1, D2, true, false>(Q1, K1, Q2, K2, s, f16, stats, acc2, dQ2, dK2, st)
-                  : launch_bwd_fused<D1, D2, false, false>(Q1, K1, Q2, K2, s, f16, stats, acc2, dQ2, dK2, st);
+    float* acc1 = reinterpret_cast<float*>(w + fused_acc_bytes_aligned(s.BH, s.NQ, pad_dim(s.d2)));
+    rc = bwd_tc_fused_launch(Q1, K1, Q2, K2, s, f16, false, workspace, acc2, dQ2, dK2, st);
     if (rc != STREAMKL_OK || !t) return rc;
-    return s.causal ? launch_bwd_fused<D1, D2, true, true>(Q1, K1, Q2, K2, s, f16, stats, acc1, dQ1, dK1, st)
-                    : launch_bwd_fused<D1, D2, false, true>(Q1, K1, Q2, K2, s, f16, stats, acc1, dQ1, dK1, st);
+    return bwd_tc_fused_launch(Q1, K1, Q2, K2, s, f16, true, workspace, acc1, dQ1, dK1, st);
   }
-#define SKL_BWD(CA, TE)                                                                                                   \
-  rc = launch_bwd_tc<D1, D2, CA, TE, false>(Q1, K1, Q2, K2, s, f16, stats, dQ1, dQ2, st);                                 \
-  if (rc != STREAMKL_OK) return rc;                                                                                       \
-  return launch_bwd_tc<D1, D2, CA, TE, true>(Q1, K1, Q2, K2, s, f16, stats, dK1, dK2, st);
-  if (s.causal) { if (t) { SKL_BWD(true, true) } else { SKL_BWD(true, false) } }
-  else          { if (t) { SKL_BWD(false, true) } else { SKL_BWD(false, false) } }
-#undef SKL_BWD
+  rc = bwd_tc_owner_q_launch(Q1, K1, Q2, K2, s, f16, workspace, dQ1, dQ2, st);
+  if (rc != STREAMKL_OK) return rc;
+  return bwd_tc_owner_k_launch(Q1, K1, Q2, K2, s, f16, workspace, dK1, dK2, st);
 }
 
 int bwd_dispatch(int dtype, const streamkl_layout* L, const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ,
@@ -471,14 +309,8 @@ int bwd_dispatch(int dtype, const streamkl_layout* L, const void* Q1, const void
     if (dK1 && cudaMemsetAsync(dK1, 0, size_t(s.BH) * NK * d1 * es, stream) != cudaSuccess) return STREAMKL_ERR_CUDA;
     return STREAMKL_OK;
   }
-  if (tc_shape(dtype, s)) {
-    const bool f16 = dtype == STREAMKL_F16;
-    const int p1 = pad_dim(d1), p2 = pad_dim(d2);
-    if (p1 == 128 && p2 == 128) return bwd_tc_both<128, 128>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, workspace, stream);
-    if (p1 == 128 && p2 == 64) return bwd_tc_both<128, 64>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, workspace, stream);
-    if (p1 == 64 && p2 == 128) return bwd_tc_both<64, 128>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, workspace, stream);
-    return bwd_tc_both<64, 64>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, workspace, stream);
-  }
+  if (tc_shape(dtype, s))
+    return bwd_tc_both(Q1, K1, Q2, K2, s, dtype == STREAMKL_F16, kl, lse1, lse2, dkl, dQ1, dK1, dQ2, dK2, workspace, stream);
   if (s.BH > 65535) return STREAMKL_ERR_SHAPE;   // SIMT grids put the head index in gridDim.y
   if (dtype == STREAMKL_BF16) {
     rc = launch_bwd_simt<__nv_bfloat16, false>(Q1, K1, Q2, K2, s, kl, lse1, lse2, dkl, dQ1, dQ2, stream);
@@ -585,9 +417,8 @@ int streamkl_fwd_splitk_splits(int B, int H, int NQ, int NK, int p_target) {
   // adaptive split selection: P_base = bsz * T_Q; W = 1 if P_base >= P_target, else min(floor(P_target / P_base), T_K)
   if (B <= 0 || H <= 0 || NQ <= 0 || NK <= 0) return 1;
   if (p_target <= 0) p_target = 148;   // one CTA per SM of a B200 = one full wave (measured best: profiles/r01d_splitk.md)
-  using C = skl::FwdCfg<128, 128>;   // tile sizes of the forward kernel (the same for every head-dim pair)
-  const long long p_base = (long long)B * H * ((NQ + C::BQ - 1) / C::BQ);
-  const long long tk = (NK + C::BK - 1) / C::BK;
+  const long long p_base = (long long)B * H * ((NQ + kFwdBQ - 1) / kFwdBQ);
+  const long long tk = (NK + kFwdBK - 1) / kFwdBK;
   if (p_base >= p_target) return 1;
   const long long w = p_target / p_base;
   return int(w < tk ? w : tk);
@@ -602,7 +433,7 @@ int streamkl_fwd_splitk(const void* Q1, const void* K1, const void* Q2, const vo
                         float c1, float c2, int causal, int splits, float* kl_rows, float* lse1, float* lse2, void* workspace,
                         size_t workspace_bytes, streamkl_stream_t stream) {
   if (splits <= 0) splits = streamkl_fwd_splitk_splits(B, H, NQ, NK, 0);
-  const int tk = NK > 0 ? (NK + skl::FwdCfg<128, 128>::BK - 1) / skl::FwdCfg<128, 128>::BK : 1;
+  const int tk = NK > 0 ? (NK + kFwdBK - 1) / kFwdBK : 1;
   if (splits > tk) splits = tk;
   const bool tc = d1 % 8 == 0 && d2 % 8 == 0 && d1 >= 8 && d2 >= 8 && d1 <= 128 && d2 <= 128;
   if (!tc || splits <= 1)   // other head dims run the (unsplit) SIMT kernel; W = 1 is the default kernel
@@ -621,7 +452,7 @@ size_t streamkl_bwd_workspace_bytes(int B, int H, int NQ, int, int d1, int d2, i
   if (B <= 0 || H <= 0 || NQ <= 0) return 0;
   if (!(d1 % 8 == 0 && d2 % 8 == 0 && d1 >= 8 && d2 >= 8 && d1 <= 128 && d2 <= 128)) return 0;   // SIMT path: no workspace
   const long long BH = (long long)B * H;
-  if (!bwd_fused_selected(NQ, want_teacher != 0)) return size_t(BH) * size_t(skl::bwd_stats_padded_rows(NQ)) * 16;
+  if (!bwd_fused_selected(NQ, want_teacher != 0)) return size_t(BH) * size_t(stats_padded_rows(NQ)) * 16;
   // one-visit kernels (mode FUSED, or AUTO with NQ <= 512): + their fp32 dQ accumulators, O(NQ d)
   return stats_bytes_aligned(BH, NQ) + fused_acc_bytes_aligned(BH, NQ, pad_dim(d2)) + (want_teacher ? fused_acc_bytes_aligned(BH, NQ, pad_dim(d1)) : 0);
 }
@@ -668,7 +499,7 @@ int streamkl_fwd_bwd_host(int dtype, const void* Q1, const void* K1, const void*
   const long long BH = s.BH;
   long long gs = BH;   // heads per group
   if (BH > 1 && (size_t(d1) * es) % 16 == 0 && (size_t(d2) * es) % 16 == 0 && size_t(BH) * (hq1 + hk1 + hq2 + hk2) >= (64u << 20)) {
-    const long long tq = (NQ + skl::FwdCfg<128, 128>::BQ - 1) / skl::FwdCfg<128, 128>::BQ;   // forward CTAs per head
+    const long long tq = (NQ + kFwdBQ - 1) / kFwdBQ;   // forward CTAs per head
     const long long fill = (2 * 148 + tq - 1) / (tq > 0 ? tq : 1);   // enough CTAs per launch for two waves
     gs = (BH + 7) / 8;
     if (gs < fill) gs = fill;

@@ -54,6 +54,7 @@ struct BwdFusedParams {
   int NQ, NK, TX, BH;    // BH = B * H query heads
   int H, HK, G;          // query heads, K heads, query heads per K head (GQA)
   uint32_t fmt16;        // 1 bf16, 0 fp16
+  int act2;              // student activation: 0 none, 1 relu (R23)
   float c1, c2;
   const float4* stats;   // as BwdParams::stats
   float* dq_acc;         // [BH][NQ][DG] fp32, zeroed by the caller of the kernel
@@ -282,7 +283,7 @@ streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const 
     };
 
     int last = -1;
-    const bool f16 = p.fmt16 == 0;
+    const bool f16 = p.fmt16 == 0, relu2 = p.act2 == 1;
     for (int it = par; it < nsteps; it += 2) {
       const int j = step_j(it);
       const int s = it % C::NSTAGE;
@@ -306,13 +307,10 @@ streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const 
       const uint32_t stat = stat_base + s * C::STAT_STAGE;
       // (o2 = the pass's dS: the teacher pass takes ds_row's dS1 output)
       uint32_t (&f1)[16] = *(TPASS ? &o2 : &o1), (&f2)[16] = *(TPASS ? &o1 : &o2);
-      if (!f16) {
-        if (masked) ds_row<32, TPASS, true, CAUSAL, true, !TPASS>(r1, r2, f1, f2, sc1, sc2, 0.f, 0.f, 0.f, stat, xrow, y0, off, p.NK);
-        else        ds_row<32, TPASS, true, CAUSAL, false, !TPASS>(r1, r2, f1, f2, sc1, sc2, 0.f, 0.f, 0.f, stat, xrow, y0, off, p.NK);
-      } else {
-        if (masked) ds_row<32, TPASS, true, CAUSAL, true, !TPASS, true>(r1, r2, f1, f2, sc1, sc2, 0.f, 0.f, 0.f, stat, xrow, y0, off, p.NK);
-        else        ds_row<32, TPASS, true, CAUSAL, false, !TPASS, true>(r1, r2, f1, f2, sc1, sc2, 0.f, 0.f, 0.f, stat, xrow, y0, off, p.NK);
-      }
+      dispatch3(masked, f16, relu2, [&](auto m, auto h, auto r) {
+        ds_row<32, TPASS, true, CAUSAL, decltype(m)::value, !TPASS, decltype(h)::value, decltype(r)::value>(
+            r1, r2, f1, f2, sc1, sc2, 0.f, 0.f, 0.f, stat, xrow, y0, off, p.NK);
+      });
       mbar_wait(&ds_empty[par], (u & 1) ^ 1);   // the MMAs of step it-2 have consumed both copies of this dS2 stage
       tc_fence_after();
       tmem_st16(ds_taddr, o2);

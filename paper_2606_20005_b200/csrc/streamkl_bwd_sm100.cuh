@@ -30,6 +30,8 @@
 #include <cuda_bf16.h>
 #include <math_constants.h>
 
+#include <type_traits>
+
 #include "sm100_ptx.cuh"
 
 // Share of the backward's exps evaluated by the FMA-pipe polynomial (ex2_poly2): one column pair in every N (0 = none),
@@ -86,6 +88,7 @@ struct BwdParams {
   int NQ, NK, TX, BH;   // BH = B * H query heads
   int H, HK, G;         // query heads, K heads (H = HK * G), query heads per K head (GQA)
   uint32_t fmt16;       // 16-bit element format of inputs and gradients: 1 bf16, 0 fp16
+  int act2;             // student activation: 0 none, 1 relu (s2 = relu(c2 <q2,k2>), R23): gates dS2 with relu'
   float c1, c2;
   const float4* stats;  // [B*H][NQP/2][2] float4, NQP = bwd_stats_padded_rows(NQ)
   uint16_t* dX1;        // dQ1 or dK1 (nullptr when !TEACHER), 16-bit elements
@@ -94,7 +97,7 @@ struct BwdParams {
 };
 
 // B1: per-query scalars in the layout the dS warps consume (see the header comment)
-__global__ void streamkl_bwd_stats_kernel(const float* __restrict__ kl, const float* __restrict__ lse1, const float* __restrict__ lse2,
+static __global__ void streamkl_bwd_stats_kernel(const float* __restrict__ kl, const float* __restrict__ lse1, const float* __restrict__ lse2,
                                           const float* __restrict__ dkl, float4* __restrict__ stats, int NQ, long long pairs_per_head,
                                           long long total_pairs) {
   const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -169,7 +172,9 @@ __device__ __forceinline__ float4 lds_f4(uint32_t saddr) {
 //   OWNER_K: per-column scalars come from shared memory (`stat`: shared-space address of these NC/2 column
 //            pairs, two float4 each), g is applied here.
 // MASKED: causal diagonal tiles and streamed-key tails; P (possibly inf for a zero-filled logit) is discarded by SELECT.
-template <int NC, bool TEACHER, bool OWNER_K, bool CAUSAL, bool MASKED, bool WANT2 = true, bool F16 = false>
+// RELU2 (R23): the student's logit is relu(s2'), i.e. x2 = max(x2_raw, -lse2 log2e) in the shifted log2 domain,
+// and relu' = 1[x2_raw > -lse2 log2e] gates dS2.
+template <int NC, bool TEACHER, bool OWNER_K, bool CAUSAL, bool MASKED, bool WANT2 = true, bool F16 = false, bool RELU2 = false>
 __device__ __forceinline__ void ds_row(const uint32_t (&r1)[NC], const uint32_t (&r2)[NC], uint32_t (&o1)[NC / 2], uint32_t (&o2)[NC / 2],
                                          float sc1, float sc2, float nL1, float nL2, float klog, uint32_t stat, int xrow,
                                          int y0, int off, int NK) {
@@ -182,7 +187,12 @@ __device__ __forceinline__ void ds_row(const uint32_t (&r1)[NC], const uint32_t 
       vn1 = make_float2(a.x, a.y); vn2 = make_float2(a.z, a.w); vg = make_float2(b.x, b.y); vk = make_float2(b.z, b.w);
     }
     const float2 x1 = fma2(make_float2(__uint_as_float(r1[e]), __uint_as_float(r1[e + 1])), vsc1, vn1);
-    const float2 x2 = fma2(make_float2(__uint_as_float(r2[e]), __uint_as_float(r2[e + 1])), vsc2, vn2);
+    float2 x2 = fma2(make_float2(__uint_as_float(r2[e]), __uint_as_float(r2[e + 1])), vsc2, vn2);
+    bool on0 = true, on1 = true;
+    if constexpr (RELU2) {
+      on0 = x2.x > vn2.x; on1 = x2.y > vn2.y;
+      x2 = make_float2(fmaxf(x2.x, vn2.x), fmaxf(x2.y, vn2.y));
+    }
     // P_t = exp(s_t - lse_t) (Alg.2 line 7); one column pair in every STREAMKL_BWD_POLY_EVERY on the FMA/ALU pipes
     constexpr int PE = TEACHER ? (OWNER_K ? STREAMKL_BWD_POLY_TEACHER_K : STREAMKL_BWD_POLY_TEACHER_Q) : STREAMKL_BWD_POLY_STUDENT;
     const bool poly = PE > 0 && ((e >> 1) % (PE > 0 ? PE : 1)) == 0;
@@ -192,6 +202,7 @@ __device__ __forceinline__ void ds_row(const uint32_t (&r1)[NC], const uint32_t 
     if constexpr (WANT2) {
       a2 = sub2(p2, p1);                                                 // dS2 / g (Alg.2 line 8): fp32 subtract, rounded once below
       if constexpr (OWNER_K) a2 = mul2(a2, vg);
+      if constexpr (RELU2) { a2.x = on0 ? a2.x : 0.f; a2.y = on1 ? a2.y : 0.f; }
     }
     float2 a1 = make_float2(0.f, 0.f);
     if constexpr (TEACHER) {                                             // dS1 / (g ln2) = P1 (x1 - x2 - kl log2e)   (Alg.3 lines 9-10, Eq.12)
@@ -211,6 +222,15 @@ __device__ __forceinline__ void ds_row(const uint32_t (&r1)[NC], const uint32_t 
   }
 }
 
+
+// three warp-uniform run-time flags -> compile-time tags (one branch tree per step; nothing inside ds_row's loop)
+template <class F>
+__device__ __forceinline__ void dispatch3(bool a, bool b, bool c, F&& f) {
+  using T = std::true_type;
+  using N = std::false_type;
+  if (a) { if (b) { if (c) f(T{}, T{}, T{}); else f(T{}, T{}, N{}); } else { if (c) f(T{}, N{}, T{}); else f(T{}, N{}, N{}); } }
+  else   { if (b) { if (c) f(N{}, T{}, T{}); else f(N{}, T{}, N{}); } else { if (c) f(N{}, N{}, T{}); else f(N{}, N{}, N{}); } }
+}
 
 template <int D1, int D2, bool CAUSAL, bool TEACHER, bool OWNER_K>
 __global__ void __launch_bounds__(BwdCfg<D1, D2, TEACHER>::THREADS, 1)
@@ -408,7 +428,7 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
     const uint32_t lane_addr = tmem_base + (uint32_t(quarter * 32) << 16);
     const uint32_t stat_base = smem_u32(sStat) + half * 32 * 16;
     const uint32_t ds_addr = lane_addr + C::COL_DS + par * 64 + half * 16;   // dS1 here, dS2 32 columns further
-    const bool f16 = p.fmt16 == 0;
+    const bool f16 = p.fmt16 == 0, relu2 = p.act2 == 1;
     for (int it = par; it < nsteps; it += 2) {
       const int j = step_j(it);
       const int s = it % C::NSTAGE;
@@ -429,13 +449,10 @@ streamkl_bwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
       const bool masked = OWNER_K ? (CAUSAL && (y0 + off < x0 + C::BX - 1))
                                   : ((CAUSAL && (y0 + 31 > x0 + off)) || (y0 + 32 > p.NK));
       const uint32_t stat = stat_base + s * C::STAT_STAGE;
-      if (!f16) {
-        if (masked) ds_row<32, TEACHER, OWNER_K, CAUSAL, true>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
-        else        ds_row<32, TEACHER, OWNER_K, CAUSAL, false>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
-      } else {
-        if (masked) ds_row<32, TEACHER, OWNER_K, CAUSAL, true, true, true>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
-        else        ds_row<32, TEACHER, OWNER_K, CAUSAL, false, true, true>(r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
-      }
+      dispatch3(masked, f16, relu2, [&](auto m, auto h, auto r) {
+        ds_row<32, TEACHER, OWNER_K, CAUSAL, decltype(m)::value, true, decltype(h)::value, decltype(r)::value>(
+            r1, r2, o1, o2, sc1, sc2, nL1, nL2, klog, stat, xrow, y0, off, p.NK);
+      });
       mbar_wait(&ds_empty[par], ((it >> 1) & 1) ^ 1);   // the dX MMAs of step it-2 have consumed this dS stage
       tc_fence_after();
       tmem_st16(ds_addr + 32, o2);

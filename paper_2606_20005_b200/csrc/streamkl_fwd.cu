@@ -1,0 +1,76 @@
+// streamkl_fwd.cu -- launchers of the tcgen05 forward kernel (default grid and split-K + reduce); see streamkl.cu for the C ABI.
+#include "streamkl_host.cuh"
+#include "streamkl_fwd_sm100.cuh"
+
+namespace sklh {
+namespace {
+
+static_assert(skl::FwdCfg<128, 128>::BQ == kFwdBQ && skl::FwdCfg<64, 64>::BK == kFwdBK, "tile sizes quoted in streamkl_host.cuh");
+
+// splits == 1: the default kernel (grid (bsz, T_Q)).  splits > 1: split-K (grid (bsz, T_Q, W), partial
+// statistics to `part`, then the reduce kernel).
+template <int D1, int D2, bool CAUSAL, bool SPLIT = false>
+int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, float* kl, float* lse1,
+                  float* lse2, cudaStream_t stream, int splits = 1, float* part = nullptr) {
+  using C = skl::FwdCfg<D1, D2>;
+  CUtensorMap tm[4];
+  if (!make_maps(tm, Q1, K1, Q2, K2, s, C::BM, C::BK, f16)) return STREAMKL_ERR_CUDA;
+  const CUtensorMap &tQ1 = tm[0], &tK1 = tm[1], &tQ2 = tm[2], &tK2 = tm[3];
+  auto kern = skl::streamkl_fwd_sm100_kernel<D1, D2, CAUSAL, SPLIT>;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
+    cudaGetLastError();
+    return STREAMKL_ERR_CUDA;
+  }
+  skl::FwdParams p;
+  p.NQ = s.NQ; p.NK = s.NK; p.BH = int(s.BH);
+  p.H = s.H; p.G = s.G(); p.fmt16 = f16 ? 0u : 1u; p.act2 = s.act2;
+  p.TQ = (s.NQ + C::BQ - 1) / C::BQ;
+  p.sc1 = s.c1 * 1.4426950408889634f;
+  p.sc2 = s.c2 * 1.4426950408889634f;
+  p.kl = kl; p.lse1 = lse1; p.lse2 = lse2;
+  const int TK = (s.NK + C::BK - 1) / C::BK;
+  p.chunk_steps = SPLIT ? (TK + splits - 1) / splits : TK;       // C_K = ceil(N_K / W), in whole BK-key steps
+  p.W = SPLIT ? (TK + p.chunk_steps - 1) / p.chunk_steps : 1;    // no empty trailing chunk
+  p.part = part;
+  const long long grid = (long long)p.TQ * s.BH * p.W;
+  if (grid > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
+  {
+    ProfScope ps(SPLIT ? KID_FWD_SPLITK_TC : KID_FWD_TC, stream);
+    kern<<<dim3((unsigned)grid), C::THREADS, C::SMEM_BYTES, stream>>>(tQ1, tK1, tQ2, tK2, p);
+  }
+  if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
+  g_last_launches += 1;
+  if (SPLIT) {
+    const long long rows = s.BH * (long long)s.NQ;
+    {
+      ProfScope ps(KID_FWD_SPLITK_REDUCE, stream);
+      skl::streamkl_fwd_splitk_reduce_kernel<<<dim3((unsigned)((rows + 127) / 128)), 128, 0, stream>>>(part, s.NQ, p.W, rows, kl, lse1, lse2);
+    }
+    if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
+    g_last_launches += 1;
+  }
+  return STREAMKL_OK;
+}
+
+}  // namespace
+
+int fwd_tc_launch(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, float* kl, float* lse1, float* lse2,
+                  cudaStream_t stream, int splits, float* part) {
+  const int p1 = pad_dim(s.d1), p2 = pad_dim(s.d2);
+#define SKL_FWD_CASE(A, Bd)                                                                                                       \
+  if (p1 == A && p2 == Bd) {                                                                                                      \
+    if (splits > 1)                                                                                                               \
+      return s.causal ? launch_fwd_tc<A, Bd, true, true>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream, splits, part)            \
+                      : launch_fwd_tc<A, Bd, false, true>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream, splits, part);          \
+    return s.causal ? launch_fwd_tc<A, Bd, true>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream)                                  \
+                    : launch_fwd_tc<A, Bd, false>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream);                                \
+  }
+  SKL_FWD_CASE(128, 128)
+  SKL_FWD_CASE(128, 64)
+  SKL_FWD_CASE(64, 128)
+  SKL_FWD_CASE(64, 64)
+#undef SKL_FWD_CASE
+  return STREAMKL_ERR_SHAPE;
+}
+
+}  // namespace sklh

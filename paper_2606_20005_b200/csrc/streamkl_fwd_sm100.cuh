@@ -29,6 +29,8 @@
 #include <cuda_bf16.h>
 #include <math_constants.h>
 
+#include <type_traits>
+
 #include "sm100_ptx.cuh"
 
 // Which of the 16 column pairs a thread evaluates per step take their two exps on the FMA pipe (ex2_poly2) instead of
@@ -74,6 +76,7 @@ struct FwdParams {
   int BH;               // B * H query heads
   int H, G;             // query heads per batch; query heads per K head (GQA: query head h reads K head h / G)
   uint32_t fmt16;       // operand format of the logit MMAs: 1 bf16, 0 fp16
+  int act2;             // student activation: 0 none, 1 relu -- s2 = relu(c2 <q2,k2>) before its softmax (R23)
   float sc1, sc2;       // c_t * log2(e)
   float* kl;
   float* lse1;
@@ -111,12 +114,15 @@ __device__ __forceinline__ void wait_chunk(LogitChunk& c) {
 struct XChunk {
   float2 x1[4], x2[4];
 };
+// RELU2: the student's logit is relu(s2 sc2) (R23): relu(y) - m = max(y - m, -m).
+template <bool RELU2>
 __device__ __forceinline__ void scale_chunk(const LogitChunk& c, float sc1, float sc2, float nm1, float nm2, XChunk& x) {
   const float2 vsc1 = make_float2(sc1, sc1), vsc2 = make_float2(sc2, sc2), vn1 = make_float2(nm1, nm1), vn2 = make_float2(nm2, nm2);
 #pragma unroll
   for (int u = 0; u < 4; ++u) {
     x.x1[u] = fma2(make_float2(__uint_as_float(c.a[2 * u]), __uint_as_float(c.a[2 * u + 1])), vsc1, vn1);
     x.x2[u] = fma2(make_float2(__uint_as_float(c.b[2 * u]), __uint_as_float(c.b[2 * u + 1])), vsc2, vn2);
+    if (RELU2) x.x2[u] = make_float2(fmaxf(x.x2[u].x, nm2), fmaxf(x.x2[u].y, nm2));
   }
 }
 // Compiler-level ordering point (no instruction): everything that uses x stays below the statements above this call --
@@ -153,7 +159,7 @@ __device__ __forceinline__ void accumulate_chunk(const XChunk& x, float2& T1, fl
 // the logits from TMEM chunk by chunk, twice.  Used for masked steps (causal diagonal, key tails; MASKED) and to redo a
 // step whose sums showed a stale reference.  `kbase` = key index of the thread's first column, `limit` = last visible key.
 template <bool MASKED>
-__device__ __noinline__ RowState safe_step(uint32_t taddr, RowState st, float sc1, float sc2, int kbase, int limit) {
+__device__ __noinline__ RowState safe_step(uint32_t taddr, RowState st, float sc1, float sc2, int kbase, int limit, bool relu2) {
   float mx1 = -CUDART_INF_F, mx2 = -CUDART_INF_F;
 #pragma unroll 1
   for (int c = 0; c < 4; ++c) {
@@ -164,7 +170,7 @@ __device__ __noinline__ RowState safe_step(uint32_t taddr, RowState st, float sc
     for (int e = 0; e < 8; ++e) {
       const bool ok = !MASKED || (kbase + c * 8 + e) <= limit;
       mx1 = fmaxf(mx1, ok ? __uint_as_float(ch.a[e]) : -CUDART_INF_F);
-      mx2 = fmaxf(mx2, ok ? __uint_as_float(ch.b[e]) : -CUDART_INF_F);
+      mx2 = fmaxf(mx2, ok ? (relu2 ? fmaxf(__uint_as_float(ch.b[e]), 0.f) : __uint_as_float(ch.b[e])) : -CUDART_INF_F);
     }
   }
   const float m1n = fmaxf(st.m1, mx1 * sc1), m2n = fmaxf(st.m2, mx2 * sc2);   // sc > 0: max commutes with the scale
@@ -189,7 +195,7 @@ __device__ __noinline__ RowState safe_step(uint32_t taddr, RowState st, float sc
 #pragma unroll
     for (int e = 0; e < 8; ++e) {
       const float x1 = fmaf(__uint_as_float(ch.a[e]), sc1, -ref1);
-      const float x2 = fmaf(__uint_as_float(ch.b[e]), sc2, -ref2);
+      const float x2 = fmaf(relu2 ? fmaxf(__uint_as_float(ch.b[e]), 0.f) : __uint_as_float(ch.b[e]), sc2, -ref2);
       // R8: zero P~ at masked entries, take the difference from the raw (finite) logits
       const bool ok = !MASKED || (kbase + c * 8 + e) <= limit;
       const float p1 = ok ? ex2_approx(x1) : 0.f;
@@ -351,7 +357,10 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
       if (lane == 0) mbar_arrive(empty_bar);
     };
 
-    if (n_fast > 0) {
+    const bool relu2 = p.act2 == 1;
+    // the fast loop, instantiated with and without the student's ReLU (chosen once per kernel: nothing on the hot path)
+    auto run_fast = [&](auto relu_tag) {
+      constexpr bool RELU2 = decltype(relu_tag)::value;
       LogitChunk A;
       XChunk X;
       wait_full(0);
@@ -367,7 +376,7 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
           mx2 = max3(mx2, __uint_as_float(A.b[e]), __uint_as_float(A.b[(e + 1) & 7]));
         }
         st.m1 = mx1 * sc1;
-        st.m2 = mx2 * sc2;
+        st.m2 = RELU2 ? fmaxf(mx2 * sc2, 0.f) : mx2 * sc2;
       }
       float nm1 = -st.m1, nm2 = -st.m2;
       // One step on TMEM stage `tcur` (its first chunk already requested into A).  Per chunk: wait for the logits, turn
@@ -378,17 +387,17 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
                            const bool has_next) {
         float2 T1, T2, TD;
         wait_chunk(A);
-        scale_chunk(A, sc1, sc2, nm1, nm2, X);
+        scale_chunk<RELU2>(A, sc1, sc2, nm1, nm2, X);
         ld_chunk(tcur + 8, A);
         pin_below(X);
         accumulate_chunk<(C::POLY_MASK >> 0) & 15u, true>(X, T1, T2, TD);
         wait_chunk(A);
-        scale_chunk(A, sc1, sc2, nm1, nm2, X);
+        scale_chunk<RELU2>(A, sc1, sc2, nm1, nm2, X);
         ld_chunk(tcur + 16, A);
         pin_below(X);
         accumulate_chunk<(C::POLY_MASK >> 4) & 15u, false>(X, T1, T2, TD);
         wait_chunk(A);
-        scale_chunk(A, sc1, sc2, nm1, nm2, X);
+        scale_chunk<RELU2>(A, sc1, sc2, nm1, nm2, X);
         ld_chunk(tcur + 24, A);
         // the next step's logits have normally been in TMEM for a long time: probe its barrier now, use the answer after
         // this chunk's arithmetic (the probe's latency is then hidden)
@@ -396,7 +405,7 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
         pin_below(X);
         accumulate_chunk<(C::POLY_MASK >> 8) & 15u, false>(X, T1, T2, TD);
         wait_chunk(A);
-        scale_chunk(A, sc1, sc2, nm1, nm2, X);
+        scale_chunk<RELU2>(A, sc1, sc2, nm1, nm2, X);
         if (has_next) {
           if (!ready) mbar_wait(full_next, par_next);
           tc_fence_after();
@@ -412,7 +421,7 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
           st.R2 = add2(st.R2, T2);
           st.RD = add2(st.RD, TD);
         } else {
-          st = safe_step<false>(tcur, st, sc1, sc2, 0, 0);
+          st = safe_step<false>(tcur, st, sc1, sc2, 0, 0, RELU2);
           nm1 = -st.m1;
           nm2 = -st.m2;
         }
@@ -430,10 +439,13 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
       }
       if (j < n_fast) fast_step(t0, t1, &s_full[1], par, &s_empty[0], j + 1 < nsteps);
       wait_chunk(A);   // a chunk requested for a masked step is read again by safe_step; nothing may stay in flight
+    };
+    if (n_fast > 0) {
+      if (relu2) run_fast(std::true_type{}); else run_fast(std::false_type{});
     }
     for (int j = n_fast; j < nsteps; ++j) {
       wait_full(j);
-      st = safe_step<true>(tbase + (j & 1) * (2 * C::BK), st, sc1, sc2, (j_begin + j) * C::BK + grp * C::BC, limit);
+      st = safe_step<true>(tbase + (j & 1) * (2 * C::BK), st, sc1, sc2, (j_begin + j) * C::BK + grp * C::BC, limit, relu2);
       release(&s_empty[j & 1]);
     }
 

@@ -16,13 +16,13 @@ from parity_util import check_fwd, check_grad_heads, to_f64, to_torch
 pytestmark = pytest.mark.gpu
 
 
-def _ref(cfg, inp, HK, teacher, g):
+def _ref(cfg, inp, HK, teacher, g, act2=None):
     """float64 definition with K heads expanded to the query heads; dK folded back onto the HK shared heads."""
     G = cfg.H // HK
     f = {k: W.widen_f64(inp[k]) for k in ("Q1", "K1", "Q2", "K2")}
     K1 = np.repeat(f["K1"], G, axis=1)
     K2 = np.repeat(f["K2"], G, axis=1)
-    ref = attention_kl(f["Q1"], K1, f["Q2"], K2, cfg.c1, cfg.c2, cfg.causal, g=g.astype(np.float64), teacher=teacher)
+    ref = attention_kl(f["Q1"], K1, f["Q2"], K2, cfg.c1, cfg.c2, cfg.causal, g=g.astype(np.float64), teacher=teacher, act2=act2)
     for name in ("dK1", "dK2"):
         if name in ref:
             a = ref[name]
@@ -43,7 +43,7 @@ def _as_bnhd(t):
     return t.permute(0, 2, 1, 3).contiguous().permute(0, 2, 1, 3)
 
 
-def _run(cfg, HK=None, teacher=True, view=None, both_modes=True):
+def _run(cfg, HK=None, teacher=True, view=None, both_modes=True, act2=None):
     import torch
 
     import paper_2606_20005_b200 as skl
@@ -51,18 +51,19 @@ def _run(cfg, HK=None, teacher=True, view=None, both_modes=True):
     HK = cfg.H if HK is None else HK
     inp = _inputs(cfg, HK)
     g_np = inp["g"]
-    ref = _ref(cfg, inp, HK, teacher, g_np)
+    ref = _ref(cfg, inp, HK, teacher, g_np, act2)
     dev = {k: to_torch(inp[k]) for k in ("Q1", "K1", "Q2", "K2")}
     if view is not None:
         dev = {k: view(v) for k, v in dev.items()}
     g = to_torch(g_np)
-    kl, l1, l2 = skl.streamkl_fwd(dev["Q1"], dev["K1"], dev["Q2"], dev["K2"], cfg.c1, cfg.c2, cfg.causal)
+    kl, l1, l2 = skl.streamkl_fwd(dev["Q1"], dev["K1"], dev["Q2"], dev["K2"], cfg.c1, cfg.c2, cfg.causal, student_activation=act2)
     check_fwd(to_f64(kl), to_f64(l1), to_f64(l2), ref, cfg.name + " fwd")
     modes = [skl.STREAMKL_BWD_AUTO] + ([skl.STREAMKL_BWD_SEPARATE, skl.STREAMKL_BWD_FUSED] if both_modes else [])
     try:
         for mode in modes:
             skl.streamkl_set_bwd_mode(mode)
-            grads = skl.streamkl_bwd(dev["Q1"], dev["K1"], dev["Q2"], dev["K2"], cfg.c1, cfg.c2, cfg.causal, kl, l1, l2, g, teacher=teacher)
+            grads = skl.streamkl_bwd(dev["Q1"], dev["K1"], dev["Q2"], dev["K2"], cfg.c1, cfg.c2, cfg.causal, kl, l1, l2, g, teacher=teacher,
+                                     student_activation=act2)
             for name, t, src in zip(("dQ1", "dK1", "dQ2", "dK2"), grads, (dev["Q1"], dev["K1"], dev["Q2"], dev["K2"])):
                 if t is None:
                     assert not teacher and name in ("dQ1", "dK1")
@@ -194,3 +195,45 @@ def test_layout_errors_are_reported_not_launched():
     assert L.streamkl_fwd_ex(ctypes.cast(ctypes.pointer(lay), vp), *args) == -2
     lay.dtype = 9
     assert L.streamkl_fwd_ex(ctypes.cast(ctypes.pointer(lay), vp), *args) == -7
+
+
+# ---------------------------------------------------------------- NEXT-4: student ReLU activation (R23)
+@pytest.mark.parametrize("causal", [False, True])
+@pytest.mark.parametrize("d1,d2,dtype", [(128, 64, "bf16"), (128, 128, "bf16"), (64, 64, "f16")])
+def test_relu_student(d1, d2, dtype, causal):
+    """s2 = relu(c2 <q2,k2>) before the student's softmax: kl / lse2 of that P2, dS2 gated by relu'; every strategy, both settings."""
+    _run(W.Config(91, "relu", 1, 3, 457, 901, d1, d2, dtype, causal), act2="relu")
+    _run(W.Config(92, "relu-long", 1, 2, 1300, 1300, d1, d2, dtype, causal), act2="relu", both_modes=False)
+
+
+def test_relu_student_with_strides_shared_heads_and_odd_dims():
+    _run(W.Config(93, "relu-all", 2, 4, 260, 777, 96, 40, "bf16", True), HK=2, view=_as_bnhd, act2="relu")
+
+
+def test_relu_student_closed_form_all_logits_negative():
+    """Every raw student logit < 0 (Q2 > 0, K2 < 0 elementwise): relu makes P2 uniform -- lse2 = log nV exactly, KL = log nV - H(P1),
+    and the student's gradients vanish identically (the gate is 0 everywhere), while the teacher's do not."""
+    import torch
+
+    import paper_2606_20005_b200 as skl
+
+    cfg = W.Config(94, "relu-neg", 1, 2, 300, 600, 128, 64, "bf16", True)
+    inp = W.all_inputs(cfg)
+    Q1, K1 = to_torch(inp["Q1"]), to_torch(inp["K1"])
+    Q2, K2 = to_torch(inp["Q2"]).abs(), -to_torch(inp["K2"]).abs()
+    g = to_torch(inp["g"])
+    kl, l1, l2 = skl.streamkl_fwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, True, student_activation="relu")
+    nV = np.arange(cfg.NQ) + (cfg.NK - cfg.NQ) + 1
+    assert np.abs(to_f64(l2)[0, 0] - np.log(nV)).max() <= 1e-4
+    f = {"Q1": W.widen_f64(inp["Q1"]), "K1": W.widen_f64(inp["K1"]), "Q2": to_f64(Q2), "K2": to_f64(K2)}
+    ref = attention_kl(f["Q1"], f["K1"], f["Q2"], f["K2"], cfg.c1, cfg.c2, True, g=inp["g"].astype(np.float64), teacher=True, act2="relu")
+    check_fwd(to_f64(kl), to_f64(l1), to_f64(l2), ref, "relu-neg fwd")
+    for mode in (skl.STREAMKL_BWD_FUSED, skl.STREAMKL_BWD_SEPARATE):
+        skl.streamkl_set_bwd_mode(mode)
+        try:
+            dQ1, dK1, dQ2, dK2 = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, True, kl, l1, l2, g, teacher=True, student_activation="relu")
+        finally:
+            skl.streamkl_set_bwd_mode(skl.STREAMKL_BWD_AUTO)
+        assert float(dQ2.float().abs().max()) == 0.0 and float(dK2.float().abs().max()) == 0.0
+        check_grad_heads(to_f64(dQ1), ref["dQ1"], f"mode {mode} dQ1")
+        check_grad_heads(to_f64(dK1), ref["dK1"], f"mode {mode} dK1")
