@@ -115,14 +115,23 @@ struct XChunk {
   float2 x1[4], x2[4];
 };
 // RELU2: the student's logit is relu(s2 sc2) (R23): relu(y) - m = max(y - m, -m).
-template <bool RELU2>
-__device__ __forceinline__ void scale_chunk(const LogitChunk& c, float sc1, float sc2, float nm1, float nm2, XChunk& x) {
+// MASKED (causal diagonal tiles, key tails): a key beyond `limit` gets x1 = x2 = kMaskedX, so that both of its P~ are exactly 0
+// (ex2.approx.ftz of a hugely negative argument) and its S1 - S2 term is 0 - 0: R8 without ever forming a difference of
+// infinities.  `k0` = key index of the chunk's first column.
+constexpr float kMaskedX = -1.0e30f;
+template <bool RELU2, bool MASKED>
+__device__ __forceinline__ void scale_chunk(const LogitChunk& c, float sc1, float sc2, float nm1, float nm2, XChunk& x, int k0, int limit) {
   const float2 vsc1 = make_float2(sc1, sc1), vsc2 = make_float2(sc2, sc2), vn1 = make_float2(nm1, nm1), vn2 = make_float2(nm2, nm2);
 #pragma unroll
   for (int u = 0; u < 4; ++u) {
     x.x1[u] = fma2(make_float2(__uint_as_float(c.a[2 * u]), __uint_as_float(c.a[2 * u + 1])), vsc1, vn1);
     x.x2[u] = fma2(make_float2(__uint_as_float(c.b[2 * u]), __uint_as_float(c.b[2 * u + 1])), vsc2, vn2);
     if (RELU2) x.x2[u] = make_float2(fmaxf(x.x2[u].x, nm2), fmaxf(x.x2[u].y, nm2));
+    if (MASKED) {
+      const bool ok0 = k0 + 2 * u <= limit, ok1 = k0 + 2 * u + 1 <= limit;
+      x.x1[u] = make_float2(ok0 ? x.x1[u].x : kMaskedX, ok1 ? x.x1[u].y : kMaskedX);
+      x.x2[u] = make_float2(ok0 ? x.x2[u].x : kMaskedX, ok1 ? x.x2[u].y : kMaskedX);
+    }
   }
 }
 // Compiler-level ordering point (no instruction): everything that uses x stays below the statements above this call --
@@ -383,36 +392,40 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
       // them into exponents (the only read of A), request the next chunk into A, then evaluate.  All addresses are stage
       // constants: the loop below is unrolled over the two stages.  `has_next`: another step follows (fast or masked) --
       // its first chunk is requested, after its s_full, before this step's last chunk is evaluated.
-      auto fast_step = [&](const uint32_t tcur, const uint32_t tnext, uint64_t* full_next, const uint32_t par_next, uint64_t* empty_cur,
-                           const bool has_next) {
+      // `masked_tag`: a step on the causal diagonal or the key tail (`k0` = key index of the thread's first column): the same
+      // pipeline with the out-of-range keys neutralised in scale_chunk and every exp on MUFU (exact zeros).
+      auto fast_step = [&](auto masked_tag, const uint32_t tcur, const uint32_t tnext, uint64_t* full_next, const uint32_t par_next,
+                           uint64_t* empty_cur, const bool has_next, const int k0) {
+        constexpr bool MASKED = decltype(masked_tag)::value;
+        constexpr uint32_t PMASK = MASKED ? 0u : C::POLY_MASK;
         float2 T1, T2, TD;
         wait_chunk(A);
-        scale_chunk<RELU2>(A, sc1, sc2, nm1, nm2, X);
+        scale_chunk<RELU2, MASKED>(A, sc1, sc2, nm1, nm2, X, k0, limit);
         ld_chunk(tcur + 8, A);
         pin_below(X);
-        accumulate_chunk<(C::POLY_MASK >> 0) & 15u, true>(X, T1, T2, TD);
+        accumulate_chunk<(PMASK >> 0) & 15u, true>(X, T1, T2, TD);
         wait_chunk(A);
-        scale_chunk<RELU2>(A, sc1, sc2, nm1, nm2, X);
+        scale_chunk<RELU2, MASKED>(A, sc1, sc2, nm1, nm2, X, k0 + 8, limit);
         ld_chunk(tcur + 16, A);
         pin_below(X);
-        accumulate_chunk<(C::POLY_MASK >> 4) & 15u, false>(X, T1, T2, TD);
+        accumulate_chunk<(PMASK >> 4) & 15u, false>(X, T1, T2, TD);
         wait_chunk(A);
-        scale_chunk<RELU2>(A, sc1, sc2, nm1, nm2, X);
+        scale_chunk<RELU2, MASKED>(A, sc1, sc2, nm1, nm2, X, k0 + 16, limit);
         ld_chunk(tcur + 24, A);
         // the next step's logits have normally been in TMEM for a long time: probe its barrier now, use the answer after
         // this chunk's arithmetic (the probe's latency is then hidden)
         const bool ready = has_next && mbar_test_wait(full_next, par_next);
         pin_below(X);
-        accumulate_chunk<(C::POLY_MASK >> 8) & 15u, false>(X, T1, T2, TD);
+        accumulate_chunk<(PMASK >> 8) & 15u, false>(X, T1, T2, TD);
         wait_chunk(A);
-        scale_chunk<RELU2>(A, sc1, sc2, nm1, nm2, X);
+        scale_chunk<RELU2, MASKED>(A, sc1, sc2, nm1, nm2, X, k0 + 24, limit);
         if (has_next) {
           if (!ready) mbar_wait(full_next, par_next);
           tc_fence_after();
           ld_chunk(tnext, A);
         }
         pin_below(X);
-        accumulate_chunk<(C::POLY_MASK >> 12) & 15u, false>(X, T1, T2, TD);
+        accumulate_chunk<(PMASK >> 12) & 15u, false>(X, T1, T2, TD);
         const float chk = (T1.x + T1.y) + (T2.x + T2.y);
         // warp-uniform decision: safe_step issues tcgen05.ld (.sync.aligned: the whole warp must execute it together);
         // a row that did not need the redo loses nothing by taking it
@@ -421,7 +434,7 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
           st.R2 = add2(st.R2, T2);
           st.RD = add2(st.RD, TD);
         } else {
-          st = safe_step<false>(tcur, st, sc1, sc2, 0, 0, RELU2);
+          st = MASKED ? safe_step<true>(tcur, st, sc1, sc2, k0, limit, RELU2) : safe_step<false>(tcur, st, sc1, sc2, 0, 0, RELU2);
           nm1 = -st.m1;
           nm2 = -st.m2;
         }
@@ -433,20 +446,27 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
       for (; j + 2 <= n_fast; j += 2) {
         // (`has_next` is always true here, but it is kept a run-time value: the prefetch then sits in a basic block of its
         // own, ahead of the last chunk's arithmetic, instead of being sunk to the end of the step by the scheduler)
-        fast_step(t0, t1, &s_full[1], par, &s_empty[0], j + 1 < nsteps);
-        fast_step(t1, t0, &s_full[0], par ^ 1, &s_empty[1], j + 2 < nsteps);
+        fast_step(std::false_type{}, t0, t1, &s_full[1], par, &s_empty[0], j + 1 < nsteps, 0);
+        fast_step(std::false_type{}, t1, t0, &s_full[0], par ^ 1, &s_empty[1], j + 2 < nsteps, 0);
         par ^= 1;
       }
-      if (j < n_fast) fast_step(t0, t1, &s_full[1], par, &s_empty[0], j + 1 < nsteps);
-      wait_chunk(A);   // a chunk requested for a masked step is read again by safe_step; nothing may stay in flight
+      // what is left -- an odd unmasked step, then the masked steps (the row already has a reference) -- one step at a time
+      for (; j < nsteps; ++j) {
+        const uint32_t tc = (j & 1) ? t1 : t0, tn = (j & 1) ? t0 : t1;
+        uint64_t* fn = &s_full[(j + 1) & 1];
+        const uint32_t pn = uint32_t((j + 1) >> 1) & 1u;
+        if (j < n_fast) fast_step(std::false_type{}, tc, tn, fn, pn, &s_empty[j & 1], j + 1 < nsteps, 0);
+        else            fast_step(std::true_type{}, tc, tn, fn, pn, &s_empty[j & 1], j + 1 < nsteps, (j_begin + j) * C::BK + grp * C::BC);
+      }
     };
-    if (n_fast > 0) {
+    if (n_fast > 0) {   // (the group sees at least one whole unmasked step: every row has a finite reference before any masked step)
       if (relu2) run_fast(std::true_type{}); else run_fast(std::false_type{});
-    }
-    for (int j = n_fast; j < nsteps; ++j) {
-      wait_full(j);
-      st = safe_step<true>(tbase + (j & 1) * (2 * C::BK), st, sc1, sc2, (j_begin + j) * C::BK + grp * C::BC, limit, relu2);
-      release(&s_empty[j & 1]);
+    } else {
+      for (int j = 0; j < nsteps; ++j) {   // first Q tile of a causal head, NK < 128, ...: Alg.1 literally
+        wait_full(j);
+        st = safe_step<true>(tbase + (j & 1) * (2 * C::BK), st, sc1, sc2, (j_begin + j) * C::BK + grp * C::BC, limit, relu2);
+        release(&s_empty[j & 1]);
+      }
     }
 
     // this thread's partial statistics in Alg.1's form (log2 domain): l_t = R_t, acc = RD + (m1 - m2) R1
