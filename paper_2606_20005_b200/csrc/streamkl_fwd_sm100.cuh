@@ -35,12 +35,15 @@
 
 // Which of the 16 column pairs a thread evaluates per step take their two exps on the FMA pipe (ex2_poly2) instead of
 // MUFU: one 4-bit mask per chunk (bit u = column pair u of the chunk), chunks 0..3 in nibbles 0..3.  The forward is
-// MUFU-bound 2:1 (d2 = 128) to 2.7:1 (d2 = 64) against the tensor pipe; measured per head-dim pair.
+// MUFU-bound 2:1 (d1 + d2 = 256) to 2.7:1 (192) against the tensor pipe, but it also runs into the 1000 W cap, and a
+// polynomial exp costs six times the instructions of a MUFU one.  Measured in a sustained loop on B200:
+// d = 128/128: 2/16 10.23 ms, 3/16 9.97, 4/16 10.08, 5/16 10.37 (cfg4 with 8 heads); d = 128/64: 3/16 2.355 ms, 4/16 2.343,
+// 5/16 2.42, 6/16 2.47 (cfg3).
 #ifndef STREAMKL_FWD_POLY_MASK_WIDE
-#define STREAMKL_FWD_POLY_MASK_WIDE 0x1111u   // d1 + d2 = 256: a quarter of the exps
+#define STREAMKL_FWD_POLY_MASK_WIDE 0x1011u   // d1 + d2 = 256: three column pairs in sixteen
 #endif
 #ifndef STREAMKL_FWD_POLY_MASK_NARROW
-#define STREAMKL_FWD_POLY_MASK_NARROW 0x1111u // d1 + d2 < 256: less tensor work per step, the exps bind harder
+#define STREAMKL_FWD_POLY_MASK_NARROW 0x1111u // d1 + d2 < 256: a quarter of the exps
 #endif
 
 namespace skl {
