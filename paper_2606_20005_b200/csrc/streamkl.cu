@@ -79,16 +79,41 @@ bool device_is_sm100() {
 
 // 4-D map {d, N, heads, B} of a 16-bit tensor with arbitrary (batch, head, row) strides; box = {64 elements (128 B), box_rows, 1, 1},
 // 128-byte swizzle, zero OOB fill: rows beyond N and columns beyond d (head dims that are not 64 / 128) arrive as zeros.
+// Encoding a tensor map is a driver call of a microsecond or two, and a backward launches three kernels with four maps each:
+// the last few encodings are kept per host thread (a decode-sized split-K forward is ~40 us of GPU time).
+struct TmapKey {
+  const void* base; int B, heads, N, d, box_rows, f16; long long sb, sh, sn;
+  bool operator==(const TmapKey& o) const {
+    return base == o.base && B == o.B && heads == o.heads && N == o.N && d == o.d && box_rows == o.box_rows && f16 == o.f16 && sb == o.sb &&
+           sh == o.sh && sn == o.sn;
+  }
+};
+struct TmapCache {
+  static constexpr int N = 16;
+  TmapKey key[N];
+  CUtensorMap map[N];
+  int used = 0, next = 0;
+};
+thread_local TmapCache g_tmaps;
+
 bool make_tmap_16(CUtensorMap* m, const void* base, int B, int heads, int N, int d, const Strides& st, int box_rows, bool f16) {
+  const TmapKey k{base, B, heads, N, d, box_rows, f16 ? 1 : 0, st.b, st.h, st.n};
+  for (int i = 0; i < g_tmaps.used; ++i)
+    if (g_tmaps.key[i] == k) { *m = g_tmaps.map[i]; return true; }
   EncodeTiledFn enc = get_encode_fn();
   if (!enc) return false;
   cuuint64_t dims[4] = {cuuint64_t(d), cuuint64_t(N), cuuint64_t(heads), cuuint64_t(B)};
   cuuint64_t strides[3] = {cuuint64_t(st.n) * 2, cuuint64_t(st.h) * 2, cuuint64_t(st.b) * 2};
   cuuint32_t box[4] = {64, cuuint32_t(box_rows), 1, 1};
   cuuint32_t estr[4] = {1, 1, 1, 1};
-  return enc(m, f16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(base), dims, strides, box,
-             estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+  if (enc(m, f16 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT16 : CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(base), dims, strides, box,
+          estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+    return false;
+  const int slot = g_tmaps.used < TmapCache::N ? g_tmaps.used++ : (g_tmaps.next = (g_tmaps.next + 1) % TmapCache::N);
+  g_tmaps.key[slot] = k;
+  g_tmaps.map[slot] = *m;
+  return true;
 }
 
 Strides contiguous(int heads, int N, int d) { return Strides{(long long)heads * N * d, (long long)N * d, (long long)d}; }
@@ -365,6 +390,12 @@ struct HostStreams {
          cudaStreamCreateWithFlags(&out, cudaStreamNonBlocking) == cudaSuccess &&
          cudaStreamCreateWithFlags(&cmp, cudaStreamNonBlocking) == cudaSuccess;
     if (!ok) cudaGetLastError();
+  }
+  ~HostStreams() {   // the owning host thread ends: give the helper streams back (ignore errors at process teardown)
+    if (in) cudaStreamDestroy(in);
+    if (out) cudaStreamDestroy(out);
+    if (cmp) cudaStreamDestroy(cmp);
+    cudaGetLastError();
   }
 };
 HostStreams& host_streams() {
