@@ -165,11 +165,11 @@ int validate_common(const void* Q1, const void* K1, const void* Q2, const void* 
   return STREAMKL_OK;
 }
 
-// tensor-core path: 16-bit inputs, head dims that are multiples of 8 (TMA: 16-byte rows) up to 128.  The kernels are
-// instantiated for head dims 64 and 128; anything else runs zero-padded to the next of the two (pad_dim).
-bool tc_shape(int dtype, const Shape& s) {
-  return (dtype == STREAMKL_BF16 || dtype == STREAMKL_F16) && s.d1 % 8 == 0 && s.d2 % 8 == 0 && s.d1 <= 128 && s.d2 <= 128;
-}
+// tensor-core path: 16-bit inputs, head dims that are multiples of 8 (TMA: 16-byte rows) up to 256.  The kernels work on
+// head dims zero-padded to the next multiple of 64 (pad_dim): fixed plans for {64,128}^2, run-time K-block counts when a
+// head dim exceeds 128 (wide_dims).
+bool tc_dims(int d1, int d2) { return d1 % 8 == 0 && d2 % 8 == 0 && d1 >= 8 && d2 >= 8 && d1 <= kMaxTcDim && d2 <= kMaxTcDim; }
+bool tc_shape(int dtype, const Shape& s) { return (dtype == STREAMKL_BF16 || dtype == STREAMKL_F16) && tc_dims(s.d1, s.d2); }
 
 }  // namespace
 
@@ -192,7 +192,8 @@ const char* const kKernelNames[KID_COUNT] = {"streamkl_fwd_sm100_kernel", "strea
                                              "streamkl_bwd_simt_kernel<OWNER_Q>", "streamkl_bwd_simt_kernel<OWNER_K>",
                                              "streamkl_bwd_stats_kernel", "streamkl_fwd_sm100_kernel<SPLIT>",
                                              "streamkl_fwd_splitk_reduce_kernel", "streamkl_bwd_fused_sm100_kernel",
-                                             "streamkl_bwd_dq_convert_kernel"};
+                                             "streamkl_bwd_dq_convert_kernel", "streamkl_bwd_wide_sm100_kernel<OWNER_Q>",
+                                             "streamkl_bwd_wide_sm100_kernel<OWNER_K>"};
 // ----------------------------------------------------------------------------------------- forward (SIMT fallback, dispatch)
 int simt_block_rows(size_t floats_per_row, size_t fixed_floats, size_t* smem_bytes) {
   for (int br : {128, 64, 32}) {
@@ -275,7 +276,8 @@ int launch_bwd_simt(const void* Q1, const void* K1, const void* Q2, const void* 
 // Setting 1 (one pass: half the recomputation), at most two for Setting 2 (two passes: same work as the owner kernels, the
 // gain is the fuller K-owner grid).  streamkl_bwd_workspace_bytes applies the same rule, so the fp32 dQ accumulators are
 // only asked for when the strategy that will run needs them.
-bool bwd_fused_selected(int NQ, bool teacher) {
+bool bwd_fused_selected(int NQ, bool teacher, int d1, int d2) {
+  if (wide_dims(d1, d2)) return false;   // head dims above 128: owner kernels only (TMEM has no room for the dQ^T stages)
   return g_bwd_mode == STREAMKL_BWD_FUSED || (g_bwd_mode == STREAMKL_BWD_AUTO && (NQ + 127) / 128 <= (teacher ? 2 : 4));
 }
 size_t fused_acc_bytes_aligned(long long BH, int NQ, int d) { return (size_t(BH) * size_t(NQ) * size_t(d) * sizeof(float) + 255) & ~size_t(255); }
@@ -293,13 +295,18 @@ int bwd_tc_both(const void* Q1, const void* K1, const void* Q2, const void* K2, 
   // 1.3-3.0x up to T_Q = 4 tiles of 128 queries, level at 8; Setting 2: 1.3-1.5x up to T_Q = 2, 0.8x at 4) and lose beyond,
   // where their fp32 atomics (64 KB per 128x128 tile pair and pass) run into the L2's atomic throughput; the crossover did
   // not move with T_K (128 vs 1024), so the rule is on T_Q alone.
-  if (bwd_fused_selected(s.NQ, t)) {   // one visit per differentiated distribution, dQ through fp32 atomics
+  if (bwd_fused_selected(s.NQ, t, s.d1, s.d2)) {   // one visit per differentiated distribution, dQ through fp32 atomics
     uint8_t* w = static_cast<uint8_t*>(workspace) + stats_bytes_aligned(s.BH, s.NQ);
     float* acc2 = reinterpret_cast<float*>(w);
     float* acc1 = reinterpret_cast<float*>(w + fused_acc_bytes_aligned(s.BH, s.NQ, pad_dim(s.d2)));
     rc = bwd_tc_fused_launch(Q1, K1, Q2, K2, s, f16, false, workspace, acc2, dQ2, dK2, st);
     if (rc != STREAMKL_OK || !t) return rc;
     return bwd_tc_fused_launch(Q1, K1, Q2, K2, s, f16, true, workspace, acc1, dQ1, dK1, st);
+  }
+  if (wide_dims(s.d1, s.d2)) {
+    rc = bwd_wide_owner_q_launch(Q1, K1, Q2, K2, s, f16, workspace, dQ1, dQ2, st);
+    if (rc != STREAMKL_OK) return rc;
+    return bwd_wide_owner_k_launch(Q1, K1, Q2, K2, s, f16, workspace, dK1, dK2, st);
   }
   rc = bwd_tc_owner_q_launch(Q1, K1, Q2, K2, s, f16, workspace, dQ1, dQ2, st);
   if (rc != STREAMKL_OK) return rc;
@@ -466,7 +473,7 @@ int streamkl_fwd_splitk(const void* Q1, const void* K1, const void* Q2, const vo
   if (splits <= 0) splits = streamkl_fwd_splitk_splits(B, H, NQ, NK, 0);
   const int tk = NK > 0 ? (NK + kFwdBK - 1) / kFwdBK : 1;
   if (splits > tk) splits = tk;
-  const bool tc = d1 % 8 == 0 && d2 % 8 == 0 && d1 >= 8 && d2 >= 8 && d1 <= 128 && d2 <= 128;
+  const bool tc = tc_dims(d1, d2);
   if (!tc || splits <= 1)   // other head dims run the (unsplit) SIMT kernel; W = 1 is the default kernel
     return fwd_dispatch(STREAMKL_BF16, nullptr, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
                         static_cast<cudaStream_t>(stream));
@@ -481,9 +488,9 @@ size_t streamkl_bwd_workspace_bytes(int B, int H, int NQ, int, int d1, int d2, i
   // both gradients are produced by tile ownership: no fp32 accumulation workspace.  The tcgen05 kernels read the
   // per-query scalars (lse1, lse2, dkl, kl) from a packed copy: 16 B per query, rows padded to 64 per head -- O(NQ).
   if (B <= 0 || H <= 0 || NQ <= 0) return 0;
-  if (!(d1 % 8 == 0 && d2 % 8 == 0 && d1 >= 8 && d2 >= 8 && d1 <= 128 && d2 <= 128)) return 0;   // SIMT path: no workspace
+  if (!tc_dims(d1, d2)) return 0;   // SIMT path: no workspace
   const long long BH = (long long)B * H;
-  if (!bwd_fused_selected(NQ, want_teacher != 0)) return size_t(BH) * size_t(stats_padded_rows(NQ)) * 16;
+  if (!bwd_fused_selected(NQ, want_teacher != 0, d1, d2)) return size_t(BH) * size_t(stats_padded_rows(NQ)) * 16;
   // one-visit kernels (mode FUSED, or AUTO with NQ <= 512): + their fp32 dQ accumulators, O(NQ d)
   return stats_bytes_aligned(BH, NQ) + fused_acc_bytes_aligned(BH, NQ, pad_dim(d2)) + (want_teacher ? fused_acc_bytes_aligned(BH, NQ, pad_dim(d1)) : 0);
 }

@@ -9,6 +9,7 @@ static_assert(skl::FwdCfg<128, 128>::BQ == kFwdBQ && skl::FwdCfg<64, 64>::BK == 
 
 // splits == 1: the default kernel (grid (bsz, T_Q)).  splits > 1: split-K (grid (bsz, T_Q, W), partial
 // statistics to `part`, then the reduce kernel).
+// D1 = D2 = 0: the BLOCKED plan with run-time K-block counts (a head dim above 128, padded to 192 / 256).
 template <int D1, int D2, bool CAUSAL, bool SPLIT = false>
 int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, float* kl, float* lse1,
                   float* lse2, cudaStream_t stream, int splits = 1, float* part = nullptr) {
@@ -17,11 +18,20 @@ int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2
   if (!make_maps(tm, Q1, K1, Q2, K2, s, C::BM, C::BK, f16)) return STREAMKL_ERR_CUDA;
   const CUtensorMap &tQ1 = tm[0], &tK1 = tm[1], &tQ2 = tm[2], &tK2 = tm[3];
   auto kern = skl::streamkl_fwd_sm100_kernel<D1, D2, CAUSAL, SPLIT>;
-  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
+  skl::FwdParams p;
+  p.kb1 = pad_dim(s.d1) / 64; p.kb2 = pad_dim(s.d2) / 64; p.nring = 0;
+  int smem_bytes = 0;
+  if constexpr (C::BLOCKED) {
+    p.nring = C::ring_blocks(p.kb1, p.kb2);
+    if (p.nring < 2) return STREAMKL_ERR_SHAPE;
+    smem_bytes = C::smem_bytes(p.kb1, p.kb2);
+  } else {
+    smem_bytes = C::SMEM_BYTES;
+  }
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes) != cudaSuccess) {
     cudaGetLastError();
     return STREAMKL_ERR_CUDA;
   }
-  skl::FwdParams p;
   p.NQ = s.NQ; p.NK = s.NK; p.BH = int(s.BH);
   p.H = s.H; p.G = s.G(); p.fmt16 = f16 ? 0u : 1u; p.act2 = s.act2;
   p.TQ = (s.NQ + C::BQ - 1) / C::BQ;
@@ -36,7 +46,7 @@ int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2
   if (grid > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
   {
     ProfScope ps(SPLIT ? KID_FWD_SPLITK_TC : KID_FWD_TC, stream);
-    kern<<<dim3((unsigned)grid), C::THREADS, C::SMEM_BYTES, stream>>>(tQ1, tK1, tQ2, tK2, p);
+    kern<<<dim3((unsigned)grid), C::THREADS, smem_bytes, stream>>>(tQ1, tK1, tQ2, tK2, p);
   }
   if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
   g_last_launches += 1;
@@ -56,7 +66,8 @@ int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2
 
 int fwd_tc_launch(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, float* kl, float* lse1, float* lse2,
                   cudaStream_t stream, int splits, float* part) {
-  const int p1 = pad_dim(s.d1), p2 = pad_dim(s.d2);
+  int p1 = pad_dim(s.d1), p2 = pad_dim(s.d2);
+  if (p1 > 128 || p2 > 128) p1 = p2 = 0;   // a wide head dim: the BLOCKED plan (run-time K-block counts)
 #define SKL_FWD_CASE(A, Bd)                                                                                                       \
   if (p1 == A && p2 == Bd) {                                                                                                      \
     if (splits > 1)                                                                                                               \
@@ -69,6 +80,7 @@ int fwd_tc_launch(const void* Q1, const void* K1, const void* Q2, const void* K2
   SKL_FWD_CASE(128, 64)
   SKL_FWD_CASE(64, 128)
   SKL_FWD_CASE(64, 64)
+  SKL_FWD_CASE(0, 0)
 #undef SKL_FWD_CASE
   return STREAMKL_ERR_SHAPE;
 }

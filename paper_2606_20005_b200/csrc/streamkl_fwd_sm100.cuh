@@ -50,7 +50,8 @@ namespace skl {
 
 template <int D1, int D2>
 struct FwdCfg {
-  static_assert(D1 % 64 == 0 && D2 % 64 == 0 && D1 <= 128 && D2 <= 128, "tcgen05 path: d in {64,128}");
+  static_assert(D1 % 64 == 0 && D2 % 64 == 0 && D1 >= 64 && D2 >= 64 && D1 <= 128 && D2 <= 128, "fixed plans: d in {64,128}");
+  static constexpr bool BLOCKED = false;     // whole {K1_j, K2_j} stages in the ring (FwdCfg<0,0>: single K-blocks)
   static constexpr int BM = 128;             // rows per Q tile (TMEM lanes)
   static constexpr int BK = 128;             // keys per step = N of the logit MMAs
   static constexpr int BQ = BM;              // query rows per CTA
@@ -74,8 +75,35 @@ struct FwdCfg {
   static constexpr uint32_t POLY_MASK = (D1 + D2 == 256) ? STREAMKL_FWD_POLY_MASK_WIDE : STREAMKL_FWD_POLY_MASK_NARROW;
 };
 
+// Head dims beyond 128 (padded to 192 / 256): Q alone is up to 128 KB, so a whole 128-key stage of K1,K2 no longer fits beside
+// it.  FwdCfg<0, 0> is the BLOCKED plan: the numbers of 64-element K-blocks per row (kb1, kb2) are run-time, K is streamed
+// through a ring of single [128 keys x 64 elements] blocks (16 KB each, one full / empty barrier pair per block) and the issuer
+// accumulates a step's logits block by block.  TMEM plan, softmax warps and epilogue are those of the fixed plans.
+template <>
+struct FwdCfg<0, 0> {
+  static constexpr bool BLOCKED = true;
+  static constexpr int BM = 128, BK = 128, BQ = BM;
+  static constexpr int KB1 = 0, KB2 = 0;                 // run-time (FwdParams::kb1, kb2)
+  static constexpr int QBLK = BM * 128, KBLK = BK * 128;
+  static constexpr int MAX_RING = 12;
+  static constexpr int AUX_BYTES = 512;
+  static constexpr int SMEM_LIMIT = 227 * 1024;
+  static constexpr int Q_BYTES = 0, STAGE_BYTES = KBLK, NSTAGE = MAX_RING;   // (unused by the blocked branches)
+  static constexpr int NGRP = 4, BC = BK / NGRP, CH = 8, NCH = BC / CH;
+  static constexpr int THREADS = 128 + NGRP * 128;
+  static constexpr uint32_t TMEM_COLS = 512;
+  static constexpr uint32_t POLY_MASK = STREAMKL_FWD_POLY_MASK_WIDE;
+  // ring blocks that fit beside the resident Q tile (host side)
+  static constexpr int ring_blocks(int kb1, int kb2) {
+    const int r = (SMEM_LIMIT - 1024 - AUX_BYTES - (kb1 + kb2) * QBLK) / KBLK;
+    return r > MAX_RING ? MAX_RING : r;
+  }
+  static constexpr int smem_bytes(int kb1, int kb2) { return 1024 + (kb1 + kb2) * QBLK + ring_blocks(kb1, kb2) * KBLK + AUX_BYTES; }
+};
+
 struct FwdParams {
   int NQ, NK, TQ;       // TQ = number of 128-row Q tiles per head
+  int kb1, kb2, nring;  // BLOCKED plan only: 64-element K-blocks per row of distribution 1 / 2, ring size in blocks
   int BH;               // B * H query heads
   int H, G;             // query heads per batch; query heads per K head (GQA: query head h reads K head h / G)
   uint32_t fmt16;       // operand format of the logit MMAs: 1 bf16, 0 fp16
@@ -230,14 +258,16 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
   using C = FwdCfg<D1, D2>;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const int KB1 = C::BLOCKED ? p.kb1 : C::KB1, KB2 = C::BLOCKED ? p.kb2 : C::KB2;
+  const int NRING = C::BLOCKED ? p.nring : C::NSTAGE;      // ring entries: whole stages, or single K-blocks (BLOCKED)
   uint8_t* sQ1 = smem;
-  uint8_t* sQ2 = sQ1 + C::KB1 * C::QBLK;
-  uint8_t* sK = smem + C::Q_BYTES;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(sK + C::NSTAGE * C::STAGE_BYTES);
+  uint8_t* sQ2 = sQ1 + KB1 * C::QBLK;
+  uint8_t* sK = smem + (KB1 + KB2) * C::QBLK;
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sK + NRING * C::STAGE_BYTES);
   uint64_t* q_full = bars;                    // 1
-  uint64_t* k_full = bars + 1;                // NSTAGE
-  uint64_t* k_empty = k_full + C::NSTAGE;     // NSTAGE
-  uint64_t* s_full = k_empty + C::NSTAGE;     // 2 (TMEM stage written by the tensor pipe)
+  uint64_t* k_full = bars + 1;                // NRING
+  uint64_t* k_empty = k_full + NRING;         // NRING
+  uint64_t* s_full = k_empty + NRING;         // 2 (TMEM stage written by the tensor pipe)
   uint64_t* s_empty = s_full + 2;             // 2 (all sixteen softmax warps are done with the stage)
   uint32_t* tmem_ptr = reinterpret_cast<uint32_t*>(s_empty + 2);
 
@@ -261,7 +291,7 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
   }
   if (warp == 1 && lane == 0) {
     mbar_init(q_full, 1);
-    for (int s = 0; s < C::NSTAGE; ++s) { mbar_init(&k_full[s], 1); mbar_init(&k_empty[s], 1); }
+    for (int s = 0; s < NRING; ++s) { mbar_init(&k_full[s], 1); mbar_init(&k_empty[s], 1); }
     for (int i = 0; i < 2; ++i) { mbar_init(&s_full[i], 1); mbar_init(&s_empty[i], 4 * C::NGRP); }
     fence_mbar_init();
   }
@@ -277,11 +307,26 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
     // ===================== TMA producer =====================
     if (lane == 0 && nsteps > 0) {
       const uint64_t pol_q = l2_policy_evict_first(), pol_k = l2_policy_evict_last();
-      mbar_arrive_expect_tx(q_full, C::Q_BYTES);
+      mbar_arrive_expect_tx(q_full, uint32_t((KB1 + KB2) * C::QBLK));
 #pragma unroll
-      for (int kb = 0; kb < C::KB1; ++kb) tma_load_4d_hint(sQ1 + kb * C::QBLK, &tmQ1, q_full, kb * 64, q0, hq, bq, pol_q);
+      for (int kb = 0; kb < KB1; ++kb) tma_load_4d_hint(sQ1 + kb * C::QBLK, &tmQ1, q_full, kb * 64, q0, hq, bq, pol_q);
 #pragma unroll
-      for (int kb = 0; kb < C::KB2; ++kb) tma_load_4d_hint(sQ2 + kb * C::QBLK, &tmQ2, q_full, kb * 64, q0, hq, bq, pol_q);
+      for (int kb = 0; kb < KB2; ++kb) tma_load_4d_hint(sQ2 + kb * C::QBLK, &tmQ2, q_full, kb * 64, q0, hq, bq, pol_q);
+      if constexpr (C::BLOCKED) {
+        // one ring entry per K-block, in the order the issuer consumes them: K1 blocks of step j, then its K2 blocks
+        int slot = 0;
+        uint32_t ph = 0;
+        for (int j = 0; j < nsteps; ++j) {
+          for (int b = 0; b < KB1 + KB2; ++b) {
+            mbar_wait(&k_empty[slot], ph ^ 1);
+            mbar_arrive_expect_tx(&k_full[slot], C::KBLK);
+            const bool one = b < KB1;
+            tma_load_4d_hint(sK + slot * C::KBLK, one ? &tmK1 : &tmK2, &k_full[slot], (one ? b : b - KB1) * 64, (j_begin + j) * C::BK, hk, bq,
+                             pol_k);
+            if (++slot == NRING) { slot = 0; ph ^= 1; }
+          }
+        }
+      } else
       for (int j = 0; j < nsteps; ++j) {
         const int s = j % C::NSTAGE;
         const uint32_t ph = (j / C::NSTAGE) & 1;
@@ -308,6 +353,30 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
       mbar_wait(q_full, 0);
       tc_fence_after();
     }
+    if constexpr (C::BLOCKED) {
+      int slot = 0;
+      uint32_t ph = 0;
+      for (int j = 0; j < nsteps; ++j) {
+        const int st = j & 1;
+        mbar_wait(&s_empty[st], ((j >> 1) & 1) ^ 1);
+        const uint32_t dS1 = tmem_base + st * (2 * C::BK);
+        for (int b = 0; b < KB1 + KB2; ++b) {
+          mbar_wait(&k_full[slot], ph);
+          tc_fence_after();
+          const bool one = b < KB1;
+          const uint32_t first = (b == 0 || b == KB1) ? 0u : 1u;        // a distribution's first block starts its accumulator
+          uint64_t a = dq1 + uint64_t((b * C::QBLK) >> 4), bk = dk + uint64_t((slot * C::KBLK) >> 4);   // (Q2 blocks follow Q1's)
+          if (elect_one()) {
+#pragma unroll
+            for (int k = 0; k < 4; ++k) umma_bf16_ss(one ? dS1 : dS1 + C::BK, a + uint64_t((k * 32) >> 4), bk + uint64_t((k * 32) >> 4), idesc, first | uint32_t(k != 0));
+            umma_commit(&k_empty[slot]);                                   // the block is reusable once these MMAs have retired
+            if (b + 1 == KB1 + KB2) umma_commit(&s_full[st]);
+          }
+          __syncwarp();
+          if (++slot == NRING) { slot = 0; ph ^= 1; }
+        }
+      }
+    } else
     for (int j = 0; j < nsteps; ++j) {
       const int s = j % C::NSTAGE;
       const uint32_t ph = (j / C::NSTAGE) & 1;

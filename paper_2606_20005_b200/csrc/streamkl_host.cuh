@@ -15,7 +15,7 @@ namespace sklh {
 extern thread_local int g_last_launches;   // kernels launched by the current streamkl_* call (streamkl_last_launch_count)
 
 // ---- optional per-kernel timing (streamkl_profile_*): CUDA events recorded on the launch stream around every kernel
-enum KernelId { KID_FWD_TC = 0, KID_BWD_DQ_TC, KID_BWD_DK_TC, KID_FWD_SIMT, KID_BWD_DQ_SIMT, KID_BWD_DK_SIMT, KID_BWD_STATS, KID_FWD_SPLITK_TC, KID_FWD_SPLITK_REDUCE, KID_BWD_FUSED_TC, KID_BWD_DQ_CONVERT, KID_COUNT };
+enum KernelId { KID_FWD_TC = 0, KID_BWD_DQ_TC, KID_BWD_DK_TC, KID_FWD_SIMT, KID_BWD_DQ_SIMT, KID_BWD_DK_SIMT, KID_BWD_STATS, KID_FWD_SPLITK_TC, KID_FWD_SPLITK_REDUCE, KID_BWD_FUSED_TC, KID_BWD_DQ_CONVERT, KID_BWD_DQ_WIDE, KID_BWD_DK_WIDE, KID_COUNT };
 struct ProfScope {  // brackets ONE kernel launch; a no-op unless profiling is enabled on this thread (defined in streamkl.cu)
   cudaStream_t st;
   cudaEvent_t b = nullptr;
@@ -42,8 +42,11 @@ struct Shape {
 constexpr int kFwdBQ = 128, kFwdBK = 128;
 // queries per head in the padded per-query scalar array of the backward (= skl::bwd_stats_padded_rows)
 constexpr long long stats_padded_rows(long long NQ) { return (NQ + 63) / 64 * 64; }
-// the tensor-core kernels are instantiated for head dims 64 and 128; anything else runs zero-padded to the next of the two
-inline int pad_dim(int d) { return d <= 64 ? 64 : 128; }
+// the tensor-core kernels work on head dims that are multiples of 64 (fixed plans: 64 and 128; run-time K-block counts above
+// that: 192 and 256); anything else runs zero-padded to the next multiple
+inline int pad_dim(int d) { return d <= 64 ? 64 : (d + 63) / 64 * 64; }
+constexpr int kMaxTcDim = 256;
+inline bool wide_dims(int d1, int d2) { return pad_dim(d1) > 128 || pad_dim(d2) > 128; }
 
 // 4-D maps {d, N, heads, B} of the four inputs, box = {64 elements, rows, 1, 1}, 128-byte swizzle, zero OOB fill
 bool make_maps(CUtensorMap (&t)[4], const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, int rows_q, int rows_k,
@@ -59,6 +62,11 @@ int bwd_tc_owner_q_launch(const void* Q1, const void* K1, const void* Q2, const 
                           void* dQ2, cudaStream_t stream);
 int bwd_tc_owner_k_launch(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, const void* stats, void* dK1,
                           void* dK2, cudaStream_t stream);
+// the owner kernels for head dims above 128 (streamkl_bwd_wide_q.cu / streamkl_bwd_wide_k.cu): one or two passes per owner side
+int bwd_wide_owner_q_launch(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, const void* stats, void* dQ1,
+                            void* dQ2, cudaStream_t stream);
+int bwd_wide_owner_k_launch(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, const void* stats, void* dK1,
+                            void* dK2, cudaStream_t stream);
 // one one-visit pass (student: dS2 -> dQ2, dK2; teacher: dS1 -> dQ1, dK1) + its dQ convert (streamkl_bwd_fused.cu)
 int bwd_tc_fused_launch(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, bool teacher_pass,
                         const void* stats, float* dq_acc, void* dQ, void* dK, cudaStream_t stream);

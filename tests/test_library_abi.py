@@ -121,7 +121,8 @@ def test_bwd_workspace_follows_the_selected_strategy(L):
     assert L.streamkl_bwd_workspace_bytes(1, 32, 16384, 16384, 128, 64, 0) == a256(32 * 16384 * 16) + a256(32 * 16384 * 64 * 4)
     assert L.streamkl_set_bwd_mode(0) == 0
     assert L.streamkl_bwd_workspace_bytes(1, 1, 256, 256, 44, 80, 0) == 0                  # head dim not a multiple of 8: SIMT path, no workspace
-    assert L.streamkl_bwd_workspace_bytes(1, 1, 256, 256, 192, 64, 0) == 0                 # head dim > 128: SIMT path
+    assert L.streamkl_bwd_workspace_bytes(1, 1, 256, 256, 192, 64, 0) == 256 * 16          # head dim > 128: wide owner kernels, statistics only
+    assert L.streamkl_bwd_workspace_bytes(1, 1, 256, 256, 264, 64, 0) == 0                 # head dim > 256: SIMT path
 
 
 def test_splitk_adaptive_split_selection_follows_the_paper_rule(L):

@@ -93,9 +93,9 @@ def test_degenerate_sizes(NQ, NK, causal):
 
 
 def test_simt_path_other_head_dims_bf16():
-    """Head dims that are not multiples of 8, or exceed 128, run the fp32 SIMT kernels."""
+    """Head dims that are not multiples of 8 (up to 256) run the fp32 SIMT kernels."""
     run_case(W.Config(41, "simt-bf16", 1, 2, 200, 300, 44, 84, "bf16", True))
-    run_case(W.Config(48, "simt-bf16-wide", 1, 2, 150, 260, 160, 192, "bf16", False))
+    run_case(W.Config(48, "simt-bf16-wide", 1, 2, 150, 260, 164, 196, "bf16", False))
 
 
 def test_simt_path_fp32_causal_teacher():

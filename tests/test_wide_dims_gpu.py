@@ -1,0 +1,126 @@
+"""GPU parity for head dims above 128 on the tensor cores (the paper fixes d = 128, and the
+DeepSeek-style teacher it names, :143, has 192-wide query/key heads): the BLOCKED forward plan (K streamed in single 64-element
+K-blocks) and the wide owner backward kernels (one differentiated distribution per pass when the accumulators do not fit TMEM
+together).  Everything is compared with the float64 definition on the same stored bits, per head, at the north-star tolerances;
+the profile of each call must show tcgen05 kernels only (no SIMT fallback)."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+import workloads as W
+from oracle.streamkl_oracle import attention_kl
+from parity_util import check_fwd, check_grad_heads, to_f64, to_torch
+from test_layouts_gpu import _as_bnhd, _run
+
+pytestmark = pytest.mark.gpu
+
+# every padded pair class: both-in-one-pass (192/64, 64/192), two passes (d1 + d2 > 256), ring depths from 4 down to the
+# 2 + 1 stages of 256/256, true dims that are not multiples of 64
+WIDE_PAIRS = [(192, 64), (64, 192), (192, 128), (128, 192), (192, 192), (256, 64), (64, 256), (256, 128), (128, 256), (256, 192),
+              (192, 256), (256, 256), (136, 72), (200, 248), (160, 8)]
+
+
+def _kernels_of(fn):
+    import torch
+
+    import paper_2606_20005_b200 as skl
+
+    skl.streamkl_profile_enable(True)
+    try:
+        fn()
+        torch.cuda.synchronize()
+    finally:
+        skl.streamkl_profile_enable(False)
+    return [n for n, _ in skl.streamkl_profile_collect()]
+
+
+@pytest.mark.parametrize("d1,d2", WIDE_PAIRS)
+def test_wide_head_dims_both_settings(d1, d2):
+    """ragged sizes spanning several tiles, causal with NQ != NK and no mask; Setting 2 (all four gradients) and Setting 1"""
+    _run(W.Config(100, f"wide{d1}x{d2}-causal", 1, 2, 333, 555, d1, d2, "bf16", True), both_modes=False)
+    _run(W.Config(101, f"wide{d1}x{d2}", 1, 2, 300, 450, d1, d2, "bf16", False), teacher=False, both_modes=False)
+
+
+@pytest.mark.parametrize("d1,d2", [(192, 64), (192, 128), (256, 256)])
+def test_wide_head_dims_run_on_the_tensor_cores(d1, d2):
+    import paper_2606_20005_b200 as skl
+
+    cfg = W.Config(102, "wide-kernels", 1, 2, 200, 300, d1, d2, "bf16", True)
+    inp = W.all_inputs(cfg)
+    dev = [to_torch(inp[k]) for k in ("Q1", "K1", "Q2", "K2")]
+    g = to_torch(inp["g"])
+    out = {}
+
+    def call():
+        out["f"] = skl.streamkl_fwd(*dev, cfg.c1, cfg.c2, True)
+        skl.streamkl_bwd(*dev, cfg.c1, cfg.c2, True, *out["f"], g, teacher=True)
+
+    names = _kernels_of(call)
+    passes = 1 if d1 + d2 <= 256 else 2
+    assert names == ["streamkl_fwd_sm100_kernel", "streamkl_bwd_stats_kernel"] + ["streamkl_bwd_wide_sm100_kernel<OWNER_Q>"] * passes + [
+        "streamkl_bwd_wide_sm100_kernel<OWNER_K>"] * passes, names
+
+
+@pytest.mark.parametrize("causal", [False, True])
+def test_wide_long_streams(causal):
+    """many steps per CTA (ring wrap-around, both TMEM stage parities, several Q / K tiles per head)"""
+    _run(W.Config(103, "wide-long", 1, 2, 1500, 1500, 192, 128, "bf16", causal), both_modes=False)
+    _run(W.Config(104, "wide-long256", 1, 1, 1100, 2100, 256, 256, "bf16", causal), both_modes=False)
+
+
+def test_wide_fp16_strided_shared_heads_relu():
+    """the layout features of the narrow kernels carry over: fp16, [B,N,H,d] strides, shared K heads, student ReLU"""
+    _run(W.Config(105, "wide-f16", 1, 3, 260, 520, 192, 64, "f16", True), both_modes=False)
+    _run(W.Config(106, "wide-bnhd", 2, 2, 300, 300, 192, 192, "bf16", True), view=_as_bnhd, both_modes=False)
+    _run(W.Config(107, "wide-gqa", 1, 4, 200, 400, 256, 128, "bf16", False), HK=2, both_modes=False)
+    _run(W.Config(108, "wide-relu", 1, 2, 300, 500, 192, 64, "bf16", True), act2="relu", both_modes=False)
+    _run(W.Config(109, "wide-all", 2, 4, 260, 777, 200, 72, "f16", True), HK=2, view=_as_bnhd, act2="relu", both_modes=False)
+
+
+def test_wide_degenerate_sizes():
+    """one key, one query, a single partial tile, NQ = 1 against many keys"""
+    _run(W.Config(110, "wide-1x1", 1, 1, 1, 1, 192, 192, "bf16", False), both_modes=False)
+    _run(W.Config(111, "wide-1xN", 1, 2, 1, 700, 256, 64, "bf16", True), both_modes=False)
+    _run(W.Config(112, "wide-tile", 1, 1, 127, 129, 192, 256, "bf16", True), both_modes=False)
+
+
+@pytest.mark.parametrize("d1,d2", [(192, 64), (256, 256)])
+def test_wide_splitk(d1, d2):
+    """split-K forward through the BLOCKED plan"""
+    import paper_2606_20005_b200 as skl
+
+    cfg = W.Config(113, "wide-splitk", 1, 2, 40, 5000, d1, d2, "bf16", False)
+    inp = W.all_inputs(cfg)
+    f = {k: W.widen_f64(inp[k]) for k in ("Q1", "K1", "Q2", "K2")}
+    ref = attention_kl(f["Q1"], f["K1"], f["Q2"], f["K2"], cfg.c1, cfg.c2, False)
+    dev = [to_torch(inp[k]) for k in ("Q1", "K1", "Q2", "K2")]
+    for splits in (0, 3, 40):
+        names = _kernels_of(lambda: check_fwd(*(to_f64(t) for t in skl.streamkl_fwd_splitk(*dev, cfg.c1, cfg.c2, False, splits=splits)), ref,
+                                              f"wide split-K W={splits}"))
+        assert names == ["streamkl_fwd_sm100_kernel<SPLIT>", "streamkl_fwd_splitk_reduce_kernel"], names
+
+
+def test_wide_gradient_padding_columns_are_left_untouched():
+    """d = 160 inside a 256-wide row: the columns between rows belong to the caller and must survive the backward"""
+    import torch
+
+    import paper_2606_20005_b200 as skl
+
+    cfg = W.Config(114, "d160-in-256", 1, 2, 200, 300, 160, 160, "bf16", False)
+    inp = W.all_inputs(cfg)
+    f = {k: W.widen_f64(inp[k]) for k in ("Q1", "K1", "Q2", "K2")}
+    ref = attention_kl(f["Q1"], f["K1"], f["Q2"], f["K2"], cfg.c1, cfg.c2, False, g=inp["g"].astype(np.float64), teacher=True)
+    wide = {k: torch.full((cfg.B, cfg.H, inp[k].shape[2], 256), 7.0, dtype=torch.bfloat16, device="cuda") for k in ("Q1", "K1", "Q2", "K2")}
+    dev = {}
+    for k in wide:
+        wide[k][..., :160] = to_torch(inp[k])
+        dev[k] = wide[k][..., :160]
+    kl, l1, l2 = skl.streamkl_fwd(dev["Q1"], dev["K1"], dev["Q2"], dev["K2"], cfg.c1, cfg.c2, False)
+    check_fwd(to_f64(kl), to_f64(l1), to_f64(l2), ref, "d160-in-256 fwd")
+    outs = {k: torch.full_like(wide[k], 5.0) for k in wide}
+    skl.streamkl_bwd(dev["Q1"], dev["K1"], dev["Q2"], dev["K2"], cfg.c1, cfg.c2, False, kl, l1, l2, to_torch(inp["g"]), teacher=True,
+                     dQ1=outs["Q1"][..., :160], dK1=outs["K1"][..., :160], dQ2=outs["Q2"][..., :160], dK2=outs["K2"][..., :160])
+    for k, name in (("Q1", "dQ1"), ("K1", "dK1"), ("Q2", "dQ2"), ("K2", "dK2")):
+        check_grad_heads(to_f64(outs[k][..., :160]), ref[name], name)
+        assert bool((outs[k][..., 160:] == 5.0).all()), f"{name} wrote beyond its head dim"
