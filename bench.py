@@ -41,7 +41,7 @@ UNIT = "TFLOP/s"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 SPEC_BF16_TFLOPS = 2250.0
 WORKLOADS = {"cfg2": 2, "cfg3": 3, "cfg4": 4, "cfg5": 5}
-SIDE_LEGS = ("splitk", "bwd-strategies")   # --workload <leg>: run only that secondary measurement (profiling runs)
+SIDE_LEGS = ("splitk", "bwd-strategies", "wide-dims")   # --workload <leg>: run only that secondary measurement (profiling runs)
 
 
 def peaks():
@@ -403,6 +403,29 @@ def kernel_flops_one_visit(cfg: W.Config, name: str, launches_of_bwd_kernels: fl
 BWD_MODES = {"auto": 0, "separate": 1, "fused": 2}
 
 
+def time_wide_dims(skl, steps: int = 5, warmup: int = 3, heads: int = 8, N: int = 16384, pairs=None):
+    """Head dims above 128: fwd + bwd at N = 16K, causal, `heads` heads, next to the d = 128/128 and 128/64 fixed
+    plans at the same size.  TFLOP/s on the one-visit count (executed FLOPs of the wide backward are higher: a launch
+    differentiates one distribution when d1 + d2 > 256 padded, and every launch recomputes both logit tiles)."""
+    import torch
+
+    rows = {}
+    for d1, d2, teacher in (pairs or ((128, 128, True), (128, 64, False), (192, 64, False), (192, 64, True), (192, 128, True), (192, 192, True),
+                                      (256, 128, True), (256, 256, False), (256, 256, True))):
+        cfg = W.Config(72, f"wide-{d1}x{d2}", 1, heads, N, N, d1, d2, "bf16", True, teacher_grads=teacher)
+        h = W.all_inputs(cfg)
+        d = tuple(to_dev(h[k]) for k in ("Q1", "K1", "Q2", "K2", "g"))
+        r = time_passes(skl, cfg, d, steps, warmup, lambda: None)
+        bwd_launches = sum(v["launches_per_step"] for k, v in r["kernels"].items() if "bwd" in k and "sm100" in k)
+        rows[f"d={d1}/{d2} " + ("all four grads" if teacher else "dQ2,dK2 only")] = {
+            "fwd_ms": r["fwd_ms"], "bwd_ms": r["bwd_ms"], "fwd_tflops": cfg.fwd_flop() / (r["fwd_ms"] * 1e-3) / 1e12,
+            "bwd_tflops_one_visit": cfg.bwd_flop() / (r["bwd_ms"] * 1e-3) / 1e12, "bwd_tensor_core_launches": bwd_launches,
+            "kernels_ms": {k: v["avg_ms"] for k, v in r["kernels"].items()}}
+        del d, h, r
+        torch.cuda.empty_cache()
+    return {"shape": f"B=1, H={heads}, NQ=NK={N}, bf16, causal", "rows": rows}
+
+
 def time_bwd_strategies(skl, iters: int = 20, nqs=(16, 128, 256, 512, 1024, 4096)):
     """Backward strategy table (Fig.13): separate owner kernels vs the one-visit kernels,
     both settings, small-to-medium N_Q, bsz 16, N_K = 16384, d = 128/128, no mask.  ms per streamkl_bwd call."""
@@ -471,6 +494,8 @@ def main():
         torch.cuda.set_device(local)
         if args.workload == "splitk":
             out = time_splitk(skl, iters=args.iters)
+        elif args.workload == "wide-dims":
+            out = time_wide_dims(skl)
         else:
             out = time_bwd_strategies(skl, iters=args.iters, nqs=(args.nq,) if args.nq > 0 else (16, 128, 256, 512, 1024, 4096))
         if rank == 0:
@@ -575,6 +600,7 @@ def main():
                           "frac": sk["hbm_gbs"] / float(pk["hbm_gbs"])}
         also["split-K forward (bsz=16, NQ=16, NK=131072, d=128/128, no mask)"] = sk
         also["backward strategies (separate owner kernels vs one-visit kernels)"] = time_bwd_strategies(skl)
+        also["head dims above 128 (BLOCKED forward plan, wide owner backward kernels)"] = time_wide_dims(skl)
 
     # ---- e2e: host buffers through streamkl_fwd_bwd_host (copies inside the timed region)
     e2e = None
