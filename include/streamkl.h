@@ -19,8 +19,9 @@
  *    always contiguous [B][H][NQ] float32.  Outputs are in natural-log units.
  *  - The plain entry points take bf16, `*_f32` fp32, `*_ex` the element type named in the layout (bf16 / fp16 / fp32); gradients
  *    come back in the input type (one rounding from fp32 accumulators).  All accumulation is fp32.  16-bit inputs with d1, d2
- *    multiples of 8 up to 128 run the tcgen05/TMA kernels (head dims other than 64 / 128 zero-padded to the next of the two);
- *    every other case (fp32 inputs, head dims up to 256 that are not multiples of 8 or exceed 128) runs the SIMT fp32 kernels.
+ *    multiples of 8 up to 256 run the tcgen05/TMA kernels (head dims zero-padded to the next multiple of 64 inside the kernels;
+ *    above 128 the forward streams K in 64-element K-blocks and the backward differentiates one distribution per launch when
+ *    d1 + d2 > 256 padded); every other case (fp32 inputs, head dims up to 256 that are not multiples of 8) runs the SIMT fp32 kernels.
  *  - Device entry points take DEVICE pointers owned by the caller; the library never allocates, frees or
  *    retains them, and only enqueues work on `stream` (asynchronous; device faults surface at the caller's next
  *    synchronisation).  `*_host` entry points take HOST pointers, allocate their own device scratch, copy in,
@@ -87,8 +88,8 @@ int streamkl_fwd_f32(const void* Q1, const void* K1, const void* Q2, const void*
  *                STREAMKL_ACT_RELU: the student's logit is s2[j] = relu(c2 <Q2[i], K2[j]>) -- that indexer's score with one head and
  *                unit weight -- and P2 = softmax_j(s2) as before; kl / lse2 are those of this P2, and the student's logit gradient
  *                is gated by relu': dS2 = g (P2 - P1) 1[<Q2[i],K2[j]> > 0].  The teacher side (P1, dS1 of Eq.3) is unchanged.
- * Non-default strides, kv_heads and activations need the tensor-core path: 16-bit dtype and d1, d2 multiples of 8 up to 128 (STREAMKL_ERR_SHAPE
- * otherwise).  Head dims other than 64 / 128 run zero-padded to the next of the two inside the kernels (TMA zero fill): the
+ * Non-default strides, kv_heads and activations need the tensor-core path: 16-bit dtype and d1, d2 multiples of 8 up to 256 (STREAMKL_ERR_SHAPE
+ * otherwise).  Head dims that are not multiples of 64 run zero-padded to the next multiple inside the kernels (TMA zero fill): the
  * results are exact, the padded columns cost tensor work.
  */
 enum { STREAMKL_ACT_NONE = 0, STREAMKL_ACT_RELU = 1 };
@@ -110,7 +111,7 @@ int streamkl_bwd_ex(const streamkl_layout* layout, const void* Q1, const void* K
                     void* workspace, size_t workspace_bytes, streamkl_stream_t stream);
 
 /*
- * Split-K forward for small NQ (Eq.11; bf16, d1,d2 in {64,128}).  The key range is cut into W
+ * Split-K forward for small NQ (Eq.11; bf16, d1,d2 multiples of 8 up to 256).  The key range is cut into W
  * contiguous chunks of C_K = 128*ceil(ceil(NK/128)/W) keys (the paper's ceil(NK/W), rounded up to whole 128-key tiles);
  * the grid becomes (bsz, T_Q, W); every CTA writes its chunk's partial statistics (m1,l1,m2,l2,acc) -- 5 floats per
  * row and chunk -- to `workspace`, and a reduce kernel merges them with Eq.11 ((m2,l2) merged the same way) and
@@ -165,6 +166,9 @@ int streamkl_bwd_f32(const void* Q1, const void* K1, const void* Q2, const void*
  *                           NQ <= 256 with them (the paper's rule T_Q*C <= T_K, with the crossover found
  *                           independent of T_K) -- else SEPARATE.  NOTE: AUTO is therefore NOT bit-reproducible for small NQ;
  *                           select STREAMKL_BWD_SEPARATE where that matters.
+ * Head dims above 128 always run the owner kernels (deterministic) whatever the mode: one launch per owner side when the
+ * gradient accumulators of everything requested fit TMEM together (d1 + d2 <= 256 after padding to multiples of 64, or no
+ * teacher gradients), else a student launch and a teacher launch per owner side.
  * Returns STREAMKL_OK, or STREAMKL_ERR_SHAPE for an unknown mode.
  */
 enum { STREAMKL_BWD_AUTO = 0, STREAMKL_BWD_SEPARATE = 1, STREAMKL_BWD_FUSED = 2 };
