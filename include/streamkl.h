@@ -174,6 +174,19 @@ int streamkl_bwd_f32(const void* Q1, const void* K1, const void* Q2, const void*
 enum { STREAMKL_BWD_AUTO = 0, STREAMKL_BWD_SEPARATE = 1, STREAMKL_BWD_FUSED = 2 };
 int streamkl_set_bwd_mode(int mode);
 
+/*
+ * Forward plan of the default (unsplit) tcgen05 kernel, per calling thread (SURVEY 8(f) NEXT-3 "2-CTA / multicast variants"):
+ *   STREAMKL_FWD_SINGLE    : (default) one CTA per 128-row Q tile, each streaming the head's K tiles from L2 on its own.
+ *   STREAMKL_FWD_MULTICAST : clusters of two CTAs own the Q tiles (2i, 2i+1) of a head and share ONE K stream -- each CTA's
+ *                            producer loads half of every stage's K-blocks with TMA multicast into both rings, a stage is
+ *                            refilled once both CTAs' MMAs on it have retired.  Half the L2 -> SM traffic; bit-identical
+ *                            results.  Measured on B200 it is a tie for head dims <= 128 and 6-8 % slower above (the pair
+ *                            runs in lock step on a shallow ring), which is why it is not the default.
+ * Returns STREAMKL_OK, or STREAMKL_ERR_SHAPE for an unknown plan.
+ */
+enum { STREAMKL_FWD_SINGLE = 0, STREAMKL_FWD_MULTICAST = 1 };
+int streamkl_set_fwd_plan(int plan);
+
 /* Bytes of device scratch streamkl_bwd needs for this shape UNDER THE CALLING THREAD'S CURRENT MODE (O((NQ+NK)*d) at most,
  * never O(NQ*NK)): 16 B per query of packed per-query scalars, plus -- only when the one-visit strategy will run (mode FUSED,
  * or AUTO below its crossover) -- the fp32 dQ2 (and dQ1) accumulators, each region padded to 256 B. */

@@ -16,6 +16,9 @@ from .binding import (  # noqa: F401
     streamkl_fwd_splitk,
     streamkl_host_trim,
     streamkl_set_bwd_mode,
+    streamkl_set_fwd_plan,
+    STREAMKL_FWD_SINGLE,
+    STREAMKL_FWD_MULTICAST,
     STREAMKL_BWD_AUTO,
     STREAMKL_BWD_SEPARATE,
     STREAMKL_BWD_FUSED,

@@ -19,6 +19,7 @@
 namespace sklh {
 
 thread_local int g_last_launches = 0;
+thread_local int g_fwd_plan = STREAMKL_FWD_SINGLE;
 
 namespace {
 struct ProfRecord { int id; cudaEvent_t a, b; };
@@ -493,6 +494,12 @@ size_t streamkl_bwd_workspace_bytes(int B, int H, int NQ, int, int d1, int d2, i
   if (!bwd_fused_selected(NQ, want_teacher != 0, d1, d2)) return size_t(BH) * size_t(stats_padded_rows(NQ)) * 16;
   // one-visit kernels (mode FUSED, or AUTO with NQ <= 512): + their fp32 dQ accumulators, O(NQ d)
   return stats_bytes_aligned(BH, NQ) + fused_acc_bytes_aligned(BH, NQ, pad_dim(d2)) + (want_teacher ? fused_acc_bytes_aligned(BH, NQ, pad_dim(d1)) : 0);
+}
+
+int streamkl_set_fwd_plan(int plan) {
+  if (plan != STREAMKL_FWD_SINGLE && plan != STREAMKL_FWD_MULTICAST) return STREAMKL_ERR_SHAPE;
+  g_fwd_plan = plan;
+  return STREAMKL_OK;
 }
 
 int streamkl_set_bwd_mode(int mode) {

@@ -10,14 +10,14 @@ static_assert(skl::FwdCfg<128, 128>::BQ == kFwdBQ && skl::FwdCfg<64, 64>::BK == 
 // splits == 1: the default kernel (grid (bsz, T_Q)).  splits > 1: split-K (grid (bsz, T_Q, W), partial
 // statistics to `part`, then the reduce kernel).
 // D1 = D2 = 0: the BLOCKED plan with run-time K-block counts (a head dim above 128, padded to 192 / 256).
-template <int D1, int D2, bool CAUSAL, bool SPLIT = false>
+template <int D1, int D2, bool CAUSAL, bool SPLIT = false, bool MC = false>
 int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, float* kl, float* lse1,
                   float* lse2, cudaStream_t stream, int splits = 1, float* part = nullptr) {
   using C = skl::FwdCfg<D1, D2>;
   CUtensorMap tm[4];
   if (!make_maps(tm, Q1, K1, Q2, K2, s, C::BM, C::BK, f16)) return STREAMKL_ERR_CUDA;
   const CUtensorMap &tQ1 = tm[0], &tK1 = tm[1], &tQ2 = tm[2], &tK2 = tm[3];
-  auto kern = skl::streamkl_fwd_sm100_kernel<D1, D2, CAUSAL, SPLIT>;
+  auto kern = skl::streamkl_fwd_sm100_kernel<D1, D2, CAUSAL, SPLIT, MC>;
   skl::FwdParams p;
   p.kb1 = pad_dim(s.d1) / 64; p.kb2 = pad_dim(s.d2) / 64; p.nring = 0;
   int smem_bytes = 0;
@@ -42,11 +42,21 @@ int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2
   p.chunk_steps = SPLIT ? (TK + splits - 1) / splits : TK;       // C_K = ceil(N_K / W), in whole BK-key steps
   p.W = SPLIT ? (TK + p.chunk_steps - 1) / p.chunk_steps : 1;    // no empty trailing chunk
   p.part = part;
-  const long long grid = (long long)p.TQ * s.BH * p.W;
+  const long long grid = MC ? 2LL * ((p.TQ + 1) / 2) * s.BH : (long long)p.TQ * s.BH * p.W;
   if (grid > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
   {
     ProfScope ps(SPLIT ? KID_FWD_SPLITK_TC : KID_FWD_TC, stream);
-    kern<<<dim3((unsigned)grid), C::THREADS, smem_bytes, stream>>>(tQ1, tK1, tQ2, tK2, p);
+    if constexpr (MC) {   // clusters of two CTAs: the Q tiles (2i, 2i+1) of a head share one multicast K stream
+      cudaLaunchConfig_t cfg = {};
+      cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(C::THREADS); cfg.dynamicSmemBytes = size_t(smem_bytes); cfg.stream = stream;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension;
+      at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+      cfg.attrs = at; cfg.numAttrs = 1;
+      if (cudaLaunchKernelEx(&cfg, kern, tQ1, tK1, tQ2, tK2, p) != cudaSuccess) { cudaGetLastError(); return STREAMKL_ERR_CUDA; }
+    } else {
+      kern<<<dim3((unsigned)grid), C::THREADS, smem_bytes, stream>>>(tQ1, tK1, tQ2, tK2, p);
+    }
   }
   if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
   g_last_launches += 1;
@@ -68,6 +78,18 @@ int fwd_tc_launch(const void* Q1, const void* K1, const void* Q2, const void* K2
                   cudaStream_t stream, int splits, float* part) {
   int p1 = pad_dim(s.d1), p2 = pad_dim(s.d2);
   if (p1 > 128 || p2 > 128) p1 = p2 = 0;   // a wide head dim: the BLOCKED plan (run-time K-block counts)
+  // the multicast pair plan (streamkl_set_fwd_plan): the default grid only, and only when a head has a second Q tile to pair
+  const bool mc = g_fwd_plan == STREAMKL_FWD_MULTICAST && splits <= 1 && s.NQ > skl::FwdCfg<64, 64>::BQ;
+#define SKL_FWD_MC_CASE(A, Bd)                                                                                                    \
+  if (mc && p1 == A && p2 == Bd)                                                                                                  \
+    return s.causal ? launch_fwd_tc<A, Bd, true, false, true>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream)                     \
+                    : launch_fwd_tc<A, Bd, false, false, true>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream);
+  SKL_FWD_MC_CASE(128, 128)
+  SKL_FWD_MC_CASE(128, 64)
+  SKL_FWD_MC_CASE(64, 128)
+  SKL_FWD_MC_CASE(64, 64)
+  SKL_FWD_MC_CASE(0, 0)
+#undef SKL_FWD_MC_CASE
 #define SKL_FWD_CASE(A, Bd)                                                                                                       \
   if (p1 == A && p2 == Bd) {                                                                                                      \
     if (splits > 1)                                                                                                               \

@@ -251,7 +251,11 @@ __device__ __noinline__ RowState safe_step(uint32_t taddr, RowState st, float sc
   return st;   // by value: the state stays in registers across the call (a reference parameter would pin it to local memory)
 }
 
-template <int D1, int D2, bool CAUSAL, bool SPLIT = false>
+// MC: launched as clusters of two CTAs that own the two Q tiles (2i, 2i+1) of one head and share ONE K stream -- each CTA's
+// producer loads half of every stage's K-blocks and multicasts them into both CTAs' rings (half the L2 -> SM traffic per
+// tile pair; SURVEY 8(f) NEXT-3 "2-CTA / multicast variants").  Both CTAs run the K pipeline for the pair's longer step
+// count; a stage is reloaded only after BOTH issuers' MMAs on it have retired (k_empty counts two multicast commits).
+template <int D1, int D2, bool CAUSAL, bool SPLIT = false, bool MC = false>
 __global__ void __launch_bounds__(FwdCfg<D1, D2>::THREADS, 1)
 streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid_constant__ CUtensorMap tmK1,
                           const __grid_constant__ CUtensorMap tmQ2, const __grid_constant__ CUtensorMap tmK2, const FwdParams p) {
@@ -273,31 +277,42 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   // heavy (late, causal) query tiles first within each head; consecutive CTAs share a head (K stays in L2)
-  const int tile = SPLIT ? int(blockIdx.x) / p.W : int(blockIdx.x);
+  static_assert(!(MC && SPLIT), "the multicast pair plan exists for the default grid");
+  const int tile = SPLIT ? int(blockIdx.x) / p.W : (MC ? int(blockIdx.x) >> 1 : int(blockIdx.x));
   const int wk = SPLIT ? int(blockIdx.x) % p.W : 0;          // key chunk of this CTA (split-K grid (b, i, w))
-  const int bh = tile / p.TQ;
+  const int crank = MC ? int(blockIdx.x) & 1 : 0;            // rank within the cluster pair
+  const int TQU = MC ? (p.TQ + 1) / 2 : p.TQ;                // scheduling units per head: Q tiles, or pairs of them
+  const int bh = tile / TQU;
   const int hq = bh % p.H, bq = bh / p.H, hk = hq / p.G;      // TMA coordinates {d, row, head, batch}
-  const int qt = p.TQ - 1 - (tile % p.TQ);
+  // MC: pair u (heavy first) = tiles TQ-1-2u (rank 0) and TQ-2-2u (rank 1; absent for the last pair of an odd TQ)
+  const int qt = MC ? p.TQ - 1 - 2 * (tile % TQU) - crank : p.TQ - 1 - (tile % p.TQ);
   const int q0 = qt * C::BQ;
   const int off = p.NK - p.NQ;
   const int TK = (p.NK + C::BK - 1) / C::BK;
   const int j_begin = SPLIT ? wk * p.chunk_steps : 0;        // this CTA's 128-key steps are [j_begin, j_begin + nsteps)
   int j_end = SPLIT ? min(TK, j_begin + p.chunk_steps) : TK;
   if (CAUSAL) j_end = min(j_end, min(p.NK - 1, q0 + C::BM - 1 + off) / C::BK + 1);   // past the tile's causal frontier
-  const int nsteps = max(0, j_end - j_begin);
+  const int nsteps = (MC && qt < 0) ? 0 : max(0, j_end - j_begin);
+  // MC: steps of the K pipeline both CTAs run = the pair's longer count (rank 0 owns the later tile: never the shorter one)
+  int nsteps_pair = nsteps;
+  if (MC) {
+    const int q0a = (qt + crank) * C::BQ;                    // rank 0's tile
+    nsteps_pair = CAUSAL ? min(TK, min(p.NK - 1, q0a + C::BM - 1 + off) / C::BK + 1) : TK;
+  }
 
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tmQ1); tma_prefetch_desc(&tmK1); tma_prefetch_desc(&tmQ2); tma_prefetch_desc(&tmK2);
   }
   if (warp == 1 && lane == 0) {
     mbar_init(q_full, 1);
-    for (int s = 0; s < NRING; ++s) { mbar_init(&k_full[s], 1); mbar_init(&k_empty[s], 1); }
+    for (int s = 0; s < NRING; ++s) { mbar_init(&k_full[s], 1); mbar_init(&k_empty[s], MC ? 2 : 1); }
     for (int i = 0; i < 2; ++i) { mbar_init(&s_full[i], 1); mbar_init(&s_empty[i], 4 * C::NGRP); }
     fence_mbar_init();
   }
   if (warp == 2) tmem_alloc<C::TMEM_COLS>(tmem_ptr);
   tc_fence_before();
   __syncthreads();
+  if (MC) cluster_sync_all();   // the peer's barriers exist before anything is multicast to them
   tc_fence_after();
   const uint32_t tmem_base = *tmem_ptr;
 
@@ -305,13 +320,52 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
    reg_dealloc<24>();   // (pool: (96-24)*128 = 9216 >= (112-96)*512) producer / MMA / allocator warpgroup gives its registers to the softmax warpgroups
    if (warp == 0) {
     // ===================== TMA producer =====================
-    if (lane == 0 && nsteps > 0) {
+    if (lane == 0 && (MC ? nsteps_pair : nsteps) > 0) {
       const uint64_t pol_q = l2_policy_evict_first(), pol_k = l2_policy_evict_last();
-      mbar_arrive_expect_tx(q_full, uint32_t((KB1 + KB2) * C::QBLK));
+      if (nsteps > 0) {
+        mbar_arrive_expect_tx(q_full, uint32_t((KB1 + KB2) * C::QBLK));
 #pragma unroll
-      for (int kb = 0; kb < KB1; ++kb) tma_load_4d_hint(sQ1 + kb * C::QBLK, &tmQ1, q_full, kb * 64, q0, hq, bq, pol_q);
+        for (int kb = 0; kb < KB1; ++kb) tma_load_4d_hint(sQ1 + kb * C::QBLK, &tmQ1, q_full, kb * 64, q0, hq, bq, pol_q);
 #pragma unroll
-      for (int kb = 0; kb < KB2; ++kb) tma_load_4d_hint(sQ2 + kb * C::QBLK, &tmQ2, q_full, kb * 64, q0, hq, bq, pol_q);
+        for (int kb = 0; kb < KB2; ++kb) tma_load_4d_hint(sQ2 + kb * C::QBLK, &tmQ2, q_full, kb * 64, q0, hq, bq, pol_q);
+      }
+      if constexpr (MC && C::BLOCKED) {
+        // every CTA expects every block on its own barrier; it issues (and multicasts) the blocks of its own parity
+        int slot = 0, cnt = 0;
+        uint32_t ph = 0;
+        for (int j = 0; j < nsteps_pair; ++j) {
+          for (int b = 0; b < KB1 + KB2; ++b, ++cnt) {
+            mbar_wait(&k_empty[slot], ph ^ 1);
+            mbar_arrive_expect_tx(&k_full[slot], C::KBLK);
+            const bool one = b < KB1;
+            if ((cnt & 1) == crank)
+              tma_load_4d_mcast(sK + slot * C::KBLK, one ? &tmK1 : &tmK2, &k_full[slot], (one ? b : b - KB1) * 64, j * C::BK, hk, bq, uint16_t(3),
+                                pol_k);
+            if (++slot == NRING) { slot = 0; ph ^= 1; }
+          }
+        }
+        // drain: the last NRING blocks' release by both issuers (slot / ph now name the entry after the last one used)
+        const int total = nsteps_pair * (KB1 + KB2);
+        for (int i = 0; i < min(total, NRING); ++i) {
+          mbar_wait(&k_empty[slot], ph ^ 1);
+          if (++slot == NRING) { slot = 0; ph ^= 1; }
+        }
+      } else if constexpr (MC) {
+        for (int j = 0; j < nsteps_pair; ++j) {
+          const int s = j % C::NSTAGE;
+          const uint32_t ph = (j / C::NSTAGE) & 1;
+          mbar_wait(&k_empty[s], ph ^ 1);                       // both CTAs' MMAs on this stage have retired
+          mbar_arrive_expect_tx(&k_full[s], C::STAGE_BYTES);    // the whole stage: this CTA's blocks and the peer's
+          uint8_t* st = sK + s * C::STAGE_BYTES;
+#pragma unroll
+          for (int kb = 0; kb < C::KB1 + C::KB2; ++kb)
+            if ((kb & 1) == crank)
+              tma_load_4d_mcast(st + kb * C::KBLK, kb < C::KB1 ? &tmK1 : &tmK2, &k_full[s], (kb < C::KB1 ? kb : kb - C::KB1) * 64, j * C::BK, hk, bq,
+                                uint16_t(3), pol_k);
+        }
+        // drain: the last commits of both issuers have arrived here before this CTA may leave the cluster
+        for (int j = max(0, nsteps_pair - C::NSTAGE); j < nsteps_pair; ++j) mbar_wait(&k_empty[j % C::NSTAGE], (j / C::NSTAGE) & 1);
+      } else
       if constexpr (C::BLOCKED) {
         // one ring entry per K-block, in the order the issuer consumes them: K1 blocks of step j, then its K2 blocks
         int slot = 0;
@@ -356,20 +410,28 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
     if constexpr (C::BLOCKED) {
       int slot = 0;
       uint32_t ph = 0;
-      for (int j = 0; j < nsteps; ++j) {
+      for (int j = 0; j < (MC ? nsteps_pair : nsteps); ++j) {
         const int st = j & 1;
-        mbar_wait(&s_empty[st], ((j >> 1) & 1) ^ 1);
+        const bool own = !MC || j < nsteps;   // MC: beyond this CTA's own steps only the shared ring is kept moving
+        if (own) mbar_wait(&s_empty[st], ((j >> 1) & 1) ^ 1);
         const uint32_t dS1 = tmem_base + st * (2 * C::BK);
         for (int b = 0; b < KB1 + KB2; ++b) {
           mbar_wait(&k_full[slot], ph);
           tc_fence_after();
+          if (!own) {
+            if (elect_one()) umma_commit_mcast(&k_empty[slot], uint16_t(3));
+            __syncwarp();
+            if (++slot == NRING) { slot = 0; ph ^= 1; }
+            continue;
+          }
           const bool one = b < KB1;
           const uint32_t first = (b == 0 || b == KB1) ? 0u : 1u;        // a distribution's first block starts its accumulator
           uint64_t a = dq1 + uint64_t((b * C::QBLK) >> 4), bk = dk + uint64_t((slot * C::KBLK) >> 4);   // (Q2 blocks follow Q1's)
           if (elect_one()) {
 #pragma unroll
             for (int k = 0; k < 4; ++k) umma_bf16_ss(one ? dS1 : dS1 + C::BK, a + uint64_t((k * 32) >> 4), bk + uint64_t((k * 32) >> 4), idesc, first | uint32_t(k != 0));
-            umma_commit(&k_empty[slot]);                                   // the block is reusable once these MMAs have retired
+            // the block is reusable once these MMAs have retired (MC: in both CTAs)
+            if (MC) umma_commit_mcast(&k_empty[slot], uint16_t(3)); else umma_commit(&k_empty[slot]);
             if (b + 1 == KB1 + KB2) umma_commit(&s_full[st]);
           }
           __syncwarp();
@@ -377,10 +439,15 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
         }
       }
     } else
-    for (int j = 0; j < nsteps; ++j) {
+    for (int j = 0; j < (MC ? nsteps_pair : nsteps); ++j) {
       const int s = j % C::NSTAGE;
       const uint32_t ph = (j / C::NSTAGE) & 1;
       mbar_wait(&k_full[s], ph);
+      if (MC && j >= nsteps) {   // the peer's tile is longer: keep the shared K pipeline moving, compute nothing
+        if (elect_one()) umma_commit_mcast(&k_empty[s], uint16_t(3));
+        __syncwarp();
+        continue;
+      }
       const int st = j & 1;
       const uint32_t sph = (j >> 1) & 1;
       mbar_wait(&s_empty[st], sph ^ 1);
@@ -406,7 +473,8 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
             umma_bf16_ss(dS2, a2 + uint64_t((kb * C::QBLK + k * 32) >> 4),
                          bk + uint64_t(((C::KB1 + kb) * C::KBLK + k * 32) >> 4), idesc, (kb | k) != 0);
         umma_commit(&s_full[st]);
-        umma_commit(&k_empty[s]);  // K stage reusable once every MMA that read it has retired
+        // K stage reusable once every MMA that read it has retired (MC: in both CTAs -- the arrive goes to both rings)
+        if (MC) umma_commit_mcast(&k_empty[s], uint16_t(3)); else umma_commit(&k_empty[s]);
       }
       __syncwarp();
     }
@@ -590,6 +658,7 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
   }
   tc_fence_before();
   __syncthreads();
+  if (MC) cluster_sync_all();   // neither CTA leaves while the other may still multicast into its ring or arrive on its barriers
   if (warp == 2) {
     tc_fence_after();
     tmem_dealloc<C::TMEM_COLS>(tmem_base);

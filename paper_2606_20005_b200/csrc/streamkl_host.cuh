@@ -12,6 +12,7 @@
 
 namespace sklh {
 
+extern thread_local int g_fwd_plan;        // streamkl_set_fwd_plan: STREAMKL_FWD_SINGLE | STREAMKL_FWD_MULTICAST
 extern thread_local int g_last_launches;   // kernels launched by the current streamkl_* call (streamkl_last_launch_count)
 
 // ---- optional per-kernel timing (streamkl_profile_*): CUDA events recorded on the launch stream around every kernel

@@ -124,3 +124,36 @@ def test_wide_gradient_padding_columns_are_left_untouched():
     for k, name in (("Q1", "dQ1"), ("K1", "dK1"), ("Q2", "dQ2"), ("K2", "dK2")):
         check_grad_heads(to_f64(outs[k][..., :160]), ref[name], name)
         assert bool((outs[k][..., 160:] == 5.0).all()), f"{name} wrote beyond its head dim"
+
+
+# ---------------------------------------------------------------- NEXT-3: the multicast pair plan of the forward
+@pytest.mark.parametrize("causal", [False, True])
+@pytest.mark.parametrize("d1,d2", [(128, 128), (128, 64), (64, 64), (192, 64), (256, 256), (96, 40)])
+def test_multicast_pair_plan_is_bit_identical(d1, d2, causal):
+    """STREAMKL_FWD_MULTICAST: clusters of two CTAs share one multicast K stream.  Same arithmetic in the same order per row, so
+    kl / lse must equal the single-CTA plan bit for bit -- and both match the oracle.  Odd tile counts (a pair with one tile),
+    ragged tails, NQ != NK, shared K heads and many steps (ring wrap-around) are covered."""
+    import torch
+
+    import paper_2606_20005_b200 as skl
+
+    for idx, (B, H, HK, NQ, NK) in enumerate([(1, 2, 2, 333, 555), (2, 4, 2, 640, 1500), (1, 1, 1, 129, 129), (1, 2, 2, 2100, 2100)]):
+        cfg = W.Config(120 + idx, f"mc{d1}x{d2}", B, H, NQ, NK, d1, d2, "bf16", causal)
+        inp = W.all_inputs(cfg)
+        if HK != H:
+            inp["K1"] = np.ascontiguousarray(inp["K1"][:, :HK])
+            inp["K2"] = np.ascontiguousarray(inp["K2"][:, :HK])
+        dev = [to_torch(inp[k]) for k in ("Q1", "K1", "Q2", "K2")]
+        single = skl.streamkl_fwd(*dev, cfg.c1, cfg.c2, causal)
+        skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_MULTICAST)
+        try:
+            pair = skl.streamkl_fwd(*dev, cfg.c1, cfg.c2, causal)
+            torch.cuda.synchronize()
+        finally:
+            skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_SINGLE)
+        for a, b, name in zip(single, pair, ("kl", "lse1", "lse2")):
+            assert torch.equal(a, b), f"{cfg.name} case {idx}: {name} differs between the plans"
+        G = H // HK
+        f = {k: W.widen_f64(inp[k]) for k in ("Q1", "K1", "Q2", "K2")}
+        ref = attention_kl(f["Q1"], np.repeat(f["K1"], G, axis=1), f["Q2"], np.repeat(f["K2"], G, axis=1), cfg.c1, cfg.c2, causal)
+        check_fwd(*(to_f64(t) for t in pair), ref, f"{cfg.name} case {idx} multicast")
