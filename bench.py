@@ -477,6 +477,7 @@ def main():
     ap.add_argument("--workload", default="cfg4", choices=sorted(WORKLOADS) + list(SIDE_LEGS))
     ap.add_argument("--nq", type=int, default=0, help="--workload bwd-strategies: only this N_Q")
     ap.add_argument("--iters", type=int, default=20, help="--workload splitk / bwd-strategies: timed calls per point")
+    ap.add_argument("--dims", default="", help="--workload wide-dims: only this head-dim pair 'd1,d2' (all four gradients)")
     ap.add_argument("--no-also", action="store_true", help="skip the secondary measurements (cfg3, cfg2, cfg5, split-K, strategy table)")
     ap.add_argument("--bwd-mode", default="auto", choices=sorted(BWD_MODES), help="backward strategy of the timed step (streamkl_set_bwd_mode)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
@@ -495,7 +496,11 @@ def main():
         if args.workload == "splitk":
             out = time_splitk(skl, iters=args.iters)
         elif args.workload == "wide-dims":
-            out = time_wide_dims(skl)
+            pairs = None
+            if args.dims:
+                d1, d2 = (int(x) for x in args.dims.split(","))
+                pairs = ((d1, d2, True),)
+            out = time_wide_dims(skl, pairs=pairs)
         else:
             out = time_bwd_strategies(skl, iters=args.iters, nqs=(args.nq,) if args.nq > 0 else (16, 128, 256, 512, 1024, 4096))
         if rank == 0:
