@@ -157,3 +157,78 @@ def test_multicast_pair_plan_is_bit_identical(d1, d2, causal):
         f = {k: W.widen_f64(inp[k]) for k in ("Q1", "K1", "Q2", "K2")}
         ref = attention_kl(f["Q1"], np.repeat(f["K1"], G, axis=1), f["Q2"], np.repeat(f["K2"], G, axis=1), cfg.c1, cfg.c2, causal)
         check_fwd(*(to_f64(t) for t in pair), ref, f"{cfg.name} case {idx} multicast")
+
+
+# ---------------------------------------------------------------- larger sizes, graph capture, concurrent streams
+@pytest.mark.parametrize("d1,d2,teacher,causal", [(192, 64, True, True), (256, 256, False, False), (192, 128, True, True)])
+def test_wide_bench_sized_head(d1, d2, teacher, causal):
+    """One head at a bench-like length (N = 6000: 47 Q tiles, 94 streamed 64-row steps per owner tile, hundreds of ring
+    wrap-arounds), every output row and all of dK against the oracle."""
+    _run(W.Config(130, f"wide-big{d1}x{d2}", 1, 1, 6000, 6000, d1, d2, "bf16", causal), teacher=teacher, both_modes=False)
+
+
+def test_wide_and_multicast_kernels_are_graph_capturable_and_deterministic():
+    """The wide kernels (several passes) and the cluster launch of the multicast plan only enqueue work on the caller's stream:
+    capture fwd + bwd into a CUDA graph; replays reproduce the eager results bit for bit (tile ownership, no atomics)."""
+    import torch
+
+    import paper_2606_20005_b200 as skl
+
+    cfg = W.Config(131, "wide-graph", 1, 2, 700, 900, 256, 192, "bf16", True)
+    inp = W.all_inputs(cfg)
+    Q1, K1, Q2, K2 = (to_torch(inp[k]) for k in ("Q1", "K1", "Q2", "K2"))
+    g = to_torch(inp["g"])
+    kl, l1, l2 = skl.streamkl_fwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, True)
+    eager = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, True, kl, l1, l2, g, teacher=True)
+    ws = torch.empty(skl.streamkl_bwd_workspace_bytes(cfg.B, cfg.H, cfg.NQ, cfg.NK, cfg.d1, cfg.d2, True), dtype=torch.uint8, device="cuda")
+    outs = [torch.zeros_like(t) for t in (kl, l1, l2)]
+    grads = [torch.zeros_like(t) for t in eager]
+    torch.cuda.synchronize()
+    skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_MULTICAST)
+    try:
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            skl.streamkl_fwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, True, *outs)
+            skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, True, outs[0], outs[1], outs[2], g, teacher=True, dQ1=grads[0],
+                             dK1=grads[1], dQ2=grads[2], dK2=grads[3], workspace=ws)
+    finally:
+        skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_SINGLE)
+    for _ in range(2):
+        for t in outs + grads:
+            t.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(outs[0], kl) and torch.equal(outs[1], l1) and torch.equal(outs[2], l2)
+        for a, b in zip(grads, eager):
+            assert torch.equal(a, b)
+
+
+def test_concurrent_streams_do_not_interfere():
+    """Two different problems (a wide one and a fixed-plan one) enqueued back to back on two streams, several rounds: each
+    stream's results equal those of the same call made alone (the library keeps no cross-call device state)."""
+    import torch
+
+    import paper_2606_20005_b200 as skl
+
+    cfgs = [W.Config(132, "cs-wide", 1, 2, 900, 900, 192, 64, "bf16", True), W.Config(133, "cs-narrow", 1, 3, 1100, 1300, 128, 128, "bf16", False)]
+    devs, alone = [], []
+    for cfg in cfgs:
+        inp = W.all_inputs(cfg)
+        d = [to_torch(inp[k]) for k in ("Q1", "K1", "Q2", "K2")] + [to_torch(inp["g"])]
+        devs.append(d)
+        f = skl.streamkl_fwd(*d[:4], cfg.c1, cfg.c2, cfg.causal)
+        b = skl.streamkl_bwd(*d[:4], cfg.c1, cfg.c2, cfg.causal, *f, d[4], teacher=True)
+        alone.append((f, b))
+    torch.cuda.synchronize()
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    for _ in range(3):
+        res = []
+        for cfg, d, st in zip(cfgs, devs, streams):
+            with torch.cuda.stream(st):
+                f = skl.streamkl_fwd(*d[:4], cfg.c1, cfg.c2, cfg.causal, stream=st)
+                b = skl.streamkl_bwd(*d[:4], cfg.c1, cfg.c2, cfg.causal, *f, d[4], teacher=True, stream=st)
+            res.append((f, b))
+        torch.cuda.synchronize()
+        for (f, b), (f0, b0) in zip(res, alone):
+            for x, y in zip(list(f) + list(b), list(f0) + list(b0)):
+                assert torch.equal(x, y)
