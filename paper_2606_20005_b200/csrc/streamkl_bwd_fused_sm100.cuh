@@ -299,7 +299,6 @@ streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const 
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(&s_empty[par]);
-      if (last >= 0) drain(last);             // the previous step of this group: its dQ2^T MMAs have had a whole step to finish
       const int y0 = j * C::BY + half * 32;
       // warp-uniform: causal diagonal blocks, and the owner tile's KEY tail (TMA zero-fills those rows, P = exp2(0 - lse) may
       // be inf there, and unlike the separate K-owner kernel this kernel CONTRACTS over the owned keys: dQ2^T = K2^T dS2)
@@ -311,6 +310,9 @@ streamkl_bwd_fused_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const 
         ds_row<32, TPASS, true, CAUSAL, decltype(m)::value, !TPASS, decltype(h)::value, decltype(r)::value>(
             r1, r2, f1, f2, sc1, sc2, 0.f, 0.f, 0.f, stat, xrow, y0, off, p.NK);
       });
+      // the previous step of this group: its dQ2^T MMAs were issued when the group signalled ds_full and have had this step's
+      // whole dS computation to finish (draining right after the logit load stalled ~600 cycles per step on dq_full: ncu)
+      if (last >= 0) drain(last);
       mbar_wait(&ds_empty[par], (u & 1) ^ 1);   // the MMAs of step it-2 have consumed both copies of this dS2 stage
       tc_fence_after();
       tmem_st16(ds_taddr, o2);
