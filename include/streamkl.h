@@ -182,9 +182,14 @@ int streamkl_set_bwd_mode(int mode);
  *                            refilled once both CTAs' MMAs on it have retired.  Half the L2 -> SM traffic; bit-identical
  *                            results.  Measured on B200 it is a tie for head dims <= 128 and 6-8 % slower above (the pair
  *                            runs in lock step on a shallow ring), which is why it is not the default.
+ *   STREAMKL_FWD_PAIR_MMA  : head dims above 128 only (ignored otherwise): the pair issues ONE tcgen05.mma.cta_group::2 per K-slice --
+ *                            M = 256 (each CTA's 128 query rows, logits into each CTA's own TMEM), each CTA holding 64 of the 128 keys of
+ *                            a K-block, so the K ring beside the (up to 128 KB) Q tile is twice as deep and the stream per CTA half as
+ *                            wide.  Bit-identical results.  Measured: +2 % at d = 256/256, 5-15 % slower at 192/64 ... 256/128: not the
+ *                            default either.
  * Returns STREAMKL_OK, or STREAMKL_ERR_SHAPE for an unknown plan.
  */
-enum { STREAMKL_FWD_SINGLE = 0, STREAMKL_FWD_MULTICAST = 1 };
+enum { STREAMKL_FWD_SINGLE = 0, STREAMKL_FWD_MULTICAST = 1, STREAMKL_FWD_PAIR_MMA = 2 };
 int streamkl_set_fwd_plan(int plan);
 
 /* Bytes of device scratch streamkl_bwd needs for this shape UNDER THE CALLING THREAD'S CURRENT MODE (O((NQ+NK)*d) at most,

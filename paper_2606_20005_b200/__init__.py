@@ -19,6 +19,7 @@ from .binding import (  # noqa: F401
     streamkl_set_fwd_plan,
     STREAMKL_FWD_SINGLE,
     STREAMKL_FWD_MULTICAST,
+    STREAMKL_FWD_PAIR_MMA,
     STREAMKL_BWD_AUTO,
     STREAMKL_BWD_SEPARATE,
     STREAMKL_BWD_FUSED,

@@ -497,7 +497,7 @@ size_t streamkl_bwd_workspace_bytes(int B, int H, int NQ, int, int d1, int d2, i
 }
 
 int streamkl_set_fwd_plan(int plan) {
-  if (plan != STREAMKL_FWD_SINGLE && plan != STREAMKL_FWD_MULTICAST) return STREAMKL_ERR_SHAPE;
+  if (plan != STREAMKL_FWD_SINGLE && plan != STREAMKL_FWD_MULTICAST && plan != STREAMKL_FWD_PAIR_MMA) return STREAMKL_ERR_SHAPE;
   g_fwd_plan = plan;
   return STREAMKL_OK;
 }

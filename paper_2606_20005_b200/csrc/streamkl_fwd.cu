@@ -10,21 +10,23 @@ static_assert(skl::FwdCfg<128, 128>::BQ == kFwdBQ && skl::FwdCfg<64, 64>::BK == 
 // splits == 1: the default kernel (grid (bsz, T_Q)).  splits > 1: split-K (grid (bsz, T_Q, W), partial
 // statistics to `part`, then the reduce kernel).
 // D1 = D2 = 0: the BLOCKED plan with run-time K-block counts (a head dim above 128, padded to 192 / 256).
-template <int D1, int D2, bool CAUSAL, bool SPLIT = false, bool MC = false>
+template <int D1, int D2, bool CAUSAL, bool SPLIT = false, bool MC = false, bool P2 = false>
 int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, float* kl, float* lse1,
                   float* lse2, cudaStream_t stream, int splits = 1, float* part = nullptr) {
   using C = skl::FwdCfg<D1, D2>;
   CUtensorMap tm[4];
-  if (!make_maps(tm, Q1, K1, Q2, K2, s, C::BM, C::BK, f16)) return STREAMKL_ERR_CUDA;
+  // (cta_group::2 plan: each CTA of a pair loads its own 64 keys of every 128-key block)
+  if (!make_maps(tm, Q1, K1, Q2, K2, s, C::BM, P2 ? C::BK / 2 : C::BK, f16)) return STREAMKL_ERR_CUDA;
   const CUtensorMap &tQ1 = tm[0], &tK1 = tm[1], &tQ2 = tm[2], &tK2 = tm[3];
-  auto kern = skl::streamkl_fwd_sm100_kernel<D1, D2, CAUSAL, SPLIT, MC>;
+  auto kern = skl::streamkl_fwd_sm100_kernel<D1, D2, CAUSAL, SPLIT, MC, P2>;
   skl::FwdParams p;
   p.kb1 = pad_dim(s.d1) / 64; p.kb2 = pad_dim(s.d2) / 64; p.nring = 0;
   int smem_bytes = 0;
   if constexpr (C::BLOCKED) {
-    p.nring = C::ring_blocks(p.kb1, p.kb2);
+    const int slot = P2 ? C::KBLK / 2 : C::KBLK;
+    p.nring = C::ring_blocks(p.kb1, p.kb2, slot);
     if (p.nring < 2) return STREAMKL_ERR_SHAPE;
-    smem_bytes = C::smem_bytes(p.kb1, p.kb2);
+    smem_bytes = C::smem_bytes(p.kb1, p.kb2, slot);
   } else {
     smem_bytes = C::SMEM_BYTES;
   }
@@ -42,11 +44,11 @@ int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2
   p.chunk_steps = SPLIT ? (TK + splits - 1) / splits : TK;       // C_K = ceil(N_K / W), in whole BK-key steps
   p.W = SPLIT ? (TK + p.chunk_steps - 1) / p.chunk_steps : 1;    // no empty trailing chunk
   p.part = part;
-  const long long grid = MC ? 2LL * ((p.TQ + 1) / 2) * s.BH : (long long)p.TQ * s.BH * p.W;
+  const long long grid = (MC || P2) ? 2LL * ((p.TQ + 1) / 2) * s.BH : (long long)p.TQ * s.BH * p.W;
   if (grid > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
   {
     ProfScope ps(SPLIT ? KID_FWD_SPLITK_TC : KID_FWD_TC, stream);
-    if constexpr (MC) {   // clusters of two CTAs: the Q tiles (2i, 2i+1) of a head share one multicast K stream
+    if constexpr (MC || P2) {   // clusters of two CTAs: the Q tiles (2i, 2i+1) of a head share one multicast K stream
       cudaLaunchConfig_t cfg = {};
       cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3(C::THREADS); cfg.dynamicSmemBytes = size_t(smem_bytes); cfg.stream = stream;
       cudaLaunchAttribute at[1];
@@ -80,6 +82,10 @@ int fwd_tc_launch(const void* Q1, const void* K1, const void* Q2, const void* K2
   if (p1 > 128 || p2 > 128) p1 = p2 = 0;   // a wide head dim: the BLOCKED plan (run-time K-block counts)
   // the multicast pair plan (streamkl_set_fwd_plan): the default grid only, and only when a head has a second Q tile to pair
   const bool mc = g_fwd_plan == STREAMKL_FWD_MULTICAST && splits <= 1 && s.NQ > skl::FwdCfg<64, 64>::BQ;
+  // the cta_group::2 plan: wide head dims only (BLOCKED plan), default grid
+  if (g_fwd_plan == STREAMKL_FWD_PAIR_MMA && splits <= 1 && p1 == 0 && s.NQ > skl::FwdCfg<64, 64>::BQ)
+    return s.causal ? launch_fwd_tc<0, 0, true, false, false, true>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream)
+                    : launch_fwd_tc<0, 0, false, false, false, true>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream);
 #define SKL_FWD_MC_CASE(A, Bd)                                                                                                    \
   if (mc && p1 == A && p2 == Bd)                                                                                                  \
     return s.causal ? launch_fwd_tc<A, Bd, true, false, true>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream)                     \

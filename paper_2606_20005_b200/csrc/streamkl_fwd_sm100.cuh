@@ -94,11 +94,15 @@ struct FwdCfg<0, 0> {
   static constexpr uint32_t TMEM_COLS = 512;
   static constexpr uint32_t POLY_MASK = STREAMKL_FWD_POLY_MASK_WIDE;
   // ring blocks that fit beside the resident Q tile (host side)
-  static constexpr int ring_blocks(int kb1, int kb2) {
-    const int r = (SMEM_LIMIT - 1024 - AUX_BYTES - (kb1 + kb2) * QBLK) / KBLK;
-    return r > MAX_RING ? MAX_RING : r;
+  // (`slot` = bytes of a ring entry: a whole K-block, or this CTA's half of it under the cta_group::2 plan, whose ring may have 16 entries)
+  static constexpr int ring_blocks(int kb1, int kb2, int slot = KBLK) {
+    const int r = (SMEM_LIMIT - 1024 - AUX_BYTES - (kb1 + kb2) * QBLK) / slot;
+    const int cap = slot == KBLK ? MAX_RING : 16;
+    return r > cap ? cap : r;
   }
-  static constexpr int smem_bytes(int kb1, int kb2) { return 1024 + (kb1 + kb2) * QBLK + ring_blocks(kb1, kb2) * KBLK + AUX_BYTES; }
+  static constexpr int smem_bytes(int kb1, int kb2, int slot = KBLK) {
+    return 1024 + (kb1 + kb2) * QBLK + ring_blocks(kb1, kb2, slot) * slot + AUX_BYTES;
+  }
 };
 
 struct FwdParams {
@@ -255,7 +259,13 @@ __device__ __noinline__ RowState safe_step(uint32_t taddr, RowState st, float sc
 // producer loads half of every stage's K-blocks and multicasts them into both CTAs' rings (half the L2 -> SM traffic per
 // tile pair; SURVEY 8(f) NEXT-3 "2-CTA / multicast variants").  Both CTAs run the K pipeline for the pair's longer step
 // count; a stage is reloaded only after BOTH issuers' MMAs on it have retired (k_empty counts two multicast commits).
-template <int D1, int D2, bool CAUSAL, bool SPLIT = false, bool MC = false>
+// P2 (BLOCKED plan only): the two CTAs of a cluster pair issue ONE `tcgen05.mma.cta_group::2` per K-slice -- M = 256 (each CTA's
+// 128 query rows, logits into each CTA's own TMEM), N = 128 keys of which each CTA holds 64 in its shared memory.  A K-block costs each
+// CTA 8 KB instead of 16 (the ring beside a 128 KB Q tile is twice as deep, the L2 -> SM stream per CTA half as wide).  Rank 0 is
+// the leader: its issuer warp issues every MMA, all TMA loads of both CTAs complete on ITS full barriers, its commits are multicast
+// to both CTAs' k_empty / s_full, and both CTAs' softmax warps arrive on ITS s_empty.  Both CTAs run the pair's longer step count; a
+// CTA past its own causal frontier sees fully masked steps.
+template <int D1, int D2, bool CAUSAL, bool SPLIT = false, bool MC = false, bool P2 = false>
 __global__ void __launch_bounds__(FwdCfg<D1, D2>::THREADS, 1)
 streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid_constant__ CUtensorMap tmK1,
                           const __grid_constant__ CUtensorMap tmQ2, const __grid_constant__ CUtensorMap tmK2, const FwdParams p) {
@@ -264,10 +274,12 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   const int KB1 = C::BLOCKED ? p.kb1 : C::KB1, KB2 = C::BLOCKED ? p.kb2 : C::KB2;
   const int NRING = C::BLOCKED ? p.nring : C::NSTAGE;      // ring entries: whole stages, or single K-blocks (BLOCKED)
+  constexpr int SLOT_BYTES = P2 ? C::KBLK / 2 : C::STAGE_BYTES;   // P2: this CTA's 64 keys of a K-block
+  constexpr bool PAIRED = MC || P2;
   uint8_t* sQ1 = smem;
   uint8_t* sQ2 = sQ1 + KB1 * C::QBLK;
   uint8_t* sK = smem + (KB1 + KB2) * C::QBLK;
-  uint64_t* bars = reinterpret_cast<uint64_t*>(sK + NRING * C::STAGE_BYTES);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(sK + NRING * SLOT_BYTES);
   uint64_t* q_full = bars;                    // 1
   uint64_t* k_full = bars + 1;                // NRING
   uint64_t* k_empty = k_full + NRING;         // NRING
@@ -277,28 +289,32 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   // heavy (late, causal) query tiles first within each head; consecutive CTAs share a head (K stays in L2)
-  static_assert(!(MC && SPLIT), "the multicast pair plan exists for the default grid");
-  const int tile = SPLIT ? int(blockIdx.x) / p.W : (MC ? int(blockIdx.x) >> 1 : int(blockIdx.x));
+  static_assert(!(PAIRED && SPLIT) && !(MC && P2) && !(P2 && !C::BLOCKED), "the pair plans exist for the default grid; P2 for the BLOCKED plan");
+  const int tile = SPLIT ? int(blockIdx.x) / p.W : (PAIRED ? int(blockIdx.x) >> 1 : int(blockIdx.x));
   const int wk = SPLIT ? int(blockIdx.x) % p.W : 0;          // key chunk of this CTA (split-K grid (b, i, w))
-  const int crank = MC ? int(blockIdx.x) & 1 : 0;            // rank within the cluster pair
-  const int TQU = MC ? (p.TQ + 1) / 2 : p.TQ;                // scheduling units per head: Q tiles, or pairs of them
+  const int crank = PAIRED ? int(blockIdx.x) & 1 : 0;        // rank within the cluster pair
+  const int TQU = PAIRED ? (p.TQ + 1) / 2 : p.TQ;            // scheduling units per head: Q tiles, or pairs of them
   const int bh = tile / TQU;
   const int hq = bh % p.H, bq = bh / p.H, hk = hq / p.G;      // TMA coordinates {d, row, head, batch}
-  // MC: pair u (heavy first) = tiles TQ-1-2u (rank 0) and TQ-2-2u (rank 1; absent for the last pair of an odd TQ)
-  const int qt = MC ? p.TQ - 1 - 2 * (tile % TQU) - crank : p.TQ - 1 - (tile % p.TQ);
+  // pairs: pair u (heavy first) = tiles TQ-1-2u (rank 0) and TQ-2-2u (rank 1; absent for the last pair of an odd TQ)
+  const int qt_raw = PAIRED ? p.TQ - 1 - 2 * (tile % TQU) - crank : p.TQ - 1 - (tile % p.TQ);
+  const bool has_tile = qt_raw >= 0;
+  const int qt = (P2 && !has_tile) ? 0 : qt_raw;             // P2: an absent partner still consumes its TMEM stages: it recomputes tile 0, stores nothing
   const int q0 = qt * C::BQ;
   const int off = p.NK - p.NQ;
   const int TK = (p.NK + C::BK - 1) / C::BK;
   const int j_begin = SPLIT ? wk * p.chunk_steps : 0;        // this CTA's 128-key steps are [j_begin, j_begin + nsteps)
   int j_end = SPLIT ? min(TK, j_begin + p.chunk_steps) : TK;
   if (CAUSAL) j_end = min(j_end, min(p.NK - 1, q0 + C::BM - 1 + off) / C::BK + 1);   // past the tile's causal frontier
-  const int nsteps = (MC && qt < 0) ? 0 : max(0, j_end - j_begin);
-  // MC: steps of the K pipeline both CTAs run = the pair's longer count (rank 0 owns the later tile: never the shorter one)
-  int nsteps_pair = nsteps;
-  if (MC) {
-    const int q0a = (qt + crank) * C::BQ;                    // rank 0's tile
+  // pairs: steps of the K pipeline both CTAs run = the pair's longer count (rank 0 owns the later tile: never the shorter one)
+  int nsteps_pair = max(0, j_end - j_begin);
+  if (PAIRED) {
+    const int q0a = (qt_raw + crank) * C::BQ;                // rank 0's tile
     nsteps_pair = CAUSAL ? min(TK, min(p.NK - 1, q0a + C::BM - 1 + off) / C::BK + 1) : TK;
   }
+  // MC: a CTA computes its own steps only (an absent partner none).  P2: the MMAs are the pair's, so every role of both CTAs runs the
+  // pair's count (steps past a CTA's own frontier are fully masked for its rows)
+  const int nsteps = P2 ? nsteps_pair : ((MC && !has_tile) ? 0 : max(0, j_end - j_begin));
 
   if (warp == 0 && lane == 0) {
     tma_prefetch_desc(&tmQ1); tma_prefetch_desc(&tmK1); tma_prefetch_desc(&tmQ2); tma_prefetch_desc(&tmK2);
@@ -306,13 +322,15 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
   if (warp == 1 && lane == 0) {
     mbar_init(q_full, 1);
     for (int s = 0; s < NRING; ++s) { mbar_init(&k_full[s], 1); mbar_init(&k_empty[s], MC ? 2 : 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&s_full[i], 1); mbar_init(&s_empty[i], 4 * C::NGRP); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&s_full[i], 1); mbar_init(&s_empty[i], (P2 ? 2 : 1) * 4 * C::NGRP); }   // P2: both CTAs' softmax warps
     fence_mbar_init();
   }
-  if (warp == 2) tmem_alloc<C::TMEM_COLS>(tmem_ptr);
+  if (warp == 2) {
+    if constexpr (P2) tmem_alloc_pair<C::TMEM_COLS>(tmem_ptr); else tmem_alloc<C::TMEM_COLS>(tmem_ptr);
+  }
   tc_fence_before();
   __syncthreads();
-  if (MC) cluster_sync_all();   // the peer's barriers exist before anything is multicast to them
+  if (PAIRED) cluster_sync_all();   // the peer's barriers exist before anything is multicast to them
   tc_fence_after();
   const uint32_t tmem_base = *tmem_ptr;
 
@@ -320,6 +338,29 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
    reg_dealloc<24>();   // (pool: (96-24)*128 = 9216 >= (112-96)*512) producer / MMA / allocator warpgroup gives its registers to the softmax warpgroups
    if (warp == 0) {
     // ===================== TMA producer =====================
+    if constexpr (P2) {
+      if (lane == 0 && nsteps > 0) {
+        const uint64_t pol_q = l2_policy_evict_first(), pol_k = l2_policy_evict_last();
+        // every load of both CTAs completes on the LEADER's barrier, which expects both CTAs' bytes
+        const uint32_t lq = mapa_shared(q_full, 0);
+        if (crank == 0) mbar_arrive_expect_tx(q_full, uint32_t(2 * (KB1 + KB2) * C::QBLK));
+        for (int kb = 0; kb < KB1; ++kb) tma_load_4d_pair(sQ1 + kb * C::QBLK, &tmQ1, lq, kb * 64, q0, hq, bq, pol_q);
+        for (int kb = 0; kb < KB2; ++kb) tma_load_4d_pair(sQ2 + kb * C::QBLK, &tmQ2, lq, kb * 64, q0, hq, bq, pol_q);
+        int slot = 0;
+        uint32_t ph = 0;
+        for (int j = 0; j < nsteps; ++j) {
+          for (int b = 0; b < KB1 + KB2; ++b) {
+            mbar_wait(&k_empty[slot], ph ^ 1);                       // (the leader's commit, multicast to both CTAs)
+            if (crank == 0) mbar_arrive_expect_tx(&k_full[slot], uint32_t(2 * SLOT_BYTES));
+            const bool one = b < KB1;
+            // this CTA's 64 keys of the 128-key block (the K maps of this plan have 64-row boxes)
+            tma_load_4d_pair(sK + slot * SLOT_BYTES, one ? &tmK1 : &tmK2, mapa_shared(&k_full[slot], 0), (one ? b : b - KB1) * 64,
+                             j * C::BK + crank * (C::BK / 2), hk, bq, pol_k);
+            if (++slot == NRING) { slot = 0; ph ^= 1; }
+          }
+        }
+      }
+    } else
     if (lane == 0 && (MC ? nsteps_pair : nsteps) > 0) {
       const uint64_t pol_q = l2_policy_evict_first(), pol_k = l2_policy_evict_last();
       if (nsteps > 0) {
@@ -403,6 +444,36 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
     const uint64_t dq1 = umma_smem_desc_sw128(smem_u32(sQ1), 16, 1024);
     const uint64_t dq2 = umma_smem_desc_sw128(smem_u32(sQ2), 16, 1024);
     const uint64_t dk = umma_smem_desc_sw128(smem_u32(sK), 16, 1024);
+    if constexpr (P2) {
+      if (crank == 0 && nsteps > 0) {       // the leader issues the pair's MMAs
+        const uint32_t idesc2 = umma_idesc_16(2 * C::BM, C::BK, 0, 0, p.fmt16);
+        mbar_wait(q_full, 0);
+        tc_fence_after();
+        int slot = 0;
+        uint32_t ph = 0;
+        for (int j = 0; j < nsteps; ++j) {
+          const int st = j & 1;
+          mbar_wait(&s_empty[st], ((j >> 1) & 1) ^ 1);       // both CTAs' softmax warps are done with the stage
+          const uint32_t dS1 = tmem_base + st * (2 * C::BK);
+          for (int b = 0; b < KB1 + KB2; ++b) {
+            mbar_wait(&k_full[slot], ph);                    // both halves of the block have landed
+            tc_fence_after();
+            const bool one = b < KB1;
+            const uint32_t first = (b == 0 || b == KB1) ? 0u : 1u;
+            uint64_t a = dq1 + uint64_t((b * C::QBLK) >> 4), bk = dk + uint64_t((slot * SLOT_BYTES) >> 4);
+            if (elect_one()) {
+#pragma unroll
+              for (int k = 0; k < 4; ++k)
+                umma_bf16_ss_pair(one ? dS1 : dS1 + C::BK, a + uint64_t((k * 32) >> 4), bk + uint64_t((k * 32) >> 4), idesc2, first | uint32_t(k != 0));
+              umma_commit_pair(&k_empty[slot], uint16_t(3));
+              if (b + 1 == KB1 + KB2) umma_commit_pair(&s_full[st], uint16_t(3));
+            }
+            __syncwarp();
+            if (++slot == NRING) { slot = 0; ph ^= 1; }
+          }
+        }
+      }
+    } else {
     if (nsteps > 0) {
       mbar_wait(q_full, 0);
       tc_fence_after();
@@ -478,6 +549,7 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
       }
       __syncwarp();
     }
+    }   // (!P2)
    }
   } else {
     // ===================== softmax warps =====================
@@ -503,7 +575,10 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
     auto release = [&](uint64_t* empty_bar) {   // every tcgen05.ld of this warp on the stage has completed (wait::ld)
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(empty_bar);
+      if (lane == 0) {
+        if (P2 && crank != 0) mbar_arrive_cluster(mapa_shared(empty_bar, 0));   // the pair's stage is free when BOTH CTAs are done: the leader counts
+        else mbar_arrive(empty_bar);
+      }
     };
 
     const bool relu2 = p.act2 == 1;
@@ -622,7 +697,7 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
         x[3 * C::BM + rloc] = pl2; x[4 * C::BM + rloc] = pacc;
       }
       asm volatile("bar.sync 1, %0;" ::"n"(C::NGRP * 128) : "memory");
-      if (grp == 0 && row < p.NQ) {
+      if (grp == 0 && row < p.NQ && has_tile) {
         float m1 = st.m1, m2 = st.m2, l1 = pl1, l2 = pl2, acc = pacc;
 #pragma unroll
         for (int hb = 1; hb < C::NGRP; ++hb) {
@@ -658,10 +733,10 @@ streamkl_fwd_sm100_kernel(const __grid_constant__ CUtensorMap tmQ1, const __grid
   }
   tc_fence_before();
   __syncthreads();
-  if (MC) cluster_sync_all();   // neither CTA leaves while the other may still multicast into its ring or arrive on its barriers
+  if (PAIRED) cluster_sync_all();   // neither CTA leaves while the other may still write into its ring / TMEM or arrive on its barriers
   if (warp == 2) {
     tc_fence_after();
-    tmem_dealloc<C::TMEM_COLS>(tmem_base);
+    if constexpr (P2) tmem_dealloc_pair<C::TMEM_COLS>(tmem_base); else tmem_dealloc<C::TMEM_COLS>(tmem_base);
   }
 }
 

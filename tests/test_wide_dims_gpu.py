@@ -126,26 +126,29 @@ def test_wide_gradient_padding_columns_are_left_untouched():
         assert bool((outs[k][..., 160:] == 5.0).all()), f"{name} wrote beyond its head dim"
 
 
-# ---------------------------------------------------------------- NEXT-3: the multicast pair plan of the forward
+# ---------------------------------------------------------------- NEXT-3: the two CTA-pair plans of the forward
+@pytest.mark.parametrize("plan", ["multicast", "pair_mma"])
 @pytest.mark.parametrize("causal", [False, True])
-@pytest.mark.parametrize("d1,d2", [(128, 128), (128, 64), (64, 64), (192, 64), (256, 256), (96, 40)])
-def test_multicast_pair_plan_is_bit_identical(d1, d2, causal):
-    """STREAMKL_FWD_MULTICAST: clusters of two CTAs share one multicast K stream.  Same arithmetic in the same order per row, so
-    kl / lse must equal the single-CTA plan bit for bit -- and both match the oracle.  Odd tile counts (a pair with one tile),
-    ragged tails, NQ != NK, shared K heads and many steps (ring wrap-around) are covered."""
+@pytest.mark.parametrize("d1,d2", [(128, 128), (128, 64), (64, 64), (192, 64), (256, 256), (96, 40), (200, 136)])
+def test_cta_pair_plans_are_bit_identical(d1, d2, causal, plan):
+    """STREAMKL_FWD_MULTICAST: clusters of two CTAs share one TMA-multicast K stream.  STREAMKL_FWD_PAIR_MMA (head dims above 128; the
+    plan is ignored below): the pair issues one `tcgen05.mma.cta_group::2` per K-slice, M = 256, each CTA holding 64 of the 128 keys.
+    Same arithmetic in the same order per row, so kl / lse must equal the single-CTA plan bit for bit -- and match the oracle.  Odd
+    tile counts (a pair with one tile), ragged tails, NQ != NK, shared K heads and many steps (ring wrap-around) are covered."""
     import torch
 
     import paper_2606_20005_b200 as skl
 
+    code = skl.STREAMKL_FWD_MULTICAST if plan == "multicast" else skl.STREAMKL_FWD_PAIR_MMA
     for idx, (B, H, HK, NQ, NK) in enumerate([(1, 2, 2, 333, 555), (2, 4, 2, 640, 1500), (1, 1, 1, 129, 129), (1, 2, 2, 2100, 2100)]):
-        cfg = W.Config(120 + idx, f"mc{d1}x{d2}", B, H, NQ, NK, d1, d2, "bf16", causal)
+        cfg = W.Config(120 + idx, f"pair{d1}x{d2}", B, H, NQ, NK, d1, d2, "bf16", causal)
         inp = W.all_inputs(cfg)
         if HK != H:
             inp["K1"] = np.ascontiguousarray(inp["K1"][:, :HK])
             inp["K2"] = np.ascontiguousarray(inp["K2"][:, :HK])
         dev = [to_torch(inp[k]) for k in ("Q1", "K1", "Q2", "K2")]
         single = skl.streamkl_fwd(*dev, cfg.c1, cfg.c2, causal)
-        skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_MULTICAST)
+        skl.streamkl_set_fwd_plan(code)
         try:
             pair = skl.streamkl_fwd(*dev, cfg.c1, cfg.c2, causal)
             torch.cuda.synchronize()
@@ -156,7 +159,7 @@ def test_multicast_pair_plan_is_bit_identical(d1, d2, causal):
         G = H // HK
         f = {k: W.widen_f64(inp[k]) for k in ("Q1", "K1", "Q2", "K2")}
         ref = attention_kl(f["Q1"], np.repeat(f["K1"], G, axis=1), f["Q2"], np.repeat(f["K2"], G, axis=1), cfg.c1, cfg.c2, causal)
-        check_fwd(*(to_f64(t) for t in pair), ref, f"{cfg.name} case {idx} multicast")
+        check_fwd(*(to_f64(t) for t in pair), ref, f"{cfg.name} case {idx} {plan}")
 
 
 # ---------------------------------------------------------------- larger sizes, graph capture, concurrent streams
@@ -167,8 +170,8 @@ def test_wide_bench_sized_head(d1, d2, teacher, causal):
     _run(W.Config(130, f"wide-big{d1}x{d2}", 1, 1, 6000, 6000, d1, d2, "bf16", causal), teacher=teacher, both_modes=False)
 
 
-def test_wide_and_multicast_kernels_are_graph_capturable_and_deterministic():
-    """The wide kernels (several passes) and the cluster launch of the multicast plan only enqueue work on the caller's stream:
+def test_wide_and_cta_pair_kernels_are_graph_capturable_and_deterministic():
+    """The wide kernels (several passes) and the cluster launch of a CTA-pair plan only enqueue work on the caller's stream:
     capture fwd + bwd into a CUDA graph; replays reproduce the eager results bit for bit (tile ownership, no atomics)."""
     import torch
 
@@ -184,7 +187,7 @@ def test_wide_and_multicast_kernels_are_graph_capturable_and_deterministic():
     outs = [torch.zeros_like(t) for t in (kl, l1, l2)]
     grads = [torch.zeros_like(t) for t in eager]
     torch.cuda.synchronize()
-    skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_MULTICAST)
+    skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_PAIR_MMA)   # (a wide pair: the cta_group::2 cluster launch is what gets captured)
     try:
         graph = torch.cuda.CUDAGraph()
         with torch.cuda.graph(graph):
