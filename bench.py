@@ -480,7 +480,7 @@ def main():
     ap.add_argument("--dims", default="", help="--workload wide-dims: only this head-dim pair 'd1,d2' (all four gradients)")
     ap.add_argument("--no-also", action="store_true", help="skip the secondary measurements (cfg3, cfg2, cfg5, split-K, strategy table)")
     ap.add_argument("--bwd-mode", default="auto", choices=sorted(BWD_MODES), help="backward strategy of the timed step (streamkl_set_bwd_mode)")
-    ap.add_argument("--fwd-plan", default="single", choices=["single", "multicast", "pair-mma"], help="forward plan (streamkl_set_fwd_plan)")
+    ap.add_argument("--fwd-plan", default="auto", choices=["auto", "multicast", "pair-mma", "persistent", "per-tile"], help="forward plan (streamkl_set_fwd_plan)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer end-to-end leg (profiling runs)")
     args = ap.parse_args()
@@ -494,7 +494,7 @@ def main():
         import paper_2606_20005_b200 as skl
 
         torch.cuda.set_device(local)
-        skl.streamkl_set_fwd_plan({"single": 0, "multicast": 1, "pair-mma": 2}[args.fwd_plan])
+        skl.streamkl_set_fwd_plan({"auto": 0, "multicast": 1, "pair-mma": 2, "persistent": 3, "per-tile": 4}[args.fwd_plan])
         if args.workload == "splitk":
             out = time_splitk(skl, iters=args.iters)
         elif args.workload == "wide-dims":
@@ -531,7 +531,7 @@ def main():
 
     pk = peaks()
     skl.streamkl_set_bwd_mode(BWD_MODES[args.bwd_mode])
-    skl.streamkl_set_fwd_plan({"single": 0, "multicast": 1, "pair-mma": 2}[args.fwd_plan])
+    skl.streamkl_set_fwd_plan({"auto": 0, "multicast": 1, "pair-mma": 2, "persistent": 3, "per-tile": 4}[args.fwd_plan])
     host = gen_inputs(cfg, rank)
     dev = tuple(to_dev(host[k]) for k in ("Q1", "K1", "Q2", "K2", "g"))
     torch.cuda.synchronize()

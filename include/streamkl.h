@@ -175,21 +175,30 @@ enum { STREAMKL_BWD_AUTO = 0, STREAMKL_BWD_SEPARATE = 1, STREAMKL_BWD_FUSED = 2 
 int streamkl_set_bwd_mode(int mode);
 
 /*
- * Forward plan of the default (unsplit) tcgen05 kernel, per calling thread (SURVEY 8(f) NEXT-3 "2-CTA / multicast variants"):
- *   STREAMKL_FWD_SINGLE    : (default) one CTA per 128-row Q tile, each streaming the head's K tiles from L2 on its own.
- *   STREAMKL_FWD_MULTICAST : clusters of two CTAs own the Q tiles (2i, 2i+1) of a head and share ONE K stream -- each CTA's
- *                            producer loads half of every stage's K-blocks with TMA multicast into both rings, a stage is
- *                            refilled once both CTAs' MMAs on it have retired.  Half the L2 -> SM traffic; bit-identical
- *                            results.  Measured on B200 it is a tie for head dims <= 128 and 6-8 % slower above (the pair
- *                            runs in lock step on a shallow ring), which is why it is not the default.
- *   STREAMKL_FWD_PAIR_MMA  : head dims above 128 only (ignored otherwise): the pair issues ONE tcgen05.mma.cta_group::2 per K-slice --
- *                            M = 256 (each CTA's 128 query rows, logits into each CTA's own TMEM), each CTA holding 64 of the 128 keys of
- *                            a K-block, so the K ring beside the (up to 128 KB) Q tile is twice as deep and the stream per CTA half as
- *                            wide.  Bit-identical results.  Measured: +2 % at d = 256/256, 5-15 % slower at 192/64 ... 256/128: not the
- *                            default either.
+ * Forward plan of the default (unsplit) tcgen05 kernel, per calling thread (SURVEY 7.1 step 5 "persistent scheduling", 8(f) NEXT-3
+ * "2-CTA / multicast variants").  Every plan computes each row with the same arithmetic in the same order: results are bit-identical.
+ *   STREAMKL_FWD_AUTO       : (default) PER_TILE, or PERSISTENT where the measured rule says it wins: head dims <= 128, at most 64 key
+ *                             steps per Q tile on average (N_K <= 16K causal, <= 8K unmasked) and at least two Q tiles per SM.
+ *   STREAMKL_FWD_PER_TILE   : one CTA per 128-row Q tile (grid bsz x T_Q), each streaming the head's K tiles on its own.
+ *   STREAMKL_FWD_PERSISTENT : one CTA per SM loops over the Q tiles (same order, taken from an atomic counter): TMEM and barriers are
+ *                             set up once, the next tile's Q / K loads and first MMAs run under the previous tile's last softmax steps.
+ *                             Measured on B200: cfg 3 (16K) forward -3..6 %, cfg 2 (4K) -2..6 %, cfg 4 (64K) +1 % (slower).  Head dims
+ *                             above 128 run PER_TILE.
+ *   STREAMKL_FWD_MULTICAST  : clusters of two CTAs own the Q tiles (2i, 2i+1) of a head and share ONE K stream -- each CTA's
+ *                             producer loads half of every stage's K-blocks with TMA multicast into both rings, a stage is
+ *                             refilled once both CTAs' MMAs on it have retired.  Half the L2 -> SM traffic.  Measured a tie for head
+ *                             dims <= 128 and 6-8 % slower above (the pair runs in lock step on a shallow ring): never chosen by AUTO.
+ *   STREAMKL_FWD_PAIR_MMA   : head dims above 128 only (PER_TILE otherwise): the pair issues ONE tcgen05.mma.cta_group::2 per K-slice --
+ *                             M = 256 (each CTA's 128 query rows, logits into each CTA's own TMEM), each CTA holding 64 of the 128 keys of
+ *                             a K-block, so the K ring beside the (up to 128 KB) Q tile is twice as deep and the stream per CTA half as
+ *                             wide.  Measured: +2 % at d = 256/256, 5-15 % slower at 192/64 ... 256/128: never chosen by AUTO
+ *                             (DESIGN.md 6.1c).
+ * The persistent plan keeps a few bytes of scheduler state per launch in device memory owned by the library (1024 slots used round-robin,
+ * rearmed by the launch itself): launches may overlap freely on any streams unless 1024 of them are in flight at once.
  * Returns STREAMKL_OK, or STREAMKL_ERR_SHAPE for an unknown plan.
  */
-enum { STREAMKL_FWD_SINGLE = 0, STREAMKL_FWD_MULTICAST = 1, STREAMKL_FWD_PAIR_MMA = 2 };
+enum { STREAMKL_FWD_AUTO = 0, STREAMKL_FWD_SINGLE = 0 /* older name of AUTO */, STREAMKL_FWD_MULTICAST = 1, STREAMKL_FWD_PAIR_MMA = 2,
+       STREAMKL_FWD_PERSISTENT = 3, STREAMKL_FWD_PER_TILE = 4 };
 int streamkl_set_fwd_plan(int plan);
 
 /* Bytes of device scratch streamkl_bwd needs for this shape UNDER THE CALLING THREAD'S CURRENT MODE (O((NQ+NK)*d) at most,

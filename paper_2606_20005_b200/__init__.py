@@ -20,6 +20,9 @@ from .binding import (  # noqa: F401
     STREAMKL_FWD_SINGLE,
     STREAMKL_FWD_MULTICAST,
     STREAMKL_FWD_PAIR_MMA,
+    STREAMKL_FWD_PERSISTENT,
+    STREAMKL_FWD_PER_TILE,
+    STREAMKL_FWD_AUTO,
     STREAMKL_BWD_AUTO,
     STREAMKL_BWD_SEPARATE,
     STREAMKL_BWD_FUSED,

@@ -15,7 +15,7 @@ from .build import LIB_PATH
 __all__ = [
     "StreamKLError", "lib", "lib_path", "streamkl_fwd", "streamkl_bwd", "streamkl_bwd_workspace_bytes",
     "streamkl_fwd_splitk", "streamkl_fwd_splitk_splits", "streamkl_fwd_splitk_workspace_bytes",
-    "streamkl_fwd_host", "streamkl_fwd_bwd_host", "streamkl_host_trim", "streamkl_set_bwd_mode", "streamkl_set_fwd_plan", "STREAMKL_FWD_SINGLE", "STREAMKL_FWD_MULTICAST", "STREAMKL_FWD_PAIR_MMA",
+    "streamkl_fwd_host", "streamkl_fwd_bwd_host", "streamkl_host_trim", "streamkl_set_bwd_mode", "streamkl_set_fwd_plan", "STREAMKL_FWD_SINGLE", "STREAMKL_FWD_MULTICAST", "STREAMKL_FWD_PAIR_MMA", "STREAMKL_FWD_PERSISTENT", "STREAMKL_FWD_PER_TILE", "STREAMKL_FWD_AUTO",
     "STREAMKL_BWD_AUTO", "STREAMKL_BWD_SEPARATE", "STREAMKL_BWD_FUSED", "STREAMKL_BF16", "STREAMKL_F16", "STREAMKL_F32", "StreamKLLayout", "streamkl_last_launch_count", "streamkl_strerror",
     "streamkl_profile_enable", "streamkl_profile_collect", "streamkl_kernel_name",
     "streamkl_version",
@@ -31,7 +31,8 @@ class StreamKLLayout(ctypes.Structure):
                 ("k1_stride", ctypes.c_longlong * 3), ("q2_stride", ctypes.c_longlong * 3), ("k2_stride", ctypes.c_longlong * 3),
                 ("student_activation", ctypes.c_int)]
 STREAMKL_BWD_AUTO, STREAMKL_BWD_SEPARATE, STREAMKL_BWD_FUSED = 0, 1, 2
-STREAMKL_FWD_SINGLE, STREAMKL_FWD_MULTICAST, STREAMKL_FWD_PAIR_MMA = 0, 1, 2
+STREAMKL_FWD_SINGLE, STREAMKL_FWD_MULTICAST, STREAMKL_FWD_PAIR_MMA, STREAMKL_FWD_PERSISTENT, STREAMKL_FWD_PER_TILE = 0, 1, 2, 3, 4
+STREAMKL_FWD_AUTO = 0
 
 
 class StreamKLError(RuntimeError):
@@ -114,8 +115,9 @@ def streamkl_version() -> str:
 
 
 def streamkl_set_fwd_plan(plan: int) -> None:
-    """STREAMKL_FWD_SINGLE (default) | STREAMKL_FWD_MULTICAST (cluster pairs sharing one multicast K stream) |
-    STREAMKL_FWD_PAIR_MMA (head dims above 128: cluster pairs issuing cta_group::2 MMAs)."""
+    """STREAMKL_FWD_AUTO (default: per-tile or persistent by a measured rule) | STREAMKL_FWD_PER_TILE | STREAMKL_FWD_PERSISTENT |
+    STREAMKL_FWD_MULTICAST (cluster pairs sharing one multicast K stream) | STREAMKL_FWD_PAIR_MMA (head dims above 128: cluster
+    pairs issuing cta_group::2 MMAs).  All plans give bit-identical results."""
     rc = lib().streamkl_set_fwd_plan(int(plan))
     if rc != 0:
         raise StreamKLError(rc, "streamkl_set_fwd_plan")

@@ -19,7 +19,7 @@
 namespace sklh {
 
 thread_local int g_last_launches = 0;
-thread_local int g_fwd_plan = STREAMKL_FWD_SINGLE;
+thread_local int g_fwd_plan = STREAMKL_FWD_AUTO;
 
 namespace {
 struct ProfRecord { int id; cudaEvent_t a, b; };
@@ -497,7 +497,7 @@ size_t streamkl_bwd_workspace_bytes(int B, int H, int NQ, int, int d1, int d2, i
 }
 
 int streamkl_set_fwd_plan(int plan) {
-  if (plan != STREAMKL_FWD_SINGLE && plan != STREAMKL_FWD_MULTICAST && plan != STREAMKL_FWD_PAIR_MMA) return STREAMKL_ERR_SHAPE;
+  if (plan < STREAMKL_FWD_AUTO || plan > STREAMKL_FWD_PER_TILE) return STREAMKL_ERR_SHAPE;
   g_fwd_plan = plan;
   return STREAMKL_OK;
 }

@@ -1,6 +1,9 @@
 // streamkl_fwd.cu -- launchers of the tcgen05 forward kernel (default grid and split-K + reduce); see streamkl.cu for the C ABI.
 #include "streamkl_host.cuh"
+#include <atomic>
+
 #include "streamkl_fwd_sm100.cuh"
+#include "streamkl_fwd_persist_sm100.cuh"
 
 namespace sklh {
 namespace {
@@ -74,12 +77,75 @@ int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2
   return STREAMKL_OK;
 }
 
+// ---- persistent forward (streamkl_fwd_persist_sm100.cuh): one CTA per SM, dynamic work items
+// Scheduler state of the persistent kernel: {next item, finished CTAs} per slot, zero between launches (the last CTA of a launch
+// rearms its slot).  A launch takes the next slot round-robin, so launches in flight at the same time (other streams, other
+// host threads) do not share one unless 1024 of them overlap.
+constexpr int kSchedSlots = 1024;
+__device__ int g_fwd_sched[kSchedSlots][2];
+std::atomic<unsigned> g_sched_next{0};
+
+template <int D1, int D2, bool CAUSAL>
+int launch_fwd_persist(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, float* kl, float* lse1,
+                       float* lse2, cudaStream_t stream) {
+  using C = skl::FwdPersistCfg<D1, D2>;
+  CUtensorMap tm[4];
+  if (!make_maps(tm, Q1, K1, Q2, K2, s, C::BM, C::BK, f16)) return STREAMKL_ERR_CUDA;
+  auto kern = skl::streamkl_fwd_persist_sm100_kernel<D1, D2, CAUSAL>;
+  int dev = 0, sms = 0;
+  int* sched = nullptr;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+      cudaGetSymbolAddress(reinterpret_cast<void**>(&sched), g_fwd_sched) != cudaSuccess ||
+      cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES) != cudaSuccess) {
+    cudaGetLastError();
+    return STREAMKL_ERR_CUDA;
+  }
+  skl::FwdParams p;
+  p.kb1 = D1 / 64; p.kb2 = D2 / 64; p.nring = 0;
+  p.NQ = s.NQ; p.NK = s.NK; p.BH = int(s.BH);
+  p.H = s.H; p.G = s.G(); p.fmt16 = f16 ? 0u : 1u; p.act2 = s.act2;
+  p.TQ = (s.NQ + C::BQ - 1) / C::BQ;
+  p.sc1 = s.c1 * 1.4426950408889634f;
+  p.sc2 = s.c2 * 1.4426950408889634f;
+  p.kl = kl; p.lse1 = lse1; p.lse2 = lse2;
+  p.W = 1; p.chunk_steps = 0; p.part = nullptr;
+  const long long total = (long long)p.TQ * s.BH;
+  if (total > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
+  const int grid = int(total < sms ? total : sms);
+  sched += 2 * (g_sched_next.fetch_add(1) % kSchedSlots);
+  {
+    ProfScope ps(KID_FWD_TC, stream);
+    kern<<<dim3((unsigned)grid), C::THREADS, C::SMEM_BYTES, stream>>>(tm[0], tm[1], tm[2], tm[3], p, sched);
+  }
+  if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
+  g_last_launches += 1;
+  return STREAMKL_OK;
+}
+
 }  // namespace
 
 int fwd_tc_launch(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, float* kl, float* lse1, float* lse2,
                   cudaStream_t stream, int splits, float* part) {
   int p1 = pad_dim(s.d1), p2 = pad_dim(s.d2);
   if (p1 > 128 || p2 > 128) p1 = p2 = 0;   // a wide head dim: the BLOCKED plan (run-time K-block counts)
+  // the persistent plan: fixed plans (head dims <= 128), default grid
+  // Measured rule of the default plan (profiles/r02h_persistent.md): the persistent kernel wins where tiles are short -- its gain is
+  // the time between tiles -- and there are enough of them to keep every SM busy for several items: at most 64 steps per tile on
+  // average (N_K <= 16K causal, 8K otherwise) and at least two items per SM.  Long tiles (cfg 4) run 1 % faster one CTA per tile.
+  const long long tiles = (long long)s.BH * ((s.NQ + kFwdBQ - 1) / kFwdBQ);
+  const long long avg_steps = ((s.NK + kFwdBK - 1) / kFwdBK + (s.causal ? 1 : 0)) / (s.causal ? 2 : 1);
+  const bool persist_auto = g_fwd_plan == STREAMKL_FWD_AUTO && avg_steps <= 64 && tiles >= 2 * 148;
+  if ((g_fwd_plan == STREAMKL_FWD_PERSISTENT || persist_auto) && splits <= 1 && p1 != 0) {
+#define SKL_FWD_P_CASE(A, Bd)                                                                                             \
+    if (p1 == A && p2 == Bd)                                                                                              \
+      return s.causal ? launch_fwd_persist<A, Bd, true>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream)                    \
+                      : launch_fwd_persist<A, Bd, false>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream);
+    SKL_FWD_P_CASE(128, 128)
+    SKL_FWD_P_CASE(128, 64)
+    SKL_FWD_P_CASE(64, 128)
+    SKL_FWD_P_CASE(64, 64)
+#undef SKL_FWD_P_CASE
+  }
   // the multicast pair plan (streamkl_set_fwd_plan): the default grid only, and only when a head has a second Q tile to pair
   const bool mc = g_fwd_plan == STREAMKL_FWD_MULTICAST && splits <= 1 && s.NQ > skl::FwdCfg<64, 64>::BQ;
   // the cta_group::2 plan: wide head dims only (BLOCKED plan), default grid

@@ -155,4 +155,4 @@ def test_splitk_workspace_and_argument_checks(L):
 def test_bwd_mode_selector(L):
     assert L.streamkl_set_bwd_mode(1) == 0 and L.streamkl_set_bwd_mode(2) == 0 and L.streamkl_set_bwd_mode(0) == 0
     assert L.streamkl_set_bwd_mode(7) == -2
-    assert L.streamkl_set_fwd_plan(1) == 0 and L.streamkl_set_fwd_plan(2) == 0 and L.streamkl_set_fwd_plan(0) == 0 and L.streamkl_set_fwd_plan(3) == -2
+    assert all(L.streamkl_set_fwd_plan(v) == 0 for v in (1, 2, 3, 4, 0)) and L.streamkl_set_fwd_plan(5) == -2 and L.streamkl_set_fwd_plan(-1) == -2

@@ -127,33 +127,38 @@ def test_wide_gradient_padding_columns_are_left_untouched():
 
 
 # ---------------------------------------------------------------- NEXT-3: the two CTA-pair plans of the forward
-@pytest.mark.parametrize("plan", ["multicast", "pair_mma"])
+@pytest.mark.parametrize("plan", ["multicast", "pair_mma", "persistent"])
 @pytest.mark.parametrize("causal", [False, True])
 @pytest.mark.parametrize("d1,d2", [(128, 128), (128, 64), (64, 64), (192, 64), (256, 256), (96, 40), (200, 136)])
-def test_cta_pair_plans_are_bit_identical(d1, d2, causal, plan):
+def test_forward_plans_are_bit_identical(d1, d2, causal, plan):
     """STREAMKL_FWD_MULTICAST: clusters of two CTAs share one TMA-multicast K stream.  STREAMKL_FWD_PAIR_MMA (head dims above 128; the
     plan is ignored below): the pair issues one `tcgen05.mma.cta_group::2` per K-slice, M = 256, each CTA holding 64 of the 128 keys.
+    STREAMKL_FWD_PERSISTENT (head dims up to 128; ignored above): one CTA per SM loops over the Q tiles.
     Same arithmetic in the same order per row, so kl / lse must equal the single-CTA plan bit for bit -- and match the oracle.  Odd
     tile counts (a pair with one tile), ragged tails, NQ != NK, shared K heads and many steps (ring wrap-around) are covered."""
     import torch
 
     import paper_2606_20005_b200 as skl
 
-    code = skl.STREAMKL_FWD_MULTICAST if plan == "multicast" else skl.STREAMKL_FWD_PAIR_MMA
-    for idx, (B, H, HK, NQ, NK) in enumerate([(1, 2, 2, 333, 555), (2, 4, 2, 640, 1500), (1, 1, 1, 129, 129), (1, 2, 2, 2100, 2100)]):
+    code = {"multicast": skl.STREAMKL_FWD_MULTICAST, "pair_mma": skl.STREAMKL_FWD_PAIR_MMA, "persistent": skl.STREAMKL_FWD_PERSISTENT}[plan]
+    # (the last shape has 400 Q tiles: more than one work item per persistent CTA, odd and even step counts, the shared counter)
+    for idx, (B, H, HK, NQ, NK) in enumerate([(1, 2, 2, 333, 555), (2, 4, 2, 640, 1500), (1, 1, 1, 129, 129), (1, 2, 2, 2100, 2100),
+                                              (2, 40, 40, 600, 900)]):
         cfg = W.Config(120 + idx, f"pair{d1}x{d2}", B, H, NQ, NK, d1, d2, "bf16", causal)
         inp = W.all_inputs(cfg)
         if HK != H:
             inp["K1"] = np.ascontiguousarray(inp["K1"][:, :HK])
             inp["K2"] = np.ascontiguousarray(inp["K2"][:, :HK])
         dev = [to_torch(inp[k]) for k in ("Q1", "K1", "Q2", "K2")]
-        single = skl.streamkl_fwd(*dev, cfg.c1, cfg.c2, causal)
-        skl.streamkl_set_fwd_plan(code)
+        skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_PER_TILE)
         try:
+            single = skl.streamkl_fwd(*dev, cfg.c1, cfg.c2, causal)
+            skl.streamkl_set_fwd_plan(code)
             pair = skl.streamkl_fwd(*dev, cfg.c1, cfg.c2, causal)
+            pair = skl.streamkl_fwd(*dev, cfg.c1, cfg.c2, causal, *pair)   # (twice: the persistent plan's scheduler slot is rearmed by each launch)
             torch.cuda.synchronize()
         finally:
-            skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_SINGLE)
+            skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_AUTO)
         for a, b, name in zip(single, pair, ("kl", "lse1", "lse2")):
             assert torch.equal(a, b), f"{cfg.name} case {idx}: {name} differs between the plans"
         G = H // HK
@@ -195,7 +200,7 @@ def test_wide_and_cta_pair_kernels_are_graph_capturable_and_deterministic():
             skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, True, outs[0], outs[1], outs[2], g, teacher=True, dQ1=grads[0],
                              dK1=grads[1], dQ2=grads[2], dK2=grads[3], workspace=ws)
     finally:
-        skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_SINGLE)
+        skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_AUTO)
     for _ in range(2):
         for t in outs + grads:
             t.zero_()
