@@ -240,3 +240,46 @@ def test_concurrent_streams_do_not_interfere():
         for (f, b), (f0, b0) in zip(res, alone):
             for x, y in zip(list(f) + list(b), list(f0) + list(b0)):
                 assert torch.equal(x, y)
+
+
+def test_persistent_plan_in_graphs_and_on_concurrent_streams():
+    """The persistent forward keeps its scheduler state in library-owned device memory (one slot per launch, rearmed by the launch): replaying
+    a captured launch, and overlapping launches on two streams, must reproduce the per-tile kernel bit for bit every time."""
+    import torch
+
+    import paper_2606_20005_b200 as skl
+
+    cfgs = [W.Config(134, "ps-a", 1, 24, 1500, 1500, 128, 64, "bf16", True), W.Config(135, "ps-b", 2, 10, 900, 2300, 128, 128, "bf16", False)]
+    devs, want = [], []
+    skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_PER_TILE)
+    try:
+        for cfg in cfgs:
+            inp = W.all_inputs(cfg)
+            d = [to_torch(inp[k]) for k in ("Q1", "K1", "Q2", "K2")]
+            devs.append(d)
+            want.append(skl.streamkl_fwd(*d, cfg.c1, cfg.c2, cfg.causal))
+        torch.cuda.synchronize()
+        skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_PERSISTENT)
+        # (a) graph replays
+        outs = [torch.zeros_like(t) for t in want[0]]
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            skl.streamkl_fwd(*devs[0], cfgs[0].c1, cfgs[0].c2, cfgs[0].causal, *outs)
+        for _ in range(3):
+            for t in outs:
+                t.zero_()
+            graph.replay()
+            torch.cuda.synchronize()
+            assert all(torch.equal(a, b) for a, b in zip(outs, want[0]))
+        # (b) two streams, launches interleaved and overlapping
+        streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        for _ in range(4):
+            res = []
+            for cfg, d, st in zip(cfgs, devs, streams):
+                with torch.cuda.stream(st):
+                    res.append(skl.streamkl_fwd(*d, cfg.c1, cfg.c2, cfg.causal, stream=st))
+            torch.cuda.synchronize()
+            for got, exp in zip(res, want):
+                assert all(torch.equal(a, b) for a, b in zip(got, exp))
+    finally:
+        skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_AUTO)
