@@ -182,7 +182,7 @@ int streamkl_set_bwd_mode(int mode);
  *   STREAMKL_FWD_PER_TILE   : one CTA per 128-row Q tile (grid bsz x T_Q), each streaming the head's K tiles on its own.
  *   STREAMKL_FWD_PERSISTENT : one CTA per SM loops over the Q tiles (same order, taken from an atomic counter): TMEM and barriers are
  *                             set up once, the next tile's Q / K loads and first MMAs run under the previous tile's last softmax steps.
- *                             Measured on B200: cfg 3 (16K) forward -3..6 %, cfg 2 (4K) -2..6 %, cfg 4 (64K) +1 % (slower).  Head dims
+ *                             Measured on B200: cfg 3 (16K) forward -6..9 %, cfg 2 (4K) -8 %, cfg 4 (64K) +1..2 % (slower).  Head dims
  *                             above 128 run PER_TILE.
  *   STREAMKL_FWD_MULTICAST  : clusters of two CTAs own the Q tiles (2i, 2i+1) of a head and share ONE K stream -- each CTA's
  *                             producer loads half of every stage's K-blocks with TMA multicast into both rings, a stage is
