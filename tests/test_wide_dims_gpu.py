@@ -283,3 +283,17 @@ def test_persistent_plan_in_graphs_and_on_concurrent_streams():
                 assert all(torch.equal(a, b) for a, b in zip(got, exp))
     finally:
         skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_AUTO)
+
+
+def test_persistent_plan_with_layout_features():
+    """The persistent forward takes the same layout as the per-tile kernel: fp16, [B,N,H,d] strides, shared K heads, odd head dims, student ReLU
+    -- forward and (through its saved statistics) every gradient against the oracle."""
+    import paper_2606_20005_b200 as skl
+
+    skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_PERSISTENT)
+    try:
+        _run(W.Config(136, "ps-all", 2, 4, 260, 777, 96, 40, "f16", True), HK=2, view=_as_bnhd, act2="relu", both_modes=False)
+        _run(W.Config(137, "ps-f16", 1, 3, 457, 901, 128, 64, "f16", False), both_modes=False)
+        _run(W.Config(138, "ps-bnhd", 2, 3, 300, 700, 128, 128, "bf16", True), view=_as_bnhd, both_modes=False)
+    finally:
+        skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_AUTO)
