@@ -700,6 +700,6 @@ const char* streamkl_strerror(int code) {
   }
 }
 
-const char* streamkl_version(void) { return "streamkl-b200 0.2 (sm_100a; tcgen05+TMA bf16/fp16, strided + shared-K-head layouts; SIMT fp32)"; }
+const char* streamkl_version(void) { return "streamkl-b200 0.3 (sm_100a; tcgen05+TMA bf16/fp16, head dims to 256, strided + shared-K-head layouts, persistent / CTA-pair forward plans; SIMT fp32)"; }
 
 }  // extern "C"
