@@ -56,7 +56,8 @@ enum {
   STREAMKL_ERR_SCALE = -4,     /* c1 or c2 is not finite and > 0 */
   STREAMKL_ERR_WORKSPACE = -5, /* workspace NULL or smaller than streamkl_bwd_workspace_bytes() */
   STREAMKL_ERR_CUDA = -6,      /* no sm_100 device, tensor-map encode / launch / copy / allocation failure */
-  STREAMKL_ERR_DTYPE = -7      /* unknown dtype code */
+  STREAMKL_ERR_DTYPE = -7,     /* unknown dtype code */
+  STREAMKL_ERR_SCRATCH_LIMIT = -8 /* streamkl_fwd_splitk_noalloc: the partials of this shape and split count exceed the built-in scratch */
 };
 
 enum { STREAMKL_BF16 = 0, STREAMKL_F32 = 1, STREAMKL_F16 = 2 };
@@ -131,6 +132,44 @@ int streamkl_fwd_splitk(const void* Q1, const void* K1, const void* Q2, const vo
 int streamkl_fwd_splitk_splits(int B, int H, int NQ, int NK, int p_target);
 /* B*H*splits*5*NQ floats; 0 when splits <= 1. */
 size_t streamkl_fwd_splitk_workspace_bytes(int B, int H, int NQ, int splits);
+
+/*
+ * Split-K forward for callers that cannot allocate device memory: the same two kernels as streamkl_fwd_splitk (PAPER.md:236-249,
+ * Eq.11), same arguments minus the workspace, same results bit for bit for the same W.
+ *
+ * Who this is for.  streamkl_fwd_splitk needs a caller-owned device buffer for the per-chunk partial statistics.  Some callers
+ * have no way to get one at the point of the call: an operator plugged into a serving engine or inference runtime that hands its
+ * plugins a fixed arena and forbids driver allocations inside the execute callback; a decode loop with a latency budget, where
+ * cudaMalloc / cudaFree would stall every stream of the device; a process whose share of HBM was fixed at start-up (a memory
+ * cap per client, or a co-tenant that has already claimed the rest), where a late allocation simply fails.  Small N_Q against a
+ * long key cache -- decode -- is exactly where split-K is used, so this is the one entry point that gets such a variant.
+ *
+ * How.  The partials go to a fixed array of STREAMKL_NOALLOC_SCRATCH_BYTES (4 MiB) that is part of the library's device image:
+ * every GPU on which this process uses the library holds those 4 MiB from module load until the process exits, whether or not
+ * this function is ever called.  The call itself performs no cudaMalloc, cudaFree, cudaMallocAsync or other allocating call
+ * (per-kernel profiling, streamkl_profile_enable, creates events: leave it off -- its default -- on such a path).
+ *   splits : W as in streamkl_fwd_splitk.  The limit is  B*H*W*5*NQ*4 bytes <= STREAMKL_NOALLOC_SCRATCH_BYTES  (= the value of
+ *            streamkl_fwd_splitk_workspace_bytes; e.g. B*H = 32 heads, NQ = 128, W up to 51; or NQ = 1, B*H = 1024, W up to
+ *            204).  An explicit W beyond the limit returns STREAMKL_ERR_SCRATCH_LIMIT and enqueues nothing -- the array is
+ *            never grown or replaced.  splits <= 0 (adaptive) picks the paper's W and lowers it until it fits; W = 1 and head
+ *            dims off the tensor-core path run the unsplit kernels, which use no scratch at all.
+ * First call on each device: the library asks the runtime for the array's address on the device that is current (a symbol lookup,
+ * no allocation; it also makes the runtime load the library's device code if this is the first use) and remembers it per device
+ * ordinal (up to 64).  Make that first call during set-up, outside any stream capture, with the device you will run on current;
+ * later calls on that device do no lookup.
+ * Sharing.  Every call on a device, from every stream and host thread, uses the SAME array, and the array keeps whatever the last
+ * call wrote.  Nothing needs clearing between calls -- each call overwrites every slot it later reads -- but two calls whose
+ * kernels can run at the same time on one GPU (different streams without an ordering between them) overwrite each other's
+ * partials and both results are garbage, silently.  Order such calls on one stream or with events; callers that need
+ * concurrent split-K calls must use streamkl_fwd_splitk with one workspace per call in flight.
+ * Other errors as streamkl_fwd_splitk.  bf16, contiguous [B][H][N][d] only, like streamkl_fwd_splitk.
+ */
+#define STREAMKL_NOALLOC_SCRATCH_BYTES (4u << 20)
+int streamkl_fwd_splitk_noalloc(const void* Q1, const void* K1, const void* Q2, const void* K2,
+                                int B, int H, int NQ, int NK, int d1, int d2, float c1, float c2, int causal, int splits,
+                                float* kl_rows, float* lse1, float* lse2, streamkl_stream_t stream);
+/* STREAMKL_NOALLOC_SCRATCH_BYTES of the library that is actually loaded (for callers that bind at run time). */
+size_t streamkl_fwd_splitk_noalloc_capacity(void);
 
 /*
  * Backward (Algorithms 2/3 and their K-tile-owner transposes).

@@ -14,6 +14,9 @@ from .binding import (  # noqa: F401
     streamkl_fwd_bwd_host,
     streamkl_fwd_host,
     streamkl_fwd_splitk,
+    streamkl_fwd_splitk_noalloc,
+    streamkl_fwd_splitk_noalloc_capacity,
+    STREAMKL_ERR_SCRATCH_LIMIT,
     streamkl_host_trim,
     streamkl_set_bwd_mode,
     streamkl_set_fwd_plan,

@@ -15,6 +15,7 @@ from .build import LIB_PATH
 __all__ = [
     "StreamKLError", "lib", "lib_path", "streamkl_fwd", "streamkl_bwd", "streamkl_bwd_workspace_bytes",
     "streamkl_fwd_splitk", "streamkl_fwd_splitk_splits", "streamkl_fwd_splitk_workspace_bytes",
+    "streamkl_fwd_splitk_noalloc", "streamkl_fwd_splitk_noalloc_capacity", "STREAMKL_ERR_SCRATCH_LIMIT",
     "streamkl_fwd_host", "streamkl_fwd_bwd_host", "streamkl_host_trim", "streamkl_set_bwd_mode", "streamkl_set_fwd_plan", "STREAMKL_FWD_SINGLE", "STREAMKL_FWD_MULTICAST", "STREAMKL_FWD_PAIR_MMA", "STREAMKL_FWD_PERSISTENT", "STREAMKL_FWD_PER_TILE", "STREAMKL_FWD_AUTO",
     "STREAMKL_BWD_AUTO", "STREAMKL_BWD_SEPARATE", "STREAMKL_BWD_FUSED", "STREAMKL_BF16", "STREAMKL_F16", "STREAMKL_F32", "StreamKLLayout", "streamkl_last_launch_count", "streamkl_strerror",
     "streamkl_profile_enable", "streamkl_profile_collect", "streamkl_kernel_name",
@@ -22,6 +23,7 @@ __all__ = [
 ]
 
 STREAMKL_BF16, STREAMKL_F32, STREAMKL_F16 = 0, 1, 2
+STREAMKL_ERR_SCRATCH_LIMIT = -8
 
 
 class StreamKLLayout(ctypes.Structure):
@@ -78,6 +80,10 @@ def lib() -> ctypes.CDLL:
     L.streamkl_fwd_splitk_splits.restype = ci
     L.streamkl_fwd_splitk_workspace_bytes.argtypes = [ci] * 4
     L.streamkl_fwd_splitk_workspace_bytes.restype = sz
+    L.streamkl_fwd_splitk_noalloc.argtypes = [vp] * 4 + shape + [ci] + [vp] * 3 + [vp]
+    L.streamkl_fwd_splitk_noalloc.restype = ci
+    L.streamkl_fwd_splitk_noalloc_capacity.argtypes = []
+    L.streamkl_fwd_splitk_noalloc_capacity.restype = sz
     L.streamkl_bwd_workspace_bytes.argtypes = [ci] * 7
     L.streamkl_bwd_workspace_bytes.restype = sz
     L.streamkl_fwd_host.argtypes = [ci] + [vp] * 4 + shape + [vp] * 3 + [vp]
@@ -305,6 +311,41 @@ def streamkl_fwd_splitk(Q1, K1, Q2, K2, c1, c2, causal, splits=0, kl_rows=None, 
                                        ctypes.c_size_t(ws_bytes), _stream_handle(stream))
     if rc != 0:
         raise StreamKLError(rc, "streamkl_fwd_splitk")
+    return tuple(outs)
+
+
+def streamkl_fwd_splitk_noalloc_capacity() -> int:
+    """Bytes of split-K scratch built into the loaded library (STREAMKL_NOALLOC_SCRATCH_BYTES, 4 MiB)."""
+    return int(lib().streamkl_fwd_splitk_noalloc_capacity())
+
+
+def streamkl_fwd_splitk_noalloc(Q1, K1, Q2, K2, c1, c2, causal, splits=0, kl_rows=None, lse1=None, lse2=None, stream=None):
+    """Split-K forward whose partial statistics live in a fixed 4 MiB array inside the library instead of a workspace tensor,
+    for code that must not allocate device memory at the time of the call (a plugin running inside someone else's memory arena,
+    a latency-bound decode loop, a process whose HBM share is already spent).  Pass `kl_rows`, `lse1`, `lse2` and this binding
+    allocates nothing either; leave them out and it creates the three output tensors for you, as the other bindings do.
+    `splits` beyond what fits (B*H*W*5*NQ*4 bytes <= streamkl_fwd_splitk_noalloc_capacity()) raises StreamKLError with code
+    STREAMKL_ERR_SCRATCH_LIMIT; splits <= 0 picks a W that fits.  All calls on a GPU share that one array: do not let two of
+    them run at the same time (keep them on one stream).  Returns (kl_rows, lse1, lse2)."""
+    import torch
+
+    for n, t in (("Q1", Q1), ("K1", K1), ("Q2", Q2), ("K2", K2)):
+        _check_dev(n, t, torch.bfloat16)
+    B, H, NQ, NK, d1, d2, HK = _shape_of(Q1, K1, Q2, K2)
+    if HK != H:
+        raise ValueError("streamkl_fwd_splitk_noalloc: shared K heads are not supported")
+    outs = []
+    for n, t in (("kl_rows", kl_rows), ("lse1", lse1), ("lse2", lse2)):
+        if t is None:
+            t = torch.empty((B, H, NQ), dtype=torch.float32, device=Q1.device)
+        _check_dev(n, t, torch.float32)
+        outs.append(t)
+    with torch.cuda.device(Q1.device):
+        rc = lib().streamkl_fwd_splitk_noalloc(_ptr(Q1), _ptr(K1), _ptr(Q2), _ptr(K2), B, H, NQ, NK, d1, d2, float(c1), float(c2),
+                                               int(bool(causal)), int(splits), _ptr(outs[0]), _ptr(outs[1]), _ptr(outs[2]),
+                                               _stream_handle(stream))
+    if rc != 0:
+        raise StreamKLError(rc, "streamkl_fwd_splitk_noalloc")
     return tuple(outs)
 
 

@@ -8,9 +8,11 @@
 #include <cuda_fp16.h>
 
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdint>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 #include "streamkl_host.cuh"
@@ -411,6 +413,37 @@ HostStreams& host_streams() {
   return hs;
 }
 
+// ---- streamkl_fwd_splitk_noalloc: split-K partials in memory that is part of the loaded library image
+// The array below is reserved on every GPU this process uses the library on, from the moment the CUDA module is loaded there until
+// the process exits.  Host code must never hand the NAME of the array to a kernel: on the host that name is only a handle for the
+// runtime's symbol table (a kernel given it would fault or, on systems where the GPU can read host memory, quietly use the wrong
+// bytes).  The real device address is asked for once per device, with that device current, and remembered.
+constexpr size_t kNoAllocScratchBytes = size_t(STREAMKL_NOALLOC_SCRATCH_BYTES);
+static __device__ __align__(256) unsigned char g_noalloc_scratch[kNoAllocScratchBytes];
+
+constexpr int kNoAllocMaxDevices = 64;
+std::atomic<float*> g_noalloc_addr[kNoAllocMaxDevices];   // zero-initialised: "not looked up yet" for that device ordinal
+std::mutex g_noalloc_mutex;
+
+// Device address of g_noalloc_scratch on the CURRENT device (looked up on the first call per device, then cached).
+int noalloc_scratch_on_current_device(float** out) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kNoAllocMaxDevices) { cudaGetLastError(); return STREAMKL_ERR_CUDA; }
+  float* p = g_noalloc_addr[dev].load(std::memory_order_acquire);
+  if (!p) {
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    p = g_noalloc_addr[dev].load(std::memory_order_relaxed);
+    if (!p) {
+      void* q = nullptr;
+      if (cudaGetSymbolAddress(&q, g_noalloc_scratch) != cudaSuccess || !q) { cudaGetLastError(); return STREAMKL_ERR_CUDA; }
+      p = static_cast<float*>(q);
+      g_noalloc_addr[dev].store(p, std::memory_order_release);
+    }
+  }
+  *out = p;
+  return STREAMKL_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -483,6 +516,36 @@ int streamkl_fwd_splitk(const void* Q1, const void* K1, const void* Q2, const vo
   if (reinterpret_cast<uintptr_t>(workspace) & 15) return STREAMKL_ERR_ALIGN;
   return fwd_dispatch(STREAMKL_BF16, nullptr, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
                       static_cast<cudaStream_t>(stream), splits, static_cast<float*>(workspace));
+}
+
+size_t streamkl_fwd_splitk_noalloc_capacity(void) { return kNoAllocScratchBytes; }
+
+int streamkl_fwd_splitk_noalloc(const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1, int d2,
+                                float c1, float c2, int causal, int splits, float* kl_rows, float* lse1, float* lse2,
+                                streamkl_stream_t stream) {
+  const bool adaptive = splits <= 0;
+  if (adaptive) splits = streamkl_fwd_splitk_splits(B, H, NQ, NK, 0);
+  const int tk = NK > 0 ? (NK + kFwdBK - 1) / kFwdBK : 1;
+  if (splits > tk) splits = tk;
+  // an adaptive W is lowered until its partials fit the built-in scratch (W = 1 needs none); an explicit W that does not fit is refused
+  while (adaptive && splits > 1 && streamkl_fwd_splitk_workspace_bytes(B, H, NQ, splits) > kNoAllocScratchBytes) --splits;
+  if (!tc_dims(d1, d2) || splits <= 1)   // unsplit kernels: they write nothing but the outputs, so there is no scratch to provide
+    return fwd_dispatch(STREAMKL_BF16, nullptr, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
+                        static_cast<cudaStream_t>(stream));
+  if (streamkl_fwd_splitk_workspace_bytes(B, H, NQ, splits) > kNoAllocScratchBytes) return STREAMKL_ERR_SCRATCH_LIMIT;
+  // argument errors are reported before the device is touched (the same checks fwd_dispatch repeats below)
+  Shape s{B, H, NQ, NK, d1, d2, causal ? 1 : 0, c1, c2, (long long)B * (long long)H};
+  int rc = validate_common(Q1, K1, Q2, K2, s);
+  if (rc != STREAMKL_OK) return rc;
+  if (s.BH == 0 || s.NQ == 0) return STREAMKL_OK;
+  if (!kl_rows || !lse1 || !lse2) return STREAMKL_ERR_NULLPTR;
+  if (!device_is_sm100()) return STREAMKL_ERR_CUDA;
+  float* part = nullptr;
+  if ((rc = noalloc_scratch_on_current_device(&part)) != STREAMKL_OK) return rc;
+  // Nothing has to be cleared: the split kernel stores all five statistics of every (head, chunk, row) slot the reduce kernel
+  // reads -- identity values for chunks a causal row cannot see -- so what an earlier call left in the array is never read.
+  return fwd_dispatch(STREAMKL_BF16, nullptr, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
+                      static_cast<cudaStream_t>(stream), splits, part);
 }
 
 size_t streamkl_bwd_workspace_bytes(int B, int H, int NQ, int, int d1, int d2, int want_teacher) {
@@ -696,6 +759,7 @@ const char* streamkl_strerror(int code) {
     case STREAMKL_ERR_WORKSPACE: return "workspace missing or too small";
     case STREAMKL_ERR_CUDA: return "CUDA failure (no sm_100 device, tensor-map, launch, copy or allocation)";
     case STREAMKL_ERR_DTYPE: return "unknown dtype code";
+    case STREAMKL_ERR_SCRATCH_LIMIT: return "split-K partials exceed the library's built-in scratch (streamkl_fwd_splitk_noalloc_capacity)";
     default: return "unknown error code";
   }
 }

@@ -54,8 +54,8 @@ def test_binding_exposes_the_same_names():
 def test_version_and_strerror(L):
     assert b"sm_100a" in L.streamkl_version()
     assert L.streamkl_strerror(0) == b"ok"
-    msgs = {L.streamkl_strerror(c) for c in range(-7, 1)}
-    assert len(msgs) == 8
+    msgs = {L.streamkl_strerror(c) for c in range(-8, 1)}
+    assert len(msgs) == 9
 
 
 def _call_fwd(L, ptrs=(16, 16, 16, 16), B=1, H=1, NQ=8, NK=8, d1=64, d2=64, c1=0.125, c2=0.125, causal=0, outs=(16, 16, 16)):
@@ -156,3 +156,25 @@ def test_bwd_mode_selector(L):
     assert L.streamkl_set_bwd_mode(1) == 0 and L.streamkl_set_bwd_mode(2) == 0 and L.streamkl_set_bwd_mode(0) == 0
     assert L.streamkl_set_bwd_mode(7) == -2
     assert all(L.streamkl_set_fwd_plan(v) == 0 for v in (1, 2, 3, 4, 0)) and L.streamkl_set_fwd_plan(5) == -2 and L.streamkl_set_fwd_plan(-1) == -2
+
+
+def test_no_alloc_splitk_limit_is_checked_on_the_host(L):
+    """streamkl_fwd_splitk_noalloc: the capacity is the header's constant, an explicit split count whose partials exceed it is
+    refused before the device is touched, and argument errors still come first when it fits."""
+    L.streamkl_fwd_splitk_noalloc.restype = ctypes.c_int
+    L.streamkl_fwd_splitk_noalloc_capacity.restype = ctypes.c_size_t
+    assert L.streamkl_fwd_splitk_noalloc_capacity() == 4 << 20
+    assert "#define STREAMKL_NOALLOC_SCRATCH_BYTES (4u << 20)" in open(HEADER).read()
+    vp = ctypes.c_void_p
+
+    def call(B, H, NQ, NK, splits, c1=0.125, ptr=16):
+        return L.streamkl_fwd_splitk_noalloc(vp(ptr), vp(16), vp(16), vp(16), B, H, NQ, NK, 64, 64, ctypes.c_float(c1),
+                                             ctypes.c_float(0.125), 0, splits, vp(16), vp(16), vp(16), vp(0))
+
+    # 32 heads x 256 rows: 160 KiB of partials per chunk, so 25 chunks fit in 4 MiB and 26 do not
+    assert call(1, 32, 256, 8192, 26) == -8
+    assert L.streamkl_strerror(-8) not in (b"unknown error code", b"workspace missing or too small")
+    assert call(1, 32, 256, 8192, 25, c1=float("nan")) == -4          # STREAMKL_ERR_SCALE before any device work
+    assert call(1, 32, 256, 8192, 25, ptr=8) == -3                    # STREAMKL_ERR_ALIGN
+    assert call(1, 32, 256, 8192, 25) == -6                           # valid arguments, no GPU here: STREAMKL_ERR_CUDA
+
