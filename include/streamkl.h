@@ -84,6 +84,10 @@ int streamkl_fwd_f32(const void* Q1, const void* K1, const void* Q2, const void*
  *                contiguous default for that tensor ([B][H][N][d], or [B][HK][NK][d] for K).  E.g. a [B][N][H][d] tensor is
  *                {N*H*d, d, H*d}.  Strides must be multiples of 8 elements (16 bytes, TMA) and the row stride >= d.
  *                dQ_t is written with Q_t's strides, dK_t with K_t's; kl_rows / lse / dkl_rows stay contiguous [B][H][NQ].
+ *                The forward also accepts batch / head stride 0 (a broadcast tensor).  The backward does not: a tensor that receives a
+ *                gradient (Q2, K2; Q1, K1 with teacher gradients) must address disjoint rows for distinct (b, h, n) -- no zero or
+ *                self-overlapping strides -- because its gradient is stored, not summed, through the same strides
+ *                (STREAMKL_ERR_SHAPE otherwise; to share K across query heads use kv_heads, which does sum).
  *   student_activation : SURVEY 8(f) NEXT-4, "Generalizability beyond Softmax" ("the ReLU variant used in the indexer
  *                training of DeepSeek-V3.2"; the paper prints no formula, so this is the library's reading, R23).
  *                STREAMKL_ACT_RELU: the student's logit is s2[j] = relu(c2 <Q2[i], K2[j]>) -- that indexer's score with one head and

@@ -191,6 +191,18 @@ def _check_dev(name, t, dtype=None, strided=False):
         raise TypeError(f"{name}: expected dtype {dtype}, got {t.dtype}")
 
 
+def _rows_are_disjoint(t) -> bool:
+    """The library's test (rows_are_disjoint in csrc/streamkl.cu) on a [B,H,N,d] tensor: distinct (b,h,n) -> disjoint rows."""
+    span = int(t.shape[3])
+    for stride, extent in sorted((int(t.stride(i)), int(t.shape[i])) for i in range(3)):
+        if extent <= 1:
+            continue
+        if stride < span:
+            return False
+        span += stride * (extent - 1)
+    return True
+
+
 def _shape_of(Q1, K1, Q2, K2):
     """-> (B, H, NQ, NK, d1, d2, HK): K tensors may carry HK <= H heads (H % HK == 0; query head h reads K head h // (H // HK))."""
     if Q1.dim() != 4 or K1.dim() != 4 or Q2.dim() != 4 or K2.dim() != 4:
@@ -360,6 +372,12 @@ def streamkl_bwd(Q1, K1, Q2, K2, c1, c2, causal, kl_rows, lse1, lse2, dkl_rows, 
         _check_dev(n, t, torch.float32)
     B, H, NQ, NK, d1, d2, HK = _shape_of(Q1, K1, Q2, K2)
     layout = _layout_of(Q1, K1, Q2, K2, HK, student_activation)
+    # gradients are stored through their input's strides: an expanded (stride 0) or self-overlapping view would have several
+    # CTAs overwrite one another where the true gradient is a sum -- refuse it here, as the library does
+    for n, t in (("Q2", Q2), ("K2", K2)) + ((("Q1", Q1), ("K1", K1)) if teacher else ()):
+        if not _rows_are_disjoint(t):
+            raise ValueError(f"{n}: a tensor that receives a gradient must not be a broadcast or self-overlapping view "
+                             "(share K across query heads by giving K fewer heads instead)")
     # every gradient has the shape AND the strides of its input (dQ_t like Q_t, dK_t like K_t)
     like = lambda t: torch.empty_strided(t.shape, t.stride(), dtype=t.dtype, device=t.device)
     if dQ2 is None:

@@ -155,6 +155,26 @@ int apply_layout(Shape& s, const streamkl_layout* L) {
   return STREAMKL_OK;
 }
 
+// true iff the [B][heads][N][d] view with these element strides maps distinct (b, h, n) to disjoint d-element rows.  The test is
+// the nested one -- dimensions of extent > 1 taken by growing stride, each stride at least the span of everything below it -- so
+// broadcast dimensions (stride 0 with extent > 1), head strides below d and interleavings that fold onto themselves fail it.
+// Gradients are written with their input's strides by one owner CTA per tile: on a view that overlaps itself several owners
+// would store to the same addresses and the last one would win where the true gradient is the sum.
+bool rows_are_disjoint(const Strides& st, long long B, long long heads, long long N, int d) {
+  long long sv[3] = {st.b, st.h, st.n}, ev[3] = {B, heads, N};
+  for (int i = 0; i < 3; ++i)
+    for (int j = i + 1; j < 3; ++j)
+      if (sv[j] < sv[i]) { std::swap(sv[i], sv[j]); std::swap(ev[i], ev[j]); }
+  long long span = d;
+  for (int i = 0; i < 3; ++i) {
+    if (ev[i] <= 1) continue;
+    if (sv[i] < span) return false;
+    if (sv[i] > (1LL << 46) / ev[i]) return false;   // (also keeps span inside 64 bits; validate_common bounds the extents)
+    span += sv[i] * (ev[i] - 1);
+  }
+  return true;
+}
+
 int validate_common(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s) {
   if (s.B < 0 || s.H < 0 || s.NQ < 0 || s.NK < 1 || s.d1 < 1 || s.d2 < 1 || s.d1 > 256 || s.d2 > 256) return STREAMKL_ERR_SHAPE;
   if (s.causal && s.NQ > s.NK) return STREAMKL_ERR_SHAPE;
@@ -326,6 +346,11 @@ int bwd_dispatch(int dtype, const streamkl_layout* L, const void* Q1, const void
   if ((rc = apply_layout(s, L)) != STREAMKL_OK) return rc;
   g_last_launches = 0;
   if ((dQ1 == nullptr) != (dK1 == nullptr)) return STREAMKL_ERR_NULLPTR;
+  // the forward may read broadcast or overlapping views; the backward writes dX through the same strides, so every view that
+  // receives a gradient must address disjoint rows
+  if (!rows_are_disjoint(s.q2, s.B, s.H, s.NQ, s.d2) || !rows_are_disjoint(s.k2, s.B, s.HK, s.NK, s.d2)) return STREAMKL_ERR_SHAPE;
+  if (dQ1 && dK1 && (!rows_are_disjoint(s.q1, s.B, s.H, s.NQ, s.d1) || !rows_are_disjoint(s.k1, s.B, s.HK, s.NK, s.d1)))
+    return STREAMKL_ERR_SHAPE;
   if (s.BH == 0) return STREAMKL_OK;
   if (!dK2) return STREAMKL_ERR_NULLPTR;
   if (s.NQ > 0 && (!kl || !lse1 || !lse2 || !dkl || !dQ2)) return STREAMKL_ERR_NULLPTR;

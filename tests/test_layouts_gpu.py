@@ -197,6 +197,23 @@ def test_layout_errors_are_reported_not_launched():
     assert L.streamkl_fwd_ex(ctypes.cast(ctypes.pointer(lay), vp), *args) == -7
 
 
+def test_expanded_k_runs_forward_and_is_refused_by_backward():
+    """K2.expand over heads (head stride 0): the forward reads it like H copies; the backward would have H owner CTAs store to the
+    one dK2 head, so the binding and the library refuse it instead of returning the last writer's values."""
+    import paper_2606_20005_b200 as skl
+
+    cfg = W.Config(93, "expand", 1, 4, 200, 300, 64, 64, "bf16", False)
+    inp = W.all_inputs(cfg)
+    Q1, K1, Q2, K2 = (to_torch(inp[k]) for k in ("Q1", "K1", "Q2", "K2"))
+    K2e = K2[:, :1].expand(-1, cfg.H, -1, -1)
+    kl, l1, l2 = skl.streamkl_fwd(Q1, K1, Q2, K2e, cfg.c1, cfg.c2, False)
+    kl_c, l1_c, l2_c = skl.streamkl_fwd(Q1, K1, Q2, K2e.contiguous(), cfg.c1, cfg.c2, False)
+    assert np.array_equal(to_f64(kl), to_f64(kl_c)) and np.array_equal(to_f64(l2), to_f64(l2_c))
+    g = to_torch(np.ones((cfg.B, cfg.H, cfg.NQ), dtype=np.float32))
+    with pytest.raises(ValueError, match="broadcast or self-overlapping"):
+        skl.streamkl_bwd(Q1, K1, Q2, K2e, cfg.c1, cfg.c2, False, kl, l1, l2, g)
+
+
 # ---------------------------------------------------------------- NEXT-4: student ReLU activation (PAPER.md:143, DESIGN.md R23)
 @pytest.mark.parametrize("causal", [False, True])
 @pytest.mark.parametrize("d1,d2,dtype", [(128, 64, "bf16"), (128, 128, "bf16"), (64, 64, "f16")])

@@ -178,3 +178,40 @@ def test_no_alloc_splitk_limit_is_checked_on_the_host(L):
     assert call(1, 32, 256, 8192, 25, ptr=8) == -3                    # STREAMKL_ERR_ALIGN
     assert call(1, 32, 256, 8192, 25) == -6                           # valid arguments, no GPU here: STREAMKL_ERR_CUDA
 
+
+def test_bwd_refuses_views_whose_gradient_rows_would_overlap(L):
+    """Gradients are stored through the input's strides, so a broadcast (stride 0) or self-overlapping view of a tensor that
+    receives a gradient is an argument error in the backward (the forward, which only reads, accepts it)."""
+    from paper_2606_20005_b200 import StreamKLLayout
+
+    vp = ctypes.c_void_p
+    B, H, NQ, NK, d = 2, 4, 8, 16, 64
+
+    def bwd(lay, teacher):
+        g1 = vp(16) if teacher else vp(0)
+        return L.streamkl_bwd_ex(ctypes.cast(ctypes.pointer(lay), vp), vp(16), vp(16), vp(16), vp(16), B, H, NQ, NK, d, d,
+                                 ctypes.c_float(0.125), ctypes.c_float(0.125), 0, vp(16), vp(16), vp(16), vp(16), g1, g1, vp(16), vp(16),
+                                 vp(16), ctypes.c_size_t(1 << 30), vp(0))
+
+    def fwd(lay):
+        return L.streamkl_fwd_ex(ctypes.cast(ctypes.pointer(lay), vp), vp(16), vp(16), vp(16), vp(16), B, H, NQ, NK, d, d,
+                                 ctypes.c_float(0.125), ctypes.c_float(0.125), 0, vp(16), vp(16), vp(16), vp(0))
+
+    def layout(**strides):
+        lay = StreamKLLayout()
+        lay.dtype = 0
+        for name, v in strides.items():
+            for i in range(3):
+                getattr(lay, name)[i] = v[i]
+        return lay
+
+    ok = -6                                                   # valid arguments reach the device check (no GPU here)
+    assert bwd(layout(k2_stride=(H * NK * d, NK * d, d)), False) == ok
+    assert bwd(layout(k2_stride=(NK * H * d, d, H * d)), False) == ok          # [B][N][H][d]: interleaved, disjoint
+    expanded = layout(k2_stride=(H * NK * d, 0, d))           # K2.expand over heads: H owners would store to one dK2 head
+    assert fwd(expanded) == ok and bwd(expanded, False) == -2
+    assert bwd(layout(q2_stride=(0, NQ * d, d)), False) == -2                  # broadcast batch
+    assert bwd(layout(k2_stride=(H * NK * d, d, d)), False) == -2              # heads one row apart: rows of different heads coincide
+    assert bwd(layout(q2_stride=(H * NQ * d, NQ * d - 8, d)), False) == -2     # head stride short of a head's rows
+    frozen_teacher = layout(k1_stride=(H * NK * d, 0, d))     # a broadcast teacher is fine while it receives no gradient
+    assert bwd(frozen_teacher, False) == ok and bwd(frozen_teacher, True) == -2
