@@ -236,8 +236,11 @@ int streamkl_set_bwd_mode(int mode);
  *                             a K-block, so the K ring beside the (up to 128 KB) Q tile is twice as deep and the stream per CTA half as
  *                             wide.  Measured: +2 % at d = 256/256, 5-15 % slower at 192/64 ... 256/128: never chosen by AUTO
  *                             (DESIGN.md 6.1c).
- * The persistent plan keeps a few bytes of scheduler state per launch in device memory owned by the library (1024 slots used round-robin,
- * rearmed by the launch itself): launches may overlap freely on any streams unless 1024 of them are in flight at once.
+ * The persistent plan keeps a few bytes of scheduler state per launch in device memory owned by the library: 1024 slots, each leased to
+ * one launch at a time (the library records an event behind the launch and reuses the slot only after that event has completed), so
+ * launches may overlap freely on any streams and host threads.  Two cases run the PER_TILE kernel instead, whatever the plan says,
+ * with bit-identical results: a call on a stream that is being captured into a CUDA graph (a captured launch would hold its slot for
+ * the life of the graph), and a call that finds no free slot (hundreds of persistent launches queued and unfinished).
  * Returns STREAMKL_OK, or STREAMKL_ERR_SHAPE for an unknown plan.
  */
 enum { STREAMKL_FWD_AUTO = 0, STREAMKL_FWD_SINGLE = 0 /* older name of AUTO */, STREAMKL_FWD_MULTICAST = 1, STREAMKL_FWD_PAIR_MMA = 2,

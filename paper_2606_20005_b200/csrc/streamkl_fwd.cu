@@ -1,6 +1,7 @@
 // streamkl_fwd.cu -- launchers of the tcgen05 forward kernel (default grid and split-K + reduce); see streamkl.cu for the C ABI.
 #include "streamkl_host.cuh"
-#include <atomic>
+#include <mutex>
+#include <new>
 
 #include "streamkl_fwd_sm100.cuh"
 #include "streamkl_fwd_persist_sm100.cuh"
@@ -79,11 +80,66 @@ int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2
 
 // ---- persistent forward (streamkl_fwd_persist_sm100.cuh): one CTA per SM, dynamic work items
 // Scheduler state of the persistent kernel: {next item, finished CTAs} per slot, zero between launches (the last CTA of a launch
-// rearms its slot).  A launch takes the next slot round-robin, so launches in flight at the same time (other streams, other
-// host threads) do not share one unless 1024 of them overlap.
+// rearms its slot).  Two launches that can be in flight at the same time must not share a slot (they would take each other's
+// tickets and skip tiles), so a slot is LEASED: the host records an event behind every launch that used it and hands the slot out
+// again only once that event has completed.  When no slot is free (hundreds of launches queued) or the stream is being captured
+// into a CUDA graph (a captured launch would keep its slot for as long as the graph lives, and an event recorded during capture
+// cannot be queried), the caller runs the per-tile kernel instead: same results bit for bit.
 constexpr int kSchedSlots = 1024;
+constexpr int kSchedProbe = 16;      // slots examined per launch before giving up
+constexpr int kSchedMaxDevices = 64;
 __device__ int g_fwd_sched[kSchedSlots][2];
-std::atomic<unsigned> g_sched_next{0};
+
+struct SchedLeases {
+  std::mutex mu;
+  unsigned next = 0;
+  cudaEvent_t done[kSchedSlots] = {};   // recorded behind the last launch that used the slot (created on first use)
+  bool held[kSchedSlots] = {};          // between acquire() and release(): the launch and its event are being enqueued
+};
+std::mutex g_sched_mu;
+SchedLeases* g_sched_leases[kSchedMaxDevices] = {};
+
+SchedLeases* sched_leases(int dev) {
+  if (dev < 0 || dev >= kSchedMaxDevices) return nullptr;
+  std::lock_guard<std::mutex> lock(g_sched_mu);
+  if (!g_sched_leases[dev]) g_sched_leases[dev] = new (std::nothrow) SchedLeases();
+  return g_sched_leases[dev];
+}
+
+// a slot no launch in flight is using, or -1
+int sched_acquire(SchedLeases& L) {
+  std::lock_guard<std::mutex> lock(L.mu);
+  for (int probe = 0; probe < kSchedProbe; ++probe) {
+    const int i = int(L.next++ % kSchedSlots);
+    if (L.held[i]) continue;
+    if (!L.done[i]) {
+      if (cudaEventCreateWithFlags(&L.done[i], cudaEventDisableTiming) != cudaSuccess) { cudaGetLastError(); L.done[i] = nullptr; return -1; }
+    } else if (cudaEventQuery(L.done[i]) != cudaSuccess) {
+      cudaGetLastError();   // cudaErrorNotReady: the last launch on this slot has not finished
+      continue;
+    }
+    L.held[i] = true;
+    return i;
+  }
+  return -1;
+}
+
+// after the launch (or a failed one): mark the slot busy until everything enqueued on `stream` so far has finished
+bool sched_release(SchedLeases& L, int slot, cudaStream_t stream) {
+  const bool ok = cudaEventRecord(L.done[slot], stream) == cudaSuccess;
+  if (!ok) cudaGetLastError();
+  std::lock_guard<std::mutex> lock(L.mu);
+  L.held[slot] = false;
+  return ok;
+}
+
+bool stream_is_capturing(cudaStream_t stream) {
+  cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+  if (cudaStreamIsCapturing(stream, &st) != cudaSuccess) { cudaGetLastError(); return true; }   // (e.g. the legacy stream during a global capture)
+  return st != cudaStreamCaptureStatusNone;
+}
+
+constexpr int kPersistUnavailable = 1;   // launch_fwd_persist: no scheduler slot could be leased -- run the per-tile kernel
 
 template <int D1, int D2, bool CAUSAL>
 int launch_fwd_persist(const void* Q1, const void* K1, const void* Q2, const void* K2, const Shape& s, bool f16, float* kl, float* lse1,
@@ -112,12 +168,16 @@ int launch_fwd_persist(const void* Q1, const void* K1, const void* Q2, const voi
   const long long total = (long long)p.TQ * s.BH;
   if (total > 0x7fffffffLL) return STREAMKL_ERR_SHAPE;
   const int grid = int(total < sms ? total : sms);
-  sched += 2 * (g_sched_next.fetch_add(1) % kSchedSlots);
+  SchedLeases* leases = sched_leases(dev);
+  const int slot = leases ? sched_acquire(*leases) : -1;
+  if (slot < 0) return kPersistUnavailable;
+  sched += 2 * slot;
   {
     ProfScope ps(KID_FWD_TC, stream);
     kern<<<dim3((unsigned)grid), C::THREADS, C::SMEM_BYTES, stream>>>(tm[0], tm[1], tm[2], tm[3], p, sched);
   }
-  if (cudaGetLastError() != cudaSuccess) return STREAMKL_ERR_CUDA;
+  const bool launched = cudaGetLastError() == cudaSuccess;
+  if (!sched_release(*leases, slot, stream) || !launched) return STREAMKL_ERR_CUDA;
   g_last_launches += 1;
   return STREAMKL_OK;
 }
@@ -135,16 +195,18 @@ int fwd_tc_launch(const void* Q1, const void* K1, const void* Q2, const void* K2
   const long long tiles = (long long)s.BH * ((s.NQ + kFwdBQ - 1) / kFwdBQ);
   const long long avg_steps = ((s.NK + kFwdBK - 1) / kFwdBK + (s.causal ? 1 : 0)) / (s.causal ? 2 : 1);
   const bool persist_auto = g_fwd_plan == STREAMKL_FWD_AUTO && avg_steps <= 64 && tiles >= 2 * 148;
-  if ((g_fwd_plan == STREAMKL_FWD_PERSISTENT || persist_auto) && splits <= 1 && p1 != 0) {
+  if ((g_fwd_plan == STREAMKL_FWD_PERSISTENT || persist_auto) && splits <= 1 && p1 != 0 && !stream_is_capturing(stream)) {
+    int rc = kPersistUnavailable;
 #define SKL_FWD_P_CASE(A, Bd)                                                                                             \
     if (p1 == A && p2 == Bd)                                                                                              \
-      return s.causal ? launch_fwd_persist<A, Bd, true>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream)                    \
-                      : launch_fwd_persist<A, Bd, false>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream);
+      rc = s.causal ? launch_fwd_persist<A, Bd, true>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream)                      \
+                    : launch_fwd_persist<A, Bd, false>(Q1, K1, Q2, K2, s, f16, kl, lse1, lse2, stream);
     SKL_FWD_P_CASE(128, 128)
     SKL_FWD_P_CASE(128, 64)
     SKL_FWD_P_CASE(64, 128)
     SKL_FWD_P_CASE(64, 64)
 #undef SKL_FWD_P_CASE
+    if (rc != kPersistUnavailable) return rc;   // (no free scheduler slot: the per-tile kernel below, bit-identical)
   }
   // the multicast pair plan (streamkl_set_fwd_plan): the default grid only, and only when a head has a second Q tile to pair
   const bool mc = g_fwd_plan == STREAMKL_FWD_MULTICAST && splits <= 1 && s.NQ > skl::FwdCfg<64, 64>::BQ;

@@ -243,8 +243,9 @@ def test_concurrent_streams_do_not_interfere():
 
 
 def test_persistent_plan_in_graphs_and_on_concurrent_streams():
-    """The persistent forward keeps its scheduler state in library-owned device memory (one slot per launch, rearmed by the launch): replaying
-    a captured launch, and overlapping launches on two streams, must reproduce the per-tile kernel bit for bit every time."""
+    """The persistent forward keeps its scheduler state in library-owned device memory (one slot leased per launch): overlapping launches
+    on two streams must reproduce the per-tile kernel bit for bit every time; under stream capture the library runs the per-tile kernel
+    (a captured launch would hold its slot for the life of the graph), so replays must match as well."""
     import torch
 
     import paper_2606_20005_b200 as skl
@@ -271,8 +272,23 @@ def test_persistent_plan_in_graphs_and_on_concurrent_streams():
             graph.replay()
             torch.cuda.synchronize()
             assert all(torch.equal(a, b) for a, b in zip(outs, want[0]))
-        # (b) two streams, launches interleaved and overlapping
+        # (b) two streams, launches interleaved and overlapping; many more launches than the library has scheduler slots (1024), queued
+        # without a synchronisation in between: a slot must never be handed to a launch while an earlier one may still be using it
         streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+        small = W.Config(139, "ps-c", 1, 40, 1024, 1024, 64, 64, "bf16", True)
+        ds = [to_torch(W.all_inputs(small)[k]) for k in ("Q1", "K1", "Q2", "K2")]
+        skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_PER_TILE)
+        want_small = skl.streamkl_fwd(*ds, small.c1, small.c2, small.causal)
+        skl.streamkl_set_fwd_plan(skl.STREAMKL_FWD_PERSISTENT)
+        outs_small = [[torch.empty_like(t) for t in want_small] for _ in range(2)]
+        for i in range(2600):
+            st = streams[i & 1]
+            with torch.cuda.stream(st):
+                skl.streamkl_fwd(*ds, small.c1, small.c2, small.causal, *outs_small[i & 1], stream=st)
+            if i % 325 == 324:
+                torch.cuda.synchronize()
+                for o in outs_small:
+                    assert all(torch.equal(a, b) for a, b in zip(o, want_small))
         for _ in range(4):
             res = []
             for cfg, d, st in zip(cfgs, devs, streams):
