@@ -1,5 +1,7 @@
 // streamkl_fwd.cu -- launchers of the tcgen05 forward kernel (default grid and split-K + reduce); see streamkl.cu for the C ABI.
 #include "streamkl_host.cuh"
+#include <algorithm>
+#include <atomic>
 #include <mutex>
 #include <new>
 
@@ -34,7 +36,9 @@ int launch_fwd_tc(const void* Q1, const void* K1, const void* Q2, const void* K2
   } else {
     smem_bytes = C::SMEM_BYTES;
   }
-  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes) != cudaSuccess) {
+  // (the BLOCKED plan's size depends on the head dims, and the attribute is per function, not per launch: always raise it to the
+  // same constant, so that concurrent host threads with different head-dim pairs cannot lower it under one another)
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::BLOCKED ? C::SMEM_LIMIT : smem_bytes) != cudaSuccess) {
     cudaGetLastError();
     return STREAMKL_ERR_CUDA;
   }
@@ -139,6 +143,19 @@ bool stream_is_capturing(cudaStream_t stream) {
   return st != cudaStreamCaptureStatusNone;
 }
 
+// SMs of the current device (asked once per device ordinal; 148 on a B200)
+int sm_count() {
+  static std::atomic<int> cached[kSchedMaxDevices];
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kSchedMaxDevices) { cudaGetLastError(); return 148; }
+  int n = cached[dev].load(std::memory_order_relaxed);
+  if (n <= 0) {
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) { cudaGetLastError(); return 148; }
+    cached[dev].store(n, std::memory_order_relaxed);
+  }
+  return n;
+}
+
 constexpr int kPersistUnavailable = 1;   // launch_fwd_persist: no scheduler slot could be leased -- run the per-tile kernel
 
 template <int D1, int D2, bool CAUSAL>
@@ -192,9 +209,19 @@ int fwd_tc_launch(const void* Q1, const void* K1, const void* Q2, const void* K2
   // Measured rule of the default plan (profiles/r02h_persistent.md): the persistent kernel wins where tiles are short -- its gain is
   // the time between tiles -- and there are enough of them to keep every SM busy for several items: at most 64 steps per tile on
   // average (N_K <= 16K causal, 8K otherwise) and at least two items per SM.  Long tiles (cfg 4) run 1 % faster one CTA per tile.
-  const long long tiles = (long long)s.BH * ((s.NQ + kFwdBQ - 1) / kFwdBQ);
-  const long long avg_steps = ((s.NK + kFwdBK - 1) / kFwdBK + (s.causal ? 1 : 0)) / (s.causal ? 2 : 1);
-  const bool persist_auto = g_fwd_plan == STREAMKL_FWD_AUTO && avg_steps <= 64 && tiles >= 2 * 148;
+  const int TQ = (s.NQ + kFwdBQ - 1) / kFwdBQ, TK = (s.NK + kFwdBK - 1) / kFwdBK;
+  const long long tiles = (long long)s.BH * TQ;
+  // key steps per Q tile, averaged over the head's tiles.  Causal tile t (rows q0 = t*BQ ...) streams the keys up to its last row's
+  // frontier q0 + BQ - 1 + (NK - NQ): ceil of that over BK steps, at most TK -- an arithmetic series in t until it saturates at TK
+  // (NQ << NK: every tile streams at least NK - NQ keys, so the average is close to TK, not TK / 2)
+  long long sum_steps = (long long)TQ * TK;
+  if (s.causal) {
+    sum_steps = 0;
+    for (int t = 0; t < TQ; ++t) sum_steps += std::min<long long>(TK, ((long long)t * kFwdBQ + kFwdBQ - 1 + (s.NK - s.NQ)) / kFwdBK + 1);
+  }
+  const long long avg_steps = TQ > 0 ? sum_steps / TQ : 0;   // (rounded down: NQ = NK = 16K causal is 64.5 -> 64, inside the rule)
+  bool persist_auto = g_fwd_plan == STREAMKL_FWD_AUTO && avg_steps <= 64 && p1 != 0 && splits <= 1;
+  if (persist_auto) persist_auto = tiles >= 2LL * sm_count();   // at least two items per SM of the device that will run it
   if ((g_fwd_plan == STREAMKL_FWD_PERSISTENT || persist_auto) && splits <= 1 && p1 != 0 && !stream_is_capturing(stream)) {
     int rc = kPersistUnavailable;
 #define SKL_FWD_P_CASE(A, Bd)                                                                                             \
