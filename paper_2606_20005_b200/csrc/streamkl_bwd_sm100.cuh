@@ -173,7 +173,7 @@ __device__ __forceinline__ float4 lds_f4(uint32_t saddr) {
 //            pairs, two float4 each), g is applied here.
 // MASKED: causal diagonal tiles and streamed-key tails; P (possibly inf for a zero-filled logit) is discarded by SELECT.
 // RELU2 (R23): the student's logit is relu(s2'), i.e. x2 = max(x2_raw, -lse2 log2e) in the shifted log2 domain,
-// and relu' = 1[x2_raw > -lse2 log2e] gates dS2.
+// and relu' = 1[<q2,k2> > 0] gates dS2.
 template <int NC, bool TEACHER, bool OWNER_K, bool CAUSAL, bool MASKED, bool WANT2 = true, bool F16 = false, bool RELU2 = false>
 __device__ __forceinline__ void ds_row(const uint32_t (&r1)[NC], const uint32_t (&r2)[NC], uint32_t (&o1)[NC / 2], uint32_t (&o2)[NC / 2],
                                          float sc1, float sc2, float nL1, float nL2, float klog, uint32_t stat, int xrow,
@@ -190,7 +190,9 @@ __device__ __forceinline__ void ds_row(const uint32_t (&r1)[NC], const uint32_t 
     float2 x2 = fma2(make_float2(__uint_as_float(r2[e]), __uint_as_float(r2[e + 1])), vsc2, vn2);
     bool on0 = true, on1 = true;
     if constexpr (RELU2) {
-      on0 = x2.x > vn2.x; on1 = x2.y > vn2.y;
+      // relu' on the sign of the raw accumulator (exact: sc2 > 0).  Comparing the shifted values instead would switch off a small
+      // positive logit whose product with sc2 rounds away against |lse2 log2e|, where the definition 1[s2 > 0] keeps it on.
+      on0 = __uint_as_float(r2[e]) > 0.f; on1 = __uint_as_float(r2[e + 1]) > 0.f;
       x2 = make_float2(fmaxf(x2.x, vn2.x), fmaxf(x2.y, vn2.y));
     }
     // P_t = exp(s_t - lse_t) (Alg.2 line 7); one column pair in every STREAMKL_BWD_POLY_EVERY on the FMA/ALU pipes

@@ -254,3 +254,42 @@ def test_relu_student_closed_form_all_logits_negative():
         assert float(dQ2.float().abs().max()) == 0.0 and float(dK2.float().abs().max()) == 0.0
         check_grad_heads(to_f64(dQ1), ref["dQ1"], f"mode {mode} dQ1")
         check_grad_heads(to_f64(dK1), ref["dK1"], f"mode {mode} dK1")
+
+
+def test_relu_gate_follows_the_sign_of_the_raw_logit():
+    """relu' = 1[<q2,k2> > 0] (R23) must be decided on the raw logit.  Here every student logit but one is a tiny positive number
+    (2^-20) while one key per row has logit 40, so lse2 ~ 40: in the shifted log2 domain the tiny logits round away against
+    lse2 log2e ~ 57.7 (half an ulp there is 1.9e-6), and a gate taken after the shift would switch them all off -- dS2 = 0 where the
+    definition has dS2 = g (P2 - P1) ~ -g P1.  Every strategy against the oracle."""
+    import paper_2606_20005_b200 as skl
+
+    cfg = W.Config(95, "relu-gate", 1, 2, 200, 300, 64, 64, "bf16", False)
+    inp = W.all_inputs(cfg)
+    f = {k: W.widen_f64(inp[k]) for k in ("Q1", "K1", "Q2", "K2")}
+    f["Q2"][...] = 0.0
+    f["Q2"][..., 0] = 2.0 ** -10
+    f["K2"][..., 0] = 2.0 ** -10                     # raw logit 2^-20 > 0 for every (i, j) ...
+    f["K2"][:, :, 7, 0] = 40.0 / cfg.c2 * 2.0 ** 10  # ... but key 7: logit 40 (bf16-exact: 327680 for c2 = 1/8)
+    import torch
+
+    Q1, K1 = to_torch(inp["Q1"]), to_torch(inp["K1"])
+    Q2, K2 = (torch.from_numpy(f[k]).to(torch.bfloat16).cuda() for k in ("Q2", "K2"))
+    assert np.array_equal(to_f64(Q2), f["Q2"]) and np.array_equal(to_f64(K2), f["K2"])      # bf16-exact inputs
+    g = to_torch(inp["g"])
+    ref = attention_kl(f["Q1"], f["K1"], f["Q2"], f["K2"], cfg.c1, cfg.c2, False, g=inp["g"].astype(np.float64), teacher=True, act2="relu")
+    assert np.abs(ref["dK2"][:, :, :7, 0]).min() > 0                                         # the gated-on keys do carry gradient
+    kl, l1, l2 = skl.streamkl_fwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, False, student_activation="relu")
+    check_fwd(to_f64(kl), to_f64(l1), to_f64(l2), ref, "relu-gate fwd")
+    for mode in (skl.STREAMKL_BWD_FUSED, skl.STREAMKL_BWD_SEPARATE):
+        skl.streamkl_set_bwd_mode(mode)
+        try:
+            grads = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, False, kl, l1, l2, g, teacher=True, student_activation="relu")
+        finally:
+            skl.streamkl_set_bwd_mode(skl.STREAMKL_BWD_AUTO)
+        for name, t in zip(("dQ1", "dK1", "dQ2", "dK2"), grads):
+            check_grad_heads(to_f64(t), ref[name], f"relu-gate mode {mode} {name}")
+        # the entries that exist only because the tiny logits are gated ON: dK2[j != 7, 0] = -c2 2^-10 sum_i g_i P1[i,j] (about 1e-4,
+        # 0.3 % of the column's largest entry, so the per-head bars above would not notice them missing) -- element by element
+        keys = np.arange(cfg.NK) != 7
+        got, want = to_f64(grads[3])[:, :, keys, 0], ref["dK2"][:, :, keys, 0]
+        assert np.abs(got - want).max() <= 3e-2 * np.abs(want).min(), f"relu-gate mode {mode}: dK2 of the tiny-logit keys"
