@@ -31,7 +31,7 @@ def _sources():
 
 
 def _all_inputs():
-    files = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith((".cu", ".cuh", ".h"))]
+    files = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith((".cu", ".cuh", ".h", ".inc"))]
     files += [os.path.join(INCLUDE, f) for f in sorted(os.listdir(INCLUDE)) if f.endswith(".h")]
     return files
 
@@ -41,7 +41,7 @@ def _digest(extra_flags) -> str:
     h.update(" ".join(NVCC_FLAGS + list(extra_flags)).encode())
     for f in _all_inputs():
         with open(f, "rb") as fh:
-            h.update(f.encode())
+            h.update(os.path.relpath(f, os.path.dirname(PKG_DIR)).encode())   # (relative: the stamp survives another checkout location)
             h.update(fh.read())
     return h.hexdigest()
 

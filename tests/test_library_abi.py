@@ -215,3 +215,17 @@ def test_bwd_refuses_views_whose_gradient_rows_would_overlap(L):
     assert bwd(layout(q2_stride=(H * NQ * d, NQ * d - 8, d)), False) == -2     # head stride short of a head's rows
     frozen_teacher = layout(k1_stride=(H * NK * d, 0, d))     # a broadcast teacher is fine while it receives no gradient
     assert bwd(frozen_teacher, False) == ok and bwd(frozen_teacher, True) == -2
+
+
+def test_build_digest_covers_every_source_kind_and_is_location_independent():
+    """The stamp that decides whether libstreamkl.so is current hashes every file that reaches the compiler -- the .inc launchers
+    included -- under paths relative to the repository, so the same tree gives the same digest wherever it is checked out."""
+    from paper_2606_20005_b200 import build
+
+    names = {os.path.basename(f) for f in build._all_inputs()}
+    csrc = os.path.join(os.path.dirname(build.__file__), "csrc")
+    assert {f for f in os.listdir(csrc) if f.endswith((".cu", ".cuh", ".inc", ".h"))} <= names
+    assert "streamkl_bwd_owner.inc" in names and "streamkl.h" in names
+    import inspect
+
+    assert "relpath" in inspect.getsource(build._digest)
