@@ -41,7 +41,7 @@ UNIT = "TFLOP/s"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 SPEC_BF16_TFLOPS = 2250.0
 WORKLOADS = {"cfg2": 2, "cfg3": 3, "cfg4": 4, "cfg5": 5}
-SIDE_LEGS = ("splitk", "bwd-strategies", "wide-dims")   # --workload <leg>: run only that secondary measurement (profiling runs)
+SIDE_LEGS = ("splitk", "bwd-strategies", "bwd-strategies-large", "wide-dims")   # --workload <leg>: run only that secondary measurement (profiling runs)
 
 
 def peaks():
@@ -204,7 +204,8 @@ def oracle_sample(cfg: W.Config, budget_s: float, rows_per_block: int = 256, max
             break
     dt = time.perf_counter() - t0
     desc = (f"{nb} blocks of {rows_per_block} query rows (bit-reversed spread over NQ) of head (b=0,h=0) of cfg{cfg.idx}, "
-            f"fwd+bwd by the float64 definition incl. this block's dK contribution; {rows_done} rows, {dt:.1f} s")
+            f"fwd+bwd by the float64 definition incl. this block's dK contribution; {rows_done} rows, {dt:.1f} s; "
+            "NumPy: the matmuls run on the BLAS threads counted in `cores`, the exp / log / where / reduction passes are single-threaded")
     return flops / dt / 1e12, dt, flops, desc
 
 
@@ -468,6 +469,53 @@ def time_bwd_strategies(skl, iters: int = 20, nqs=(16, 128, 256, 512, 1024, 4096
     return {"shape": "bsz=16 (B=1,H=16), NK=16384, d=128/128, bf16, no mask", "auto_rule": "one-visit kernels iff NQ <= 512 (Setting 1) / NQ <= 256 (Setting 2)", "rows": out}
 
 
+def time_bwd_strategies_large(skl, iters: int = 8):
+    """Setting-1 backward at LARGE N_Q ("adaptively selects between the two strategies at runtime", Fig.13): the two owner
+    kernels (each recomputes both logit tiles and both exps) against the one-visit student pass (one recomputation, dQ2 through fp32
+    atomics), N_Q = N_K from 4K to 64K, d1 = 128, d2 in {64, 128}, causal and not.  32 heads (8 at 64K to bound the run).  ms per call."""
+    import torch
+
+    rows = {}
+    for N in (4096, 8192, 16384, 32768, 65536):
+        H = 8 if N >= 65536 else 32
+        for d2 in (64, 128):
+            for causal in (True, False):
+                cfg = W.Config(72, "bwd-strategy-large", 1, H, N, N, 128, d2, "bf16", causal)
+                inp = W.all_inputs(cfg)
+                Q1, K1, Q2, K2 = (to_dev(inp[k]) for k in ("Q1", "K1", "Q2", "K2"))
+                g = to_dev(inp["g"])
+                kl, l1, l2 = skl.streamkl_fwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, causal)
+                row = {}
+                for mode in ("separate", "fused", "auto"):
+                    skl.streamkl_set_bwd_mode(BWD_MODES[mode])
+                    try:
+                        ws = torch.empty(max(1, skl.streamkl_bwd_workspace_bytes(cfg.B, cfg.H, N, N, cfg.d1, cfg.d2, False)), dtype=torch.uint8, device="cuda")
+                        grads = skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, causal, kl, l1, l2, g, teacher=False, workspace=ws)
+
+                        def call():
+                            skl.streamkl_bwd(Q1, K1, Q2, K2, cfg.c1, cfg.c2, causal, kl, l1, l2, g, teacher=False, dQ2=grads[2], dK2=grads[3], workspace=ws)
+
+                        for _ in range(3):
+                            call()
+                        torch.cuda.synchronize()
+                        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        a.record()
+                        for _ in range(iters):
+                            call()
+                        b.record()
+                        torch.cuda.synchronize()
+                        row[f"{mode}_ms"] = a.elapsed_time(b) / iters
+                        row[f"{mode}_workspace_bytes"] = int(ws.numel())
+                    finally:
+                        skl.streamkl_set_bwd_mode(BWD_MODES["auto"])
+                    del ws, grads
+                row["fused_speedup"] = row["separate_ms"] / row["fused_ms"]
+                rows[f"N={N} H={H} d=128/{d2} {'causal' if causal else 'full'}"] = row
+                del Q1, K1, Q2, K2, g, kl, l1, l2, inp
+                torch.cuda.empty_cache()
+    return {"shape": "Setting 1 (dQ2, dK2), B=1, N_Q = N_K = N, bf16", "rows": rows}
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -503,6 +551,8 @@ def main():
                 d1, d2 = (int(x) for x in args.dims.split(","))
                 pairs = ((d1, d2, True),)
             out = time_wide_dims(skl, pairs=pairs)
+        elif args.workload == "bwd-strategies-large":
+            out = time_bwd_strategies_large(skl, iters=min(args.iters, 8))
         else:
             out = time_bwd_strategies(skl, iters=args.iters, nqs=(args.nq,) if args.nq > 0 else (16, 128, 256, 512, 1024, 4096))
         if rank == 0:
@@ -565,6 +615,31 @@ def main():
                 "share_of_step": dom_stat["avg_ms"] * dom_stat["launches_per_step"] / res["step_ms"],
                 "avg_ms": dom_stat["avg_ms"]}
 
+    # every tensor-core kernel of the step and the forward numbers north_star asks for, inside `roofline` (a key the driver record keeps)
+    burst_tf, sust_tf = float(pk["bf16_tflops"]), float(pk["bf16_tflops_sustained"])
+
+    def tc_kernel_table(c, kernels):
+        n_b = sum(v["launches_per_step"] for k, v in kernels.items() if "bwd" in k and "sm100" in k)
+        tab = {}
+        for k, v in kernels.items():
+            if "sm100" not in k or "stats" in k:
+                continue
+            tf = kernel_flops_one_visit(c, k, n_b) / (v["avg_ms"] * 1e-3) / 1e12
+            tab[k] = {"avg_ms": v["avg_ms"], "launches_per_step": v["launches_per_step"], "tflops_algorithmic": tf,
+                      "tflops_executed": kernel_flops(c, k) / (v["avg_ms"] * 1e-3) / 1e12,
+                      "frac_of_burst": tf / burst_tf, "frac_of_sustained": tf / sust_tf}
+        return tab
+
+    def fwd_entry(c, fwd_ms, where):
+        tf = c.fwd_flop() / (fwd_ms * 1e-3) / 1e12
+        return {"workload": c.name, "ms": fwd_ms, "tflops": tf, "frac_of_burst": tf / burst_tf, "frac_of_sustained": tf / sust_tf,
+                "frac_of_spec_2250": tf / SPEC_BF16_TFLOPS, "timed": where}
+
+    roofline["kernels"] = tc_kernel_table(cfg, res["kernels"])
+    roofline["step"] = {"fwd_ms": res["fwd_ms"], "bwd_ms": res["bwd_ms"], "bwd_tflops_one_visit": flop_b / (res["bwd_ms"] * 1e-3) / 1e12,
+                        "bwd_frac_of_sustained": flop_b / (res["bwd_ms"] * 1e-3) / 1e12 / sust_tf}
+    roofline["forward_64k" if cfg.NQ >= 65536 else f"forward_{cfg.name}"] = fwd_entry(cfg, res["fwd_ms"], "inside the timed step (between backward passes)")
+
     detail = {
         "fwd_ms": res["fwd_ms"], "bwd_ms": res["bwd_ms"],
         "fwd_tflops": flop_f / (res["fwd_ms"] * 1e-3) / 1e12, "bwd_tflops": flop_b / (res["bwd_ms"] * 1e-3) / 1e12,
@@ -605,6 +680,8 @@ def main():
             "frac_of_measured_bf16_burst": flop_f / (alone_ms * 1e-3) / 1e12 / float(pk["bf16_tflops"]),
             "frac_of_measured_bf16_sustained": flop_f / (alone_ms * 1e-3) / 1e12 / float(pk["bf16_tflops_sustained"]),
             "note": "forward launches back to back for ~1.5 s, no backward in between; the in-step figure above is the bench's own"}
+        if cfg.NQ >= 65536:
+            roofline["forward_64k_alone"] = fwd_entry(cfg, alone_ms, f"{n_alone} forward launches back to back (~1.5 s), no backward in between: sustained clocks")
 
     # ---- secondary: the 16K configuration the metric also names
     also = {}
@@ -623,6 +700,11 @@ def main():
                 "fwd_frac_of_measured_bf16_burst": c.fwd_flop() / (r["fwd_ms"] * 1e-3) / 1e12 / float(pk["bf16_tflops"]),
                 "workspace_bytes": int(r["workspace_bytes"]),
                 "kernels_ms": {k: v["avg_ms"] for k, v in r["kernels"].items()}}
+            if idx == 3:   # the 16K size BASELINE.json's metric names (0.1 s timed region: the burst peak is the yardstick)
+                roofline["forward_16k"] = fwd_entry(c, r["fwd_ms"], "inside cfg3's timed steps")
+                roofline["backward_16k"] = {"workload": c.name, "ms": r["bwd_ms"], "tflops_one_visit": c.bwd_flop() / (r["bwd_ms"] * 1e-3) / 1e12,
+                                            "frac_of_burst": c.bwd_flop() / (r["bwd_ms"] * 1e-3) / 1e12 / burst_tf,
+                                            "kernels": tc_kernel_table(c, r["kernels"])}
             del d, h, r
             torch.cuda.empty_cache()
         sk = time_splitk(skl)

@@ -116,7 +116,7 @@ int streamkl_bwd_ex(const streamkl_layout* layout, const void* Q1, const void* K
                     void* workspace, size_t workspace_bytes, streamkl_stream_t stream);
 
 /*
- * Split-K forward for small NQ (Eq.11; bf16, d1,d2 multiples of 8 up to 256).  The key range is cut into W
+ * Split-K forward for small NQ (Eq.11; bf16 -- other layouts: streamkl_fwd_splitk_ex below -- d1,d2 multiples of 8 up to 256).  The key range is cut into W
  * contiguous chunks of C_K = 128*ceil(ceil(NK/128)/W) keys (the paper's ceil(NK/W), rounded up to whole 128-key tiles);
  * the grid becomes (bsz, T_Q, W); every CTA writes its chunk's partial statistics (m1,l1,m2,l2,acc) -- 5 floats per
  * row and chunk -- to `workspace`, and a reduce kernel merges them with Eq.11 ((m2,l2) merged the same way) and
@@ -130,6 +130,15 @@ int streamkl_fwd_splitk(const void* Q1, const void* K1, const void* Q2, const vo
                         int B, int H, int NQ, int NK, int d1, int d2, float c1, float c2, int causal, int splits,
                         float* kl_rows, float* lse1, float* lse2,
                         void* workspace, size_t workspace_bytes, streamkl_stream_t stream);
+/* Split-K with an explicit layout (NULL = streamkl_fwd_splitk): fp16, strided tensors (e.g. a [B][N][H][d] key cache), K heads shared by
+ * groups of query heads (kv_heads: decode against a grouped KV cache -- the H/HK query heads of a group stream the same K head, which
+ * HBM serves once and the L2 serves to the rest while their CTAs run together) and the ReLU student.  Partials and outputs are laid
+ * out by QUERY head as before ([B][H]...), so the workspace size does not depend on kv_heads.  fp32 runs the unsplit SIMT kernel
+ * (default layout only). */
+int streamkl_fwd_splitk_ex(const streamkl_layout* layout, const void* Q1, const void* K1, const void* Q2, const void* K2,
+                           int B, int H, int NQ, int NK, int d1, int d2, float c1, float c2, int causal, int splits,
+                           float* kl_rows, float* lse1, float* lse2,
+                           void* workspace, size_t workspace_bytes, streamkl_stream_t stream);
 /* Adaptive split selection, pure host arithmetic: P_base = B*H*ceil(NQ/128) CTAs of the default kernel;
  * returns 1 if P_base >= p_target, else min(floor(p_target/P_base), ceil(NK/128)).  p_target <= 0 means 148 = one CTA
  * per SM of a B200, i.e. one full wave (the paper's "typically 128 or 256" was for 108/132-SM parts). */

@@ -76,6 +76,8 @@ def lib() -> ctypes.CDLL:
     L.streamkl_bwd_ex.restype = ci
     L.streamkl_fwd_splitk.argtypes = [vp] * 4 + shape + [ci] + [vp] * 3 + [vp, sz, vp]
     L.streamkl_fwd_splitk.restype = ci
+    L.streamkl_fwd_splitk_ex.argtypes = [vp] + [vp] * 4 + shape + [ci] + [vp] * 3 + [vp, sz, vp]
+    L.streamkl_fwd_splitk_ex.restype = ci
     L.streamkl_fwd_splitk_splits.argtypes = [ci] * 5
     L.streamkl_fwd_splitk_splits.restype = ci
     L.streamkl_fwd_splitk_workspace_bytes.argtypes = [ci] * 4
@@ -296,15 +298,18 @@ def streamkl_fwd_splitk_workspace_bytes(B, H, NQ, splits) -> int:
     return int(lib().streamkl_fwd_splitk_workspace_bytes(B, H, NQ, int(splits)))
 
 
-def streamkl_fwd_splitk(Q1, K1, Q2, K2, c1, c2, causal, splits=0, kl_rows=None, lse1=None, lse2=None, workspace=None, stream=None):
-    """Split-K forward for small NQ (bf16).  splits <= 0: adaptive.  Returns (kl_rows, lse1, lse2)."""
+def streamkl_fwd_splitk(Q1, K1, Q2, K2, c1, c2, causal, splits=0, kl_rows=None, lse1=None, lse2=None, workspace=None, stream=None,
+                        student_activation=None):
+    """Split-K forward for small NQ.  splits <= 0: adaptive.  bf16 / fp16 inputs, possibly strided [B,H,N,d] views, K with fewer heads
+    than Q (shared K heads) and the ReLU student go through streamkl_fwd_splitk_ex.  Returns (kl_rows, lse1, lse2)."""
     import torch
 
     for n, t in (("Q1", Q1), ("K1", K1), ("Q2", Q2), ("K2", K2)):
-        _check_dev(n, t, torch.bfloat16)
+        _check_dev(n, t, Q1.dtype, strided=True)
     B, H, NQ, NK, d1, d2, HK = _shape_of(Q1, K1, Q2, K2)
-    if HK != H:
-        raise ValueError("streamkl_fwd_splitk: shared K heads are not supported")
+    layout = _layout_of(Q1, K1, Q2, K2, HK, student_activation)
+    if layout is None and Q1.dtype != torch.bfloat16:
+        raise TypeError("streamkl_fwd_splitk: bfloat16 or float16 inputs")
     outs = []
     for n, t in (("kl_rows", kl_rows), ("lse1", lse1), ("lse2", lse2)):
         if t is None:
@@ -317,10 +322,13 @@ def streamkl_fwd_splitk(Q1, K1, Q2, K2, c1, c2, causal, splits=0, kl_rows=None, 
         workspace = torch.empty(need, dtype=torch.uint8, device=Q1.device)
         _keep_alive_on(workspace, stream)
     ws_bytes = 0 if workspace is None else workspace.numel() * workspace.element_size()
+    args = (_ptr(Q1), _ptr(K1), _ptr(Q2), _ptr(K2), B, H, NQ, NK, d1, d2, float(c1), float(c2), int(bool(causal)), w,
+            _ptr(outs[0]), _ptr(outs[1]), _ptr(outs[2]), _ptr(workspace), ctypes.c_size_t(ws_bytes), _stream_handle(stream))
     with torch.cuda.device(Q1.device):
-        rc = lib().streamkl_fwd_splitk(_ptr(Q1), _ptr(K1), _ptr(Q2), _ptr(K2), B, H, NQ, NK, d1, d2, float(c1), float(c2),
-                                       int(bool(causal)), w, _ptr(outs[0]), _ptr(outs[1]), _ptr(outs[2]), _ptr(workspace),
-                                       ctypes.c_size_t(ws_bytes), _stream_handle(stream))
+        if layout is not None:
+            rc = lib().streamkl_fwd_splitk_ex(ctypes.cast(ctypes.pointer(layout), ctypes.c_void_p), *args)
+        else:
+            rc = lib().streamkl_fwd_splitk(*args)
     if rc != 0:
         raise StreamKLError(rc, "streamkl_fwd_splitk")
     return tuple(outs)

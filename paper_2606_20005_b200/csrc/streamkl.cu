@@ -526,21 +526,29 @@ size_t streamkl_fwd_splitk_workspace_bytes(int B, int H, int NQ, int splits) {
   return size_t(B) * size_t(H) * size_t(splits) * 5 * size_t(NQ) * sizeof(float);
 }
 
-int streamkl_fwd_splitk(const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1, int d2,
-                        float c1, float c2, int causal, int splits, float* kl_rows, float* lse1, float* lse2, void* workspace,
-                        size_t workspace_bytes, streamkl_stream_t stream) {
+int streamkl_fwd_splitk_ex(const streamkl_layout* layout, const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ,
+                           int NK, int d1, int d2, float c1, float c2, int causal, int splits, float* kl_rows, float* lse1, float* lse2,
+                           void* workspace, size_t workspace_bytes, streamkl_stream_t stream) {
+  const int dtype = layout ? layout->dtype : STREAMKL_BF16;
   if (splits <= 0) splits = streamkl_fwd_splitk_splits(B, H, NQ, NK, 0);
   const int tk = NK > 0 ? (NK + kFwdBK - 1) / kFwdBK : 1;
   if (splits > tk) splits = tk;
-  const bool tc = tc_dims(d1, d2);
-  if (!tc || splits <= 1)   // other head dims run the (unsplit) SIMT kernel; W = 1 is the default kernel
-    return fwd_dispatch(STREAMKL_BF16, nullptr, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
+  const bool tc = tc_dims(d1, d2) && (dtype == STREAMKL_BF16 || dtype == STREAMKL_F16);
+  if (!tc || splits <= 1)   // other head dims / fp32 run the (unsplit) SIMT kernel; W = 1 is the default kernel
+    return fwd_dispatch(dtype, layout, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
                         static_cast<cudaStream_t>(stream));
   const size_t need = streamkl_fwd_splitk_workspace_bytes(B, H, NQ, splits);
   if (need > 0 && (!workspace || workspace_bytes < need)) return STREAMKL_ERR_WORKSPACE;
   if (reinterpret_cast<uintptr_t>(workspace) & 15) return STREAMKL_ERR_ALIGN;
-  return fwd_dispatch(STREAMKL_BF16, nullptr, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
+  return fwd_dispatch(dtype, layout, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, kl_rows, lse1, lse2,
                       static_cast<cudaStream_t>(stream), splits, static_cast<float*>(workspace));
+}
+
+int streamkl_fwd_splitk(const void* Q1, const void* K1, const void* Q2, const void* K2, int B, int H, int NQ, int NK, int d1, int d2,
+                        float c1, float c2, int causal, int splits, float* kl_rows, float* lse1, float* lse2, void* workspace,
+                        size_t workspace_bytes, streamkl_stream_t stream) {
+  return streamkl_fwd_splitk_ex(nullptr, Q1, K1, Q2, K2, B, H, NQ, NK, d1, d2, c1, c2, causal, splits, kl_rows, lse1, lse2, workspace,
+                                workspace_bytes, stream);
 }
 
 size_t streamkl_fwd_splitk_noalloc_capacity(void) { return kNoAllocScratchBytes; }

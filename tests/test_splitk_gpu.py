@@ -60,3 +60,44 @@ def test_splitk_adaptive_choice_and_peaky_logits():
 
 def test_splitk_with_one_split_is_the_default_kernel():
     assert run_splitk(W.Config(63, "splitk-1", 1, 2, 16, 512, 128, 128, "bf16", False), 1) == 1
+
+
+# ---------------------------------------------------------------- split-K with a layout (streamkl_fwd_splitk_ex): NEXT-1 x NEXT-3
+# decode against a grouped KV cache is the paper's small-N_Q case: few query rows, K heads shared by groups
+# of query heads, keys stored [B][N][H][d], fp16 or bf16, optionally the ReLU student
+@pytest.mark.parametrize("NQ", [1, 16])
+@pytest.mark.parametrize("G", [4, 8])
+@pytest.mark.parametrize("dtype,act2", [("bf16", None), ("f16", None), ("bf16", "relu")])
+def test_splitk_with_shared_k_heads_strides_fp16_and_relu(NQ, G, dtype, act2):
+    import paper_2606_20005_b200 as skl
+    from test_layouts_gpu import _as_bnhd, _inputs, _ref
+
+    H, HK = 8, 8 // G
+    cfg = W.Config(64, "splitk-ex", 2, H, NQ, 4096 + 17, 128, 64, dtype, True)
+    inp = _inputs(cfg, HK)
+    ref = _ref(cfg, inp, HK, False, inp["g"], act2)
+    dev = {k: _as_bnhd(to_torch(inp[k])) for k in ("Q1", "K1", "Q2", "K2")}          # [B,H,N,d] views of [B,N,H,d] buffers
+    assert not dev["K1"].is_contiguous() and dev["K1"].shape[1] == HK
+    for splits in (7, 0):
+        kl, l1, l2 = skl.streamkl_fwd_splitk(dev["Q1"], dev["K1"], dev["Q2"], dev["K2"], cfg.c1, cfg.c2, cfg.causal, splits=splits,
+                                             student_activation=act2)
+        assert skl.streamkl_last_launch_count() == 2
+        check_fwd(to_f64(kl), to_f64(l1), to_f64(l2), ref, f"{cfg.name} NQ={NQ} G={G} {dtype} {act2} splits={splits}")
+    # the same statistics as the unsplit kernel on the same layout (fp32 merge order differs)
+    kl0, l10, l20 = skl.streamkl_fwd(dev["Q1"], dev["K1"], dev["Q2"], dev["K2"], cfg.c1, cfg.c2, cfg.causal, student_activation=act2)
+    assert np.abs(to_f64(l1) - to_f64(l10)).max() <= 1e-4 and np.abs(to_f64(l2) - to_f64(l20)).max() <= 1e-4
+    assert np.abs(to_f64(kl) - to_f64(kl0)).max() <= 3e-4
+
+
+def test_splitk_ex_wide_head_dims_and_odd_dims():
+    import paper_2606_20005_b200 as skl
+    from test_layouts_gpu import _inputs, _ref
+
+    for d1, d2 in ((192, 64), (96, 40)):
+        cfg = W.Config(65, "splitk-ex-d", 1, 4, 33, 2048 + 5, d1, d2, "f16", False)
+        inp = _inputs(cfg, 2)
+        ref = _ref(cfg, inp, 2, False, inp["g"], None)
+        dev = [to_torch(inp[k]) for k in ("Q1", "K1", "Q2", "K2")]
+        kl, l1, l2 = skl.streamkl_fwd_splitk(*dev, cfg.c1, cfg.c2, False, splits=5)
+        assert skl.streamkl_last_launch_count() == 2
+        check_fwd(to_f64(kl), to_f64(l1), to_f64(l2), ref, f"{cfg.name} d={d1}/{d2}")
