@@ -214,10 +214,12 @@ int streamkl_bwd_f32(const void* Q1, const void* K1, const void* Q2, const void*
  *                           pass for the student (dQ2, dK2: all of Setting 1 -- half the logit recomputation and exps of the
  *                           separate kernels), a second one for the teacher when dQ1, dK1 are requested.  dQ is reproducible
  *                           only up to fp32 summation order.
- *   STREAMKL_BWD_AUTO     : (default) FUSED below the measured crossover on B200 -- NQ <= 512 without teacher gradients,
- *                           NQ <= 256 with them (the paper's rule T_Q*C <= T_K, with the crossover found
- *                           independent of T_K) -- else SEPARATE.  NOTE: AUTO is therefore NOT bit-reproducible for small NQ;
- *                           select STREAMKL_BWD_SEPARATE where that matters.
+ *   STREAMKL_BWD_AUTO     : (default) FUSED where it was measured faster on B200, else SEPARATE: (a) small NQ -- NQ <= 512 without
+ *                           teacher gradients, NQ <= 256 with them (the paper's rule T_Q*C <= T_K, with the crossover
+ *                           found independent of T_K); (b) a frozen teacher with a narrow student at long context -- no teacher
+ *                           gradients, d2 <= 64, NQ >= 32768: 7-11 % faster (profiles/r03_bwd_strategies_large.md), at the price of
+ *                           the fp32 dQ2 accumulator (4*NQ*64 bytes per head) in the workspace.  NOTE: AUTO is therefore NOT
+ *                           bit-reproducible in cases (a) and (b); select STREAMKL_BWD_SEPARATE where that matters.
  * Head dims above 128 always run the owner kernels (deterministic) whatever the mode: one launch per owner side when the
  * gradient accumulators of everything requested fit TMEM together (d1 + d2 <= 256 after padding to multiples of 64, or no
  * teacher gradients), else a student launch and a teacher launch per owner side.

@@ -301,7 +301,13 @@ int launch_bwd_simt(const void* Q1, const void* K1, const void* Q2, const void* 
 // only asked for when the strategy that will run needs them.
 bool bwd_fused_selected(int NQ, bool teacher, int d1, int d2) {
   if (wide_dims(d1, d2)) return false;   // head dims above 128: owner kernels only (TMEM has no room for the dQ^T stages)
-  return g_bwd_mode == STREAMKL_BWD_FUSED || (g_bwd_mode == STREAMKL_BWD_AUTO && (NQ + 127) / 128 <= (teacher ? 2 : 4));
+  if (g_bwd_mode == STREAMKL_BWD_FUSED) return true;
+  if (g_bwd_mode != STREAMKL_BWD_AUTO) return false;
+  if ((NQ + 127) / 128 <= (teacher ? 2 : 4)) return true;   // small N_Q: the Q-owner grid is too small to fill the GPU
+  // Setting 1 with a narrow student at long context (the indexer case): the owner kernels pay two recomputations and four exps per
+  // pair for 2 d2 gradient MACs, the one-visit pass pays one and two.  Measured (profiles/r03_bwd_strategies_large.md, both run orders):
+  // d2 = 64, N >= 32K: one-visit 7-11 % faster (causal 10-11 %, unmasked 7.3-7.6 %); N = 16K: a tie; d2 = 128: within +-4 % everywhere.
+  return !teacher && pad_dim(d2) <= 64 && NQ >= 32768;
 }
 size_t fused_acc_bytes_aligned(long long BH, int NQ, int d) { return (size_t(BH) * size_t(NQ) * size_t(d) * sizeof(float) + 255) & ~size_t(255); }
 

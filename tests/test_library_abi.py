@@ -106,11 +106,18 @@ def test_workspace_is_never_quadratic(L):
 
 def test_bwd_workspace_follows_the_selected_strategy(L):
     """16 B of packed per-query scalars (rows padded to 64 per head) always; the fp32 dQ accumulators of the one-visit kernels
-    only when that strategy will run (mode FUSED, or AUTO with NQ <= 512 / <= 256 with teacher gradients) -- cfg 3 (Setting 1, NQ = 16384) needs 8 MB, not 143."""
+    only when that strategy will run (mode FUSED, or AUTO with NQ <= 512 / <= 256 with teacher gradients, or AUTO with a frozen teacher,
+    d2 <= 64 and NQ >= 32768) -- cfg 3 (Setting 1, NQ = 16384) needs 8 MB, not 143."""
     a256 = lambda n: (n + 255) // 256 * 256
     assert L.streamkl_set_bwd_mode(0) == 0   # AUTO
     assert L.streamkl_bwd_workspace_bytes(1, 32, 65536, 65536, 128, 128, 1) == 32 * 65536 * 16
     assert L.streamkl_bwd_workspace_bytes(1, 32, 16384, 16384, 128, 64, 0) == 32 * 16384 * 16              # cfg 3: 8 MB
+    # frozen teacher, d2 <= 64, NQ >= 32768 under AUTO: the one-visit student pass (measured 7-11 % faster), + fp32 dQ2
+    assert L.streamkl_bwd_workspace_bytes(1, 8, 32768, 32768, 128, 64, 0) == a256(8 * 32768 * 16) + a256(8 * 32768 * 64 * 4)
+    assert L.streamkl_bwd_workspace_bytes(1, 8, 32768, 32768, 128, 48, 0) == a256(8 * 32768 * 16) + a256(8 * 32768 * 64 * 4)   # padded to 64
+    assert L.streamkl_bwd_workspace_bytes(1, 8, 32768, 32768, 128, 64, 1) == 8 * 32768 * 16                # teacher gradients: owner kernels
+    assert L.streamkl_bwd_workspace_bytes(1, 8, 32768, 32768, 128, 128, 0) == 8 * 32768 * 16               # d2 = 128: owner kernels
+    assert L.streamkl_bwd_workspace_bytes(1, 8, 32704, 32768, 128, 64, 0) == 8 * 32704 * 16                # below 32K: owner kernels
     # NQ <= 512 under AUTO: one-visit kernels, + fp32 dQ2 (+ dQ1 with teacher gradients), each region 256-byte aligned
     assert L.streamkl_bwd_workspace_bytes(2, 3, 100, 777, 128, 64, 0) == a256(6 * 128 * 16) + a256(6 * 100 * 64 * 4)
     assert L.streamkl_bwd_workspace_bytes(2, 3, 100, 777, 128, 64, 1) == a256(6 * 128 * 16) + a256(6 * 100 * 64 * 4) + a256(6 * 100 * 128 * 4)

@@ -149,8 +149,9 @@ def whole_head_causal_by_prefix_blocks(cfg, head_inp, hidx, kl, l1, l2, dQ1, dK1
     return res
 
 
-def fullsize_case(idx: int, row_heads, n_random: int, dk_whole_head=None, dk_tail_rows: int = 0, whole_heads=()):
-    cfg = W.CONFIGS[idx]
+def fullsize_case(idx, row_heads, n_random: int, dk_whole_head=None, dk_tail_rows: int = 0, whole_heads=()):
+    cfg = idx if isinstance(idx, W.Config) else W.CONFIGS[idx]
+    idx = cfg.idx
     inp, per = gen_all(cfg)
     kl, l1, l2, dQ1, dK1, dQ2, dK2 = run_gpu(cfg, inp)
     check_global_properties(cfg, kl, l1, l2, (dQ1, dK1, dQ2, dK2))
@@ -196,3 +197,15 @@ def test_cfg4_fullsize():
 def test_cfg5_fullsize():
     """B=4,H=16,2048x131072,d=128/64,no mask, Q1 x4 (peaky): rows of 3 heads + whole-head dK of head 63 (last b, last h)."""
     fullsize_case(5, row_heads=[0, 37, 63], n_random=24, dk_whole_head=63)
+
+
+def test_long_context_narrow_student_under_auto_runs_the_one_visit_pass():
+    """cfg 3's recipe (frozen teacher d1 = 128, student d2 = 64, causal) at 32K: the size from which AUTO selects the one-visit student
+    pass for Setting 1 (profiles/r03_bwd_strategies_large.md).  Sampled rows of both heads, the dK2 of the last 512 keys, the global
+    properties -- and the workspace AUTO asks for shows which strategy ran."""
+    import paper_2606_20005_b200 as skl
+
+    cfg = W.shrink(W.CONFIGS[3], H=2, NQ=32768, NK=32768)
+    stats_only = cfg.B * cfg.H * cfg.NQ * 16
+    assert skl.streamkl_bwd_workspace_bytes(cfg.B, cfg.H, cfg.NQ, cfg.NK, cfg.d1, cfg.d2, False) == stats_only + cfg.B * cfg.H * cfg.NQ * 64 * 4
+    fullsize_case(cfg, row_heads=[0, 1], n_random=32, dk_tail_rows=512)
